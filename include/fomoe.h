@@ -1,0 +1,195 @@
+/*
+ * fomoe.h — C ABI of the B200-native skip-token MoE layer (FoMoE, arxiv/paper_2606_19025).
+ *
+ * The library implements the data-parallel hot path of a FoMoE worker's local training step: the
+ * partially resident MoE expert layer with the paper's "skip-token" rule, forward and backward, plus
+ * the kernel that packs resident-expert parameter deltas for the round-boundary sync.
+ *
+ * Citations are /root/reference/PAPER.md line numbers (section / equation).
+ *
+ * General conventions (every entry point):
+ *   - Pointers are DEVICE pointers unless the parameter is documented as "host".  The `cfg` structs and
+ *     `fomoe_route_state` themselves live on the host; the pointers inside them are device pointers.
+ *   - Every buffer is caller-owned.  The library never allocates, frees or keeps a pointer after return.
+ *     Workspace sizes come from fomoe_workspace_bytes().  All device pointers must be 16-byte aligned.
+ *   - Tensors are dense row-major.  Weights are [out,in].  Expert weights are stored ONLY for resident
+ *     experts ("the per-worker memory footprint for expert weights decreases") and are
+ *     indexed by resident slot: slot i <-> resident_ids[i].
+ *   - All work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = default stream).  No entry
+ *     point synchronises the device or copies device->host: the number of kept pairs P is never known to
+ *     the host, all data-dependent sizes are consumed on the device.
+ *   - Return value: FOMOE_OK (0) or a negative error.  Nothing throws across the ABI.  There is NO CPU
+ *     fallback: a shape the kernels do not cover returns FOMOE_ERR_UNSUPPORTED.
+ *   - dtype: FOMOE_BF16 runs the expert GEMMs on tcgen05 tensor cores (bf16 in, fp32 accumulate in TMEM)
+ *     when d_model % 64 == 0 and d_ff % 64 == 0 (otherwise, and for FOMOE_F32, fp32 SIMT kernels).
+ *     The router always accumulates in fp32 with fp32 W_r (BASELINE.json config 2 "fp32 router").
+ */
+#ifndef FOMOE_H_
+#define FOMOE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FOMOE_ABI_VERSION 1
+
+#if defined(__GNUC__)
+#define FOMOE_API __attribute__((visibility("default")))
+#else
+#define FOMOE_API
+#endif
+
+/* status codes */
+#define FOMOE_OK 0
+#define FOMOE_ERR_BADARG (-1)      /* NULL pointer, non-positive dim, top_k > E, n_res > E, misaligned pointer */
+#define FOMOE_ERR_UNSUPPORTED (-2) /* shape outside what the kernels cover (see fomoe_workspace_bytes) */
+#define FOMOE_ERR_CUDA (-3)        /* CUDA launch / API failure; text via fomoe_last_cuda_error() */
+
+/* fomoe_config.dtype: element type of x, expert weights, y, dy, dx and expert weight gradients */
+#define FOMOE_F32 0
+#define FOMOE_BF16 1
+
+/* fomoe_config.gate_fn */
+#define FOMOE_GATE_SOFTMAX 0 /* BASELINE.json: softmax over all E logits */
+#define FOMOE_GATE_SIGMOID 1 /* paper: independent sigmoid scores, PAPER.md:517 (Eq. 13), 595 (Eq. 17) */
+
+/* fomoe_config.gate_rule: what happens to the gates of surviving pairs when a selected expert is a ghost */
+#define FOMOE_DROP_ONLY 0       /* paper: survivors unchanged, skipped pairs contribute 0 */
+#define FOMOE_RENORM_TOPK 1     /* g = p / sum over all k selected (resident or not) */
+#define FOMOE_RENORM_RESIDENT 2 /* g = p / sum over the kept (resident) selected experts */
+
+typedef struct fomoe_config {
+  int32_t T;           /* tokens (batch x sequence, flattened) */
+  int32_t d_model;     /* d */
+  int32_t E;           /* routed experts N_e (router width), 1..512 */
+  int32_t top_k;       /* k, 1..min(E,32) */
+  int32_t d_ff;        /* F: hidden size of a routed SwiGLU expert */
+  int32_t n_shared;    /* always-resident shared experts, 0 if none */
+  int32_t d_ff_shared; /* hidden size of a shared expert, 0 if none */
+  int32_t dtype;       /* FOMOE_F32 | FOMOE_BF16 */
+  int32_t gate_fn;     /* FOMOE_GATE_* */
+  int32_t gate_rule;   /* FOMOE_DROP_ONLY | FOMOE_RENORM_* */
+  float temperature;   /* tau: logits = x W_r / tau + bias (PAPER.md:175 names it, gives no formula); 1 by default */
+} fomoe_config;
+
+/*
+ * Output of fomoe_route, input of fomoe_moe_fwd / fomoe_moe_bwd.  All pointers: device, caller-owned.
+ * P = number of kept (token, expert) pairs = sum_t |topk(t) ∩ S| lives only on the device (offsets[n_res]).
+ */
+typedef struct fomoe_route_state {
+  int32_t* topk_idx;  /* [T,k]  global expert ids, descending logit, ties -> lower id   (Eq. 14) */
+  float* gate;        /* [T,k]  gate weight g_tj after the gate rule; exactly 0 for skipped pairs             */
+  float* probs;       /* [T,E]  gate-function output p over all E experts (saved for backward)               */
+  int32_t* counts;    /* [n_res]    kept pairs per resident slot                                              */
+  int32_t* offsets;   /* [n_res+1]  exclusive scan of counts; offsets[n_res] = P                              */
+  int32_t* row_token; /* [T*k]  token of row r (rows slot-major, (t,j)-ascending inside a slot); r >= P: -1   */
+  int32_t* pair_row;  /* [T,k]  row of pair (t,j), or -1 if its expert is a ghost (skipped)     */
+  void* internal;     /* opaque, fomoe_workspace_bytes(...route_internal) bytes: tile-padded row layout       */
+} fomoe_route_state;
+
+/*
+ * Sizes (bytes) of the three caller-allocated workspaces for (cfg, n_res):
+ *   route_internal : fomoe_route_state.internal
+ *   saved_acts     : written by fomoe_moe_fwd, read by fomoe_moe_bwd (gathered x rows, a, u, h, o per row)
+ *   scratch        : temporary inside one fwd or bwd call (may be shared by both, and across layers)
+ * Sizes are worst case (every pair kept): rows = T*k + 127*n_res, rounded up to 128.
+ * Any out pointer may be NULL.  Returns FOMOE_ERR_BADARG / FOMOE_ERR_UNSUPPORTED for a config the library rejects.
+ */
+FOMOE_API int fomoe_workspace_bytes(const fomoe_config* cfg, int32_t n_res, size_t* route_internal, size_t* saved_acts,
+                          size_t* scratch);
+
+/*
+ * Router + gate + top-k + residency mask + permutation  (rows F1-F5 of SURVEY.md §8(a)).
+ *   z = x W_r / tau + bias over ALL E experts: the router is not partitioned (Eq. 17);
+ *   p = softmax(z) | sigmoid(z);  topk(t) = k largest z;  pair (t,j) kept iff topk_idx[t,j] in S;
+ *   gate per cfg->gate_rule;  kept pairs are permuted into per-slot groups (histogram + scan + stable scatter);
+ *   skipped pairs get no row.
+ * x            [T,d]  cfg->dtype
+ * w_router     [d,E]  fp32
+ * router_bias  [E] fp32 or NULL (load-skew device of BASELINE.json config 4; gets no gradient)
+ * resident_ids [n_res] int32 device, strictly ascending global ids in [0,E).  CONTENT is not validated
+ *              (that would need a device sync).  n_res = 0 is legal.
+ * out          all arrays written; row_token entries >= P are -1.
+ */
+FOMOE_API int fomoe_route(const fomoe_config* cfg, const void* x, const float* w_router, const float* router_bias,
+                const int32_t* resident_ids, int32_t n_res, const fomoe_route_state* out, void* stream);
+
+/*
+ * Forward (rows F6-F8): y_t = sum_{j kept} g_tj W_down,e (silu(W_gate,e x_t) ⊙ W_up,e x_t) + sum_s FFN_s(x_t)
+ *   (Eq. 13 over T(x) ∩ S; expert PAPER.md:589 in BASELINE.json's SwiGLU form; shared PAPER.md:86).
+ *   Tokens with no kept pair and no shared expert get y_t = 0 exactly.
+ * w_gate, w_up [n_res,F,d]; w_down [n_res,d,F]  (cfg->dtype; may be NULL iff n_res == 0)
+ * sh_gate, sh_up [n_shared,F_sh,d]; sh_down [n_shared,d,F_sh]  (NULL iff n_shared == 0)
+ * y [T,d] cfg->dtype, overwritten.   saved_acts, scratch: see fomoe_workspace_bytes.
+ */
+FOMOE_API int fomoe_moe_fwd(const fomoe_config* cfg, const void* x, const fomoe_route_state* route, int32_t n_res,
+                  const void* w_gate, const void* w_up, const void* w_down,
+                  const void* sh_gate, const void* sh_up, const void* sh_down,
+                  void* y, void* saved_acts, void* scratch, void* stream);
+
+/*
+ * Backward (rows B1-B7) for upstream dy [T,d]: gradients of the LOCAL graph only — ghost paths are absent from it
+ * and there is no storage for ghost-expert gradients ("each worker responsible solely for updating
+ * its local experts").  Must follow fomoe_moe_fwd with the same route and saved_acts.
+ * Outputs are OVERWRITTEN (not accumulated):
+ *   dx [T,d] cfg->dtype;  dw_router [d,E] fp32 (dense: the router is a dense parameter in skip-token mode);
+ *   dw_gate, dw_up [n_res,F,d], dw_down [n_res,d,F] cfg->dtype;  d_sh_* like their weights (NULL iff n_shared == 0).
+ */
+FOMOE_API int fomoe_moe_bwd(const fomoe_config* cfg, const void* dy, const void* x, const fomoe_route_state* route, int32_t n_res,
+                  const float* w_router, const void* w_gate, const void* w_up, const void* w_down,
+                  const void* sh_gate, const void* sh_up, const void* sh_down, const void* saved_acts,
+                  void* dx, float* dw_router, void* dw_gate, void* dw_up, void* dw_down,
+                  void* d_sh_gate, void* d_sh_up, void* d_sh_down, void* scratch, void* stream);
+
+/*
+ * Resident-delta pack (row S1): the worker's contribution to the per-expert replica-group all-reduce at a round
+ * boundary (Alg. 2 l.19).  For the b-th packed slot s = pack_slots[b] (or b if NULL):
+ *   payload[b*block + 0 ..)            = w_start_gate[s] - w_now_gate[s]     (elems_gate words)
+ *   payload[b*block + elems_gate ..)   = w_start_up[s]   - w_now_up[s]       (elems_up words)
+ *   payload[b*block + elems_gate+elems_up ..) = w_start_down[s] - w_now_down[s]  (elems_down words)
+ * block = elems_gate + elems_up + elems_down; an expert's payload is its projections, the router column is excluded
+ * in skip-token mode.  All fp32; each word is one IEEE subtraction (bit-exact vs the oracle).
+ * w_now / w_start: host arrays of 3 device pointers (gate, up, down), each [n_res, elems_*] fp32.
+ * pack_slots: [n_pack] int32 device or NULL (= all slots, n_pack must equal n_res).  elems_* must be multiples of 4.
+ */
+FOMOE_API int fomoe_pack_resident_deltas(const float* const w_now[3], const float* const w_start[3], int32_t n_res,
+                               int64_t elems_gate, int64_t elems_up, int64_t elems_down,
+                               const int32_t* pack_slots, int32_t n_pack, float* payload, void* stream);
+
+/*
+ * One whole step from HOST buffers (the end-to-end path bench.py times): copies x_host (and dy_host) to the device,
+ * runs fomoe_route + fomoe_moe_fwd + fomoe_moe_bwd, copies y and dx back.  x_host, dy_host, y_host, dx_host:
+ * HOST pointers, [T,d] cfg->dtype, ideally pinned.  x_dev, dy_dev, y_dev, dx_dev: device staging buffers [T,d].
+ * copy_stream: a second stream used to overlap the dy upload and the y download with compute (may equal stream).
+ * Everything else as in the three calls above.  Returns after enqueueing; the caller synchronises `stream`.
+ */
+FOMOE_API int fomoe_moe_step_host(const fomoe_config* cfg, const void* x_host, const void* dy_host, void* y_host, void* dx_host,
+                        void* x_dev, void* dy_dev, void* y_dev, void* dx_dev,
+                        const float* w_router, const float* router_bias, const int32_t* resident_ids, int32_t n_res,
+                        const fomoe_route_state* route,
+                        const void* w_gate, const void* w_up, const void* w_down,
+                        const void* sh_gate, const void* sh_up, const void* sh_down,
+                        float* dw_router, void* dw_gate, void* dw_up, void* dw_down,
+                        void* d_sh_gate, void* d_sh_up, void* d_sh_down,
+                        void* saved_acts, void* scratch, void* stream, void* copy_stream);
+
+/* Number of kernels the last call on this thread launched (bench.py's gpu_launches). */
+FOMOE_API int fomoe_last_launch_count(void);
+
+/* Text of the last CUDA error seen by this thread ("" if none). Host pointer, valid until the next failing call. */
+FOMOE_API const char* fomoe_last_cuda_error(void);
+
+/* FOMOE_ABI_VERSION the library was built with. */
+FOMOE_API int fomoe_abi_version(void);
+
+/* Force the fp32-accumulate SIMT kernels even where tcgen05 applies (1) or not (0); returns the previous value.
+ * Debug / A-B testing only. */
+FOMOE_API int fomoe_set_force_simt(int on);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FOMOE_H_ */

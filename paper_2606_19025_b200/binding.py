@@ -1,0 +1,175 @@
+"""Thin Python binding of libfomoe.so (include/fomoe.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI; PyTorch provides device memory and streams.
+The functions keep the C names (fomoe_route, fomoe_moe_fwd, fomoe_moe_bwd, fomoe_pack_resident_deltas,
+fomoe_moe_step_host, fomoe_workspace_bytes).  There is no CPU or eager fallback: if the shared library is missing
+or a call fails, an exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from dataclasses import dataclass
+from pathlib import Path
+from typing import Optional
+
+import torch
+
+_HERE = Path(__file__).resolve().parent
+LIB_PATH = _HERE / "libfomoe.so"
+
+FOMOE_OK, FOMOE_ERR_BADARG, FOMOE_ERR_UNSUPPORTED, FOMOE_ERR_CUDA = 0, -1, -2, -3
+FOMOE_F32, FOMOE_BF16 = 0, 1
+FOMOE_GATE_SOFTMAX, FOMOE_GATE_SIGMOID = 0, 1
+FOMOE_DROP_ONLY, FOMOE_RENORM_TOPK, FOMOE_RENORM_RESIDENT = 0, 1, 2
+
+EXPORTS = ("fomoe_workspace_bytes", "fomoe_route", "fomoe_moe_fwd", "fomoe_moe_bwd", "fomoe_pack_resident_deltas",
+           "fomoe_moe_step_host", "fomoe_last_launch_count", "fomoe_last_cuda_error", "fomoe_abi_version",
+           "fomoe_set_force_simt")
+
+
+class fomoe_config(C.Structure):
+    _fields_ = [("T", C.c_int32), ("d_model", C.c_int32), ("E", C.c_int32), ("top_k", C.c_int32), ("d_ff", C.c_int32),
+                ("n_shared", C.c_int32), ("d_ff_shared", C.c_int32), ("dtype", C.c_int32), ("gate_fn", C.c_int32),
+                ("gate_rule", C.c_int32), ("temperature", C.c_float)]
+
+
+class fomoe_route_state(C.Structure):
+    _fields_ = [("topk_idx", C.c_void_p), ("gate", C.c_void_p), ("probs", C.c_void_p), ("counts", C.c_void_p),
+                ("offsets", C.c_void_p), ("row_token", C.c_void_p), ("pair_row", C.c_void_p), ("internal", C.c_void_p)]
+
+
+class FomoeError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Loads libfomoe.so (built in-tree by paper_2606_19025_b200.build). Raises if it is missing: no fallback."""
+    global _lib
+    if _lib is None:
+        if not LIB_PATH.exists():
+            raise FomoeError(f"{LIB_PATH} is missing: build it with `python -m paper_2606_19025_b200.build` (no CPU fallback)")
+        _lib = C.CDLL(str(LIB_PATH))
+        for name in EXPORTS:
+            getattr(_lib, name).restype = C.c_int
+        _lib.fomoe_last_cuda_error.restype = C.c_char_p
+        if _lib.fomoe_abi_version() != 1:
+            raise FomoeError("libfomoe.so ABI version mismatch")
+    return _lib
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != FOMOE_OK:
+        name = {FOMOE_ERR_BADARG: "FOMOE_ERR_BADARG", FOMOE_ERR_UNSUPPORTED: "FOMOE_ERR_UNSUPPORTED",
+                FOMOE_ERR_CUDA: "FOMOE_ERR_CUDA"}.get(rc, str(rc))
+        raise FomoeError(f"{what} failed: {name} {lib().fomoe_last_cuda_error().decode()}")
+
+
+def _p(t: Optional[torch.Tensor]) -> C.c_void_p:
+    if t is None:
+        return C.c_void_p(0)
+    assert t.is_contiguous(), "tensors crossing the C ABI must be contiguous"
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream(stream=None) -> C.c_void_p:
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def make_config(T, d_model, E, top_k, d_ff, n_shared=0, d_ff_shared=0, dtype=FOMOE_BF16, gate_fn=FOMOE_GATE_SOFTMAX,
+                gate_rule=FOMOE_DROP_ONLY, temperature=1.0) -> fomoe_config:
+    return fomoe_config(T, d_model, E, top_k, d_ff, n_shared, d_ff_shared, dtype, gate_fn, gate_rule, temperature)
+
+
+def fomoe_workspace_bytes(cfg: fomoe_config, n_res: int):
+    r, a, s = C.c_size_t(0), C.c_size_t(0), C.c_size_t(0)
+    _check(lib().fomoe_workspace_bytes(C.byref(cfg), C.c_int32(n_res), C.byref(r), C.byref(a), C.byref(s)), "fomoe_workspace_bytes")
+    return r.value, a.value, s.value
+
+
+@dataclass
+class RouteState:
+    """Device tensors behind a fomoe_route_state (caller-owned, as the ABI requires)."""
+    topk_idx: torch.Tensor
+    gate: torch.Tensor
+    probs: torch.Tensor
+    counts: torch.Tensor
+    offsets: torch.Tensor
+    row_token: torch.Tensor
+    pair_row: torch.Tensor
+    internal: torch.Tensor
+
+    def c_struct(self) -> fomoe_route_state:
+        return fomoe_route_state(*(t.data_ptr() for t in (self.topk_idx, self.gate, self.probs, self.counts, self.offsets,
+                                                           self.row_token, self.pair_row, self.internal)))
+
+
+def alloc_route_state(cfg: fomoe_config, n_res: int, device="cuda") -> RouteState:
+    rb, _, _ = fomoe_workspace_bytes(cfg, n_res)
+    T, k, E = cfg.T, cfg.top_k, cfg.E
+    i32 = dict(dtype=torch.int32, device=device)
+    return RouteState(
+        topk_idx=torch.empty((T, k), **i32), gate=torch.empty((T, k), dtype=torch.float32, device=device),
+        probs=torch.empty((T, E), dtype=torch.float32, device=device), counts=torch.empty(max(n_res, 1), **i32)[:n_res],
+        offsets=torch.empty(n_res + 1, **i32), row_token=torch.empty(max(T * k, 1), **i32)[:T * k],
+        pair_row=torch.empty((T, k), **i32), internal=torch.empty(rb, dtype=torch.uint8, device=device))
+
+
+def fomoe_route(cfg, x, w_router, router_bias, resident_ids, n_res, route: RouteState, stream=None) -> None:
+    rs = route.c_struct()
+    _check(lib().fomoe_route(C.byref(cfg), _p(x), _p(w_router), _p(router_bias), _p(resident_ids), C.c_int32(n_res), C.byref(rs),
+                             _stream(stream)), "fomoe_route")
+
+
+def fomoe_moe_fwd(cfg, x, route: RouteState, n_res, w_gate, w_up, w_down, shared, y, saved_acts, scratch, stream=None) -> None:
+    rs = route.c_struct()
+    sg, su, sd = shared if shared is not None else (None, None, None)
+    _check(lib().fomoe_moe_fwd(C.byref(cfg), _p(x), C.byref(rs), C.c_int32(n_res), _p(w_gate), _p(w_up), _p(w_down), _p(sg), _p(su),
+                               _p(sd), _p(y), _p(saved_acts), _p(scratch), _stream(stream)), "fomoe_moe_fwd")
+
+
+def fomoe_moe_bwd(cfg, dy, x, route: RouteState, n_res, w_router, w_gate, w_up, w_down, shared, saved_acts, dx, dw_router, dw_gate,
+                  dw_up, dw_down, d_shared, scratch, stream=None) -> None:
+    rs = route.c_struct()
+    sg, su, sd = shared if shared is not None else (None, None, None)
+    dsg, dsu, dsd = d_shared if d_shared is not None else (None, None, None)
+    _check(lib().fomoe_moe_bwd(C.byref(cfg), _p(dy), _p(x), C.byref(rs), C.c_int32(n_res), _p(w_router), _p(w_gate), _p(w_up),
+                               _p(w_down), _p(sg), _p(su), _p(sd), _p(saved_acts), _p(dx), _p(dw_router), _p(dw_gate), _p(dw_up),
+                               _p(dw_down), _p(dsg), _p(dsu), _p(dsd), _p(scratch), _stream(stream)), "fomoe_moe_bwd")
+
+
+def fomoe_pack_resident_deltas(w_now, w_start, pack_slots, payload, stream=None) -> None:
+    """w_now / w_start: 3-tuples of fp32 device tensors [n_res, ...] (gate, up, down); payload fp32 [n_pack, block]."""
+    n_res = w_now[0].shape[0]
+    elems = [int(t[0].numel()) if n_res else 0 for t in w_now]
+    arr3 = C.c_void_p * 3
+    now = arr3(*(t.data_ptr() for t in w_now))
+    start = arr3(*(t.data_ptr() for t in w_start))
+    n_pack = n_res if pack_slots is None else int(pack_slots.numel())
+    _check(lib().fomoe_pack_resident_deltas(now, start, C.c_int32(n_res), C.c_int64(elems[0]), C.c_int64(elems[1]),
+                                            C.c_int64(elems[2]), _p(pack_slots), C.c_int32(n_pack), _p(payload), _stream(stream)),
+           "fomoe_pack_resident_deltas")
+
+
+def fomoe_moe_step_host(cfg, x_host, dy_host, y_host, dx_host, x_dev, dy_dev, y_dev, dx_dev, w_router, router_bias, resident_ids,
+                        n_res, route: RouteState, w_gate, w_up, w_down, shared, dw_router, dw_gate, dw_up, dw_down, d_shared,
+                        saved_acts, scratch, stream=None, copy_stream=None) -> None:
+    rs = route.c_struct()
+    sg, su, sd = shared if shared is not None else (None, None, None)
+    dsg, dsu, dsd = d_shared if d_shared is not None else (None, None, None)
+    _check(lib().fomoe_moe_step_host(
+        C.byref(cfg), _p(x_host), _p(dy_host), _p(y_host), _p(dx_host), _p(x_dev), _p(dy_dev), _p(y_dev), _p(dx_dev), _p(w_router),
+        _p(router_bias), _p(resident_ids), C.c_int32(n_res), C.byref(rs), _p(w_gate), _p(w_up), _p(w_down), _p(sg), _p(su), _p(sd),
+        _p(dw_router), _p(dw_gate), _p(dw_up), _p(dw_down), _p(dsg), _p(dsu), _p(dsd), _p(saved_acts), _p(scratch),
+        _stream(stream), _stream(copy_stream if copy_stream is not None else stream)), "fomoe_moe_step_host")
+
+
+def fomoe_last_launch_count() -> int:
+    return int(lib().fomoe_last_launch_count())
+
+
+def fomoe_set_force_simt(on: bool) -> bool:
+    return bool(lib().fomoe_set_force_simt(C.c_int(1 if on else 0)))

@@ -1,0 +1,202 @@
+// extern "C" entry points of libfomoe (include/fomoe.h): argument checks, workspace carving, kernel sequencing.
+#include <stdio.h>
+#include <string.h>
+
+#include "common.cuh"
+
+namespace fomoe {
+
+static thread_local char g_err[512] = "";
+static thread_local int g_launches = 0;
+static int g_force_simt = 0;
+
+void note_launch() { ++g_launches; }
+int set_cuda_error(cudaError_t e, const char* where) {
+  snprintf(g_err, sizeof(g_err), "%s: %s (%s)", where, cudaGetErrorName(e), cudaGetErrorString(e));
+  return FOMOE_ERR_CUDA;
+}
+
+static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+static int check_cfg(const fomoe_config* c, int n_res) {
+  if (!c) return FOMOE_ERR_BADARG;
+  if (c->T < 0 || c->d_model <= 0 || c->E <= 0 || c->top_k <= 0 || c->d_ff <= 0) return FOMOE_ERR_BADARG;
+  if (c->top_k > c->E || n_res < 0 || n_res > c->E) return FOMOE_ERR_BADARG;
+  if (c->n_shared < 0 || (c->n_shared > 0 && c->d_ff_shared <= 0)) return FOMOE_ERR_BADARG;
+  if (c->dtype != FOMOE_F32 && c->dtype != FOMOE_BF16) return FOMOE_ERR_BADARG;
+  if (c->gate_fn != FOMOE_GATE_SOFTMAX && c->gate_fn != FOMOE_GATE_SIGMOID) return FOMOE_ERR_BADARG;
+  if (c->gate_rule < FOMOE_DROP_ONLY || c->gate_rule > FOMOE_RENORM_RESIDENT) return FOMOE_ERR_BADARG;
+  if (!(c->temperature > 0.f)) return FOMOE_ERR_BADARG;
+  if (c->E > kMaxE || c->top_k > kMaxK) return FOMOE_ERR_UNSUPPORTED;
+  if ((long)c->T * c->top_k + (long)kTileM * (n_res + 1) > 0x7fffffffL / 2) return FOMOE_ERR_UNSUPPORTED;  // int32 row ids
+  return FOMOE_OK;
+}
+
+static bool use_umma(const fomoe_config& c) { return !g_force_simt && umma_supported(c); }
+
+}  // namespace fomoe
+
+using namespace fomoe;
+
+extern "C" {
+
+int fomoe_abi_version(void) { return FOMOE_ABI_VERSION; }
+const char* fomoe_last_cuda_error(void) { return g_err; }
+int fomoe_last_launch_count(void) { return g_launches; }
+int fomoe_set_force_simt(int on) { int p = g_force_simt; g_force_simt = on ? 1 : 0; return p; }
+
+int fomoe_workspace_bytes(const fomoe_config* cfg, int32_t n_res, size_t* route_internal, size_t* saved_acts, size_t* scratch) {
+  int rc = check_cfg(cfg, n_res);
+  if (rc != FOMOE_OK) return rc;
+  RouteWs r = carve_route_ws(*cfg, n_res, nullptr);
+  if (route_internal) *route_internal = r.bytes;
+  if (saved_acts) *saved_acts = carve_act_ws(*cfg, r.R_cap, nullptr).bytes;
+  if (scratch) *scratch = carve_scratch_ws(*cfg, r.R_cap, nullptr).bytes;
+  return FOMOE_OK;
+}
+
+int fomoe_route(const fomoe_config* cfg, const void* x, const float* w_router, const float* router_bias,
+                const int32_t* resident_ids, int32_t n_res, const fomoe_route_state* out, void* stream) {
+  g_launches = 0;
+  int rc = check_cfg(cfg, n_res);
+  if (rc != FOMOE_OK) return rc;
+  if (!out || !w_router || (!x && cfg->T > 0) || (n_res > 0 && !resident_ids)) return FOMOE_ERR_BADARG;
+  if (!out->offsets || !out->internal || (n_res > 0 && !out->counts)) return FOMOE_ERR_BADARG;
+  if (cfg->T > 0 && (!out->topk_idx || !out->gate || !out->probs || !out->row_token || !out->pair_row)) return FOMOE_ERR_BADARG;
+  if (!aligned16(x) || !aligned16(w_router) || !aligned16(out->internal)) return FOMOE_ERR_BADARG;
+  RouteWs ws = carve_route_ws(*cfg, n_res, out->internal);
+  return launch_route(*cfg, x, w_router, router_bias, resident_ids, n_res, *out, ws, (cudaStream_t)stream);
+}
+
+int fomoe_moe_fwd(const fomoe_config* cfg, const void* x, const fomoe_route_state* route, int32_t n_res, const void* w_gate,
+                  const void* w_up, const void* w_down, const void* sh_gate, const void* sh_up, const void* sh_down, void* y,
+                  void* saved_acts, void* scratch, void* stream) {
+  g_launches = 0;
+  int rc = check_cfg(cfg, n_res);
+  if (rc != FOMOE_OK) return rc;
+  if (!route || !route->internal || !saved_acts || !scratch || ((!x || !y) && cfg->T > 0)) return FOMOE_ERR_BADARG;
+  if (n_res > 0 && (!w_gate || !w_up || !w_down)) return FOMOE_ERR_BADARG;
+  if (cfg->n_shared > 0 && (!sh_gate || !sh_up || !sh_down)) return FOMOE_ERR_BADARG;
+  if (!aligned16(x) || !aligned16(y) || !aligned16(saved_acts) || !aligned16(scratch) || !aligned16(w_gate) || !aligned16(w_up) ||
+      !aligned16(w_down) || !aligned16(sh_gate) || !aligned16(sh_up) || !aligned16(sh_down))
+    return FOMOE_ERR_BADARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  RouteWs rws = carve_route_ws(*cfg, n_res, route->internal);
+  ActWs aws = carve_act_ws(*cfg, rws.R_cap, saved_acts);
+  ScratchWs sws = carve_scratch_ws(*cfg, rws.R_cap, scratch);
+  FfnPtrs w{w_gate, w_up, w_down, sh_gate, sh_up, sh_down};
+  if (cfg->T == 0) return FOMOE_OK;
+  if (n_res > 0) {
+    rc = launch_gather_rows(*cfg, x, rws, aws.xp, st);
+    if (rc != FOMOE_OK) return rc;
+  }
+  rc = use_umma(*cfg) ? umma_ffn_fwd(*cfg, n_res, x, rws, aws, sws, w, st) : simt_ffn_fwd(*cfg, n_res, x, rws, aws, sws, w, st);
+  if (rc != FOMOE_OK) return rc;
+  return launch_combine(*cfg, *route, rws, aws.o, cfg->n_shared > 0 ? sws.y_sh : nullptr, y, st);
+}
+
+int fomoe_moe_bwd(const fomoe_config* cfg, const void* dy, const void* x, const fomoe_route_state* route, int32_t n_res,
+                  const float* w_router, const void* w_gate, const void* w_up, const void* w_down, const void* sh_gate,
+                  const void* sh_up, const void* sh_down, const void* saved_acts, void* dx, float* dw_router, void* dw_gate,
+                  void* dw_up, void* dw_down, void* d_sh_gate, void* d_sh_up, void* d_sh_down, void* scratch, void* stream) {
+  g_launches = 0;
+  int rc = check_cfg(cfg, n_res);
+  if (rc != FOMOE_OK) return rc;
+  if (!route || !route->internal || !saved_acts || !scratch || !w_router || !dw_router) return FOMOE_ERR_BADARG;
+  if (cfg->T > 0 && (!dy || !x || !dx)) return FOMOE_ERR_BADARG;
+  if (n_res > 0 && (!w_gate || !w_up || !w_down || !dw_gate || !dw_up || !dw_down)) return FOMOE_ERR_BADARG;
+  if (cfg->n_shared > 0 && (!sh_gate || !sh_up || !sh_down || !d_sh_gate || !d_sh_up || !d_sh_down)) return FOMOE_ERR_BADARG;
+  if (!aligned16(dy) || !aligned16(x) || !aligned16(dx) || !aligned16(dw_router) || !aligned16(dw_gate) || !aligned16(dw_up) ||
+      !aligned16(dw_down) || !aligned16(d_sh_gate) || !aligned16(d_sh_up) || !aligned16(d_sh_down) || !aligned16(scratch) ||
+      !aligned16(saved_acts))
+    return FOMOE_ERR_BADARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  RouteWs rws = carve_route_ws(*cfg, n_res, route->internal);
+  ActWs aws = carve_act_ws(*cfg, rws.R_cap, const_cast<void*>(saved_acts));
+  ScratchWs sws = carve_scratch_ws(*cfg, rws.R_cap, scratch);
+  FfnPtrs w{w_gate, w_up, w_down, sh_gate, sh_up, sh_down};
+  // B1: do = g dy per row, dgate = <dy, o>
+  if (n_res > 0 && cfg->T > 0) {
+    rc = launch_combine_bwd(*cfg, dy, aws.o, rws, sws.dop, sws.dgate, st);
+    if (rc != FOMOE_OK) return rc;
+  } else {
+    FOMOE_CUDA_OK(cudaMemsetAsync(sws.dgate, 0, sizeof(float) * (size_t)cfg->T * cfg->top_k, st));
+  }
+  // B2-B4 (+ shared experts)
+  rc = use_umma(*cfg) ? umma_ffn_bwd(*cfg, n_res, x, dy, rws, aws, sws, w, dw_gate, dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, st)
+                      : simt_ffn_bwd(*cfg, n_res, x, dy, rws, aws, sws, w, dw_gate, dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, st);
+  if (rc != FOMOE_OK) return rc;
+  // B6, B7
+  rc = launch_gate_bwd(*cfg, *route, rws, sws.dgate, sws.dz, st);
+  if (rc != FOMOE_OK) return rc;
+  rc = simt_router_bwd(*cfg, x, w_router, sws, dw_router, st);
+  if (rc != FOMOE_OK) return rc;
+  // B5
+  return launch_dx_sum(*cfg, rws, sws.dxp, cfg->n_shared > 0 ? sws.dx_sh : nullptr, sws.dx_r, dx, st);
+}
+
+int fomoe_pack_resident_deltas(const float* const w_now[3], const float* const w_start[3], int32_t n_res, int64_t elems_gate,
+                               int64_t elems_up, int64_t elems_down, const int32_t* pack_slots, int32_t n_pack, float* payload,
+                               void* stream) {
+  g_launches = 0;
+  if (!w_now || !w_start || n_res < 0 || n_pack < 0 || elems_gate < 0 || elems_up < 0 || elems_down < 0) return FOMOE_ERR_BADARG;
+  if (!pack_slots && n_pack != n_res) return FOMOE_ERR_BADARG;
+  if (n_pack == 0) return FOMOE_OK;
+  if (!payload || !aligned16(payload)) return FOMOE_ERR_BADARG;
+  for (int i = 0; i < 3; ++i)
+    if (!w_now[i] || !w_start[i] || !aligned16(w_now[i]) || !aligned16(w_start[i])) return FOMOE_ERR_BADARG;
+  if (elems_gate % 4 || elems_up % 4 || elems_down % 4) return FOMOE_ERR_UNSUPPORTED;
+  return launch_pack(w_now, w_start, n_res, elems_gate, elems_up, elems_down, pack_slots, n_pack, payload, (cudaStream_t)stream);
+}
+
+int fomoe_moe_step_host(const fomoe_config* cfg, const void* x_host, const void* dy_host, void* y_host, void* dx_host, void* x_dev,
+                        void* dy_dev, void* y_dev, void* dx_dev, const float* w_router, const float* router_bias,
+                        const int32_t* resident_ids, int32_t n_res, const fomoe_route_state* route, const void* w_gate,
+                        const void* w_up, const void* w_down, const void* sh_gate, const void* sh_up, const void* sh_down,
+                        float* dw_router, void* dw_gate, void* dw_up, void* dw_down, void* d_sh_gate, void* d_sh_up, void* d_sh_down,
+                        void* saved_acts, void* scratch, void* stream, void* copy_stream) {
+  int rc = check_cfg(cfg, n_res);
+  if (rc != FOMOE_OK) return rc;
+  if (!x_host || !dy_host || !y_host || !dx_host || !x_dev || !dy_dev || !y_dev || !dx_dev) return FOMOE_ERR_BADARG;
+  cudaStream_t st = (cudaStream_t)stream, cs = (cudaStream_t)copy_stream;
+  const size_t bytes = (size_t)cfg->T * cfg->d_model * (cfg->dtype == FOMOE_BF16 ? 2 : 4);
+  int launches = 0;
+  cudaEvent_t ev_start, ev_dy, ev_y;
+  FOMOE_CUDA_OK(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
+  FOMOE_CUDA_OK(cudaEventCreateWithFlags(&ev_dy, cudaEventDisableTiming));
+  FOMOE_CUDA_OK(cudaEventCreateWithFlags(&ev_y, cudaEventDisableTiming));
+  // copy stream starts after everything already queued on the compute stream (previous step's consumers)
+  FOMOE_CUDA_OK(cudaEventRecord(ev_start, st));
+  FOMOE_CUDA_OK(cudaStreamWaitEvent(cs, ev_start, 0));
+  FOMOE_CUDA_OK(cudaMemcpyAsync(x_dev, x_host, bytes, cudaMemcpyHostToDevice, st));
+  FOMOE_CUDA_OK(cudaMemcpyAsync(dy_dev, dy_host, bytes, cudaMemcpyHostToDevice, cs));  // overlaps route + forward
+  FOMOE_CUDA_OK(cudaEventRecord(ev_dy, cs));
+  rc = fomoe_route(cfg, x_dev, w_router, router_bias, resident_ids, n_res, route, st);
+  launches += g_launches;
+  if (rc == FOMOE_OK) {
+    rc = fomoe_moe_fwd(cfg, x_dev, route, n_res, w_gate, w_up, w_down, sh_gate, sh_up, sh_down, y_dev, saved_acts, scratch, st);
+    launches += g_launches;
+  }
+  if (rc == FOMOE_OK) {
+    FOMOE_CUDA_OK(cudaEventRecord(ev_y, st));
+    FOMOE_CUDA_OK(cudaStreamWaitEvent(cs, ev_y, 0));
+    FOMOE_CUDA_OK(cudaMemcpyAsync(y_host, y_dev, bytes, cudaMemcpyDeviceToHost, cs));  // overlaps backward
+    FOMOE_CUDA_OK(cudaStreamWaitEvent(st, ev_dy, 0));
+    rc = fomoe_moe_bwd(cfg, dy_dev, x_dev, route, n_res, w_router, w_gate, w_up, w_down, sh_gate, sh_up, sh_down, saved_acts, dx_dev,
+                       dw_router, dw_gate, dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, scratch, st);
+    launches += g_launches;
+  }
+  if (rc == FOMOE_OK) {
+    FOMOE_CUDA_OK(cudaMemcpyAsync(dx_host, dx_dev, bytes, cudaMemcpyDeviceToHost, st));
+    // join: the step is complete on `stream` only when the y download is
+    FOMOE_CUDA_OK(cudaEventRecord(ev_y, cs));
+    FOMOE_CUDA_OK(cudaStreamWaitEvent(st, ev_y, 0));
+  }
+  cudaEventDestroy(ev_start);
+  cudaEventDestroy(ev_dy);
+  cudaEventDestroy(ev_y);
+  g_launches = launches;
+  return rc;
+}
+
+}  // extern "C"

@@ -1,0 +1,193 @@
+// Shared host/device helpers of libfomoe (sm_100a only).
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/fomoe.h"
+
+namespace fomoe {
+
+constexpr int kTileM = 128;      // rows of one expert-GEMM tile; every slot's row group is padded to this
+constexpr int kPermChunk = 1024; // (token, expert) pairs handled by one block of the permutation kernels
+constexpr int kMaxE = 512;
+constexpr int kMaxK = 32;
+
+// ---- per-thread error / launch bookkeeping (api.cu) ----
+void note_launch();
+int set_cuda_error(cudaError_t e, const char* where);
+#define FOMOE_CUDA_OK(expr)                                          \
+  do {                                                               \
+    cudaError_t e__ = (expr);                                        \
+    if (e__ != cudaSuccess) return fomoe::set_cuda_error(e__, #expr); \
+  } while (0)
+#define FOMOE_LAUNCH_OK(name)                                        \
+  do {                                                               \
+    fomoe::note_launch();                                            \
+    cudaError_t e__ = cudaGetLastError();                            \
+    if (e__ != cudaSuccess) return fomoe::set_cuda_error(e__, name);  \
+  } while (0)
+
+inline __host__ __device__ int ceil_div(int a, int b) { return (a + b - 1) / b; }
+inline __host__ __device__ size_t align_up(size_t a, size_t b) { return (a + b - 1) / b * b; }
+
+// ---- element access: storage type -> fp32 and back ----
+template <typename T> __device__ __forceinline__ float to_f32(T v);
+template <> __device__ __forceinline__ float to_f32<float>(float v) { return v; }
+template <> __device__ __forceinline__ float to_f32<__nv_bfloat16>(__nv_bfloat16 v) { return __bfloat162float(v); }
+template <typename T> __device__ __forceinline__ T from_f32(float v);
+template <> __device__ __forceinline__ float from_f32<float>(float v) { return v; }
+template <> __device__ __forceinline__ __nv_bfloat16 from_f32<__nv_bfloat16>(float v) { return __float2bfloat16_rn(v); }
+
+__device__ __forceinline__ float sigmoidf_(float v) { return 1.0f / (1.0f + __expf(-v)); }
+
+// ---- layout of fomoe_route_state.internal (all int32 unless noted), computed identically on every call ----
+struct RouteWs {
+  int32_t* slot_of;     // [E]            resident slot of expert e or -1 (ghost)
+  int32_t* blk_hist;    // [n_blk, n_res] kept pairs per (permutation block, slot); then exclusive over blocks
+  int32_t* pad_offsets; // [n_res+1]      first padded row of slot s (multiples of kTileM)
+  int32_t* n_mtiles;    // [4]            [0] = number of kTileM-row tiles in use, [1] = padded rows in use
+  int32_t* tile_slot;   // [max_mtiles]   slot of row tile i
+  int32_t* prow_token;  // [R_cap]        token of padded row r, -1 for padding rows
+  float* prow_gate;     // [R_cap]        gate of padded row r
+  int32_t* prow_pair;   // [R_cap]        t*k+j of padded row r
+  int32_t* pair_prow;   // [T*k]          padded row of pair, -1 if skipped
+  int n_blk, max_mtiles, R_cap;
+  size_t bytes;
+};
+
+inline RouteWs carve_route_ws(const fomoe_config& c, int n_res, void* base) {
+  RouteWs w{};
+  long pairs = (long)c.T * c.top_k;
+  w.n_blk = (int)((pairs + kPermChunk - 1) / kPermChunk);
+  if (w.n_blk < 1) w.n_blk = 1;
+  w.max_mtiles = (int)((pairs + kTileM - 1) / kTileM) + n_res;
+  if (w.max_mtiles < 1) w.max_mtiles = 1;
+  w.R_cap = w.max_mtiles * kTileM;
+  char* p = (char*)base;
+  size_t off = 0;
+  auto take = [&](size_t n) { void* r = p ? p + off : nullptr; off = align_up(off + n, 256); return r; };
+  w.slot_of = (int32_t*)take(sizeof(int32_t) * (size_t)c.E);
+  w.blk_hist = (int32_t*)take(sizeof(int32_t) * (size_t)w.n_blk * (size_t)(n_res > 0 ? n_res : 1));
+  w.pad_offsets = (int32_t*)take(sizeof(int32_t) * (size_t)(n_res + 1));
+  w.n_mtiles = (int32_t*)take(sizeof(int32_t) * 4);
+  w.tile_slot = (int32_t*)take(sizeof(int32_t) * (size_t)w.max_mtiles);
+  w.prow_token = (int32_t*)take(sizeof(int32_t) * (size_t)w.R_cap);
+  w.prow_gate = (float*)take(sizeof(float) * (size_t)w.R_cap);
+  w.prow_pair = (int32_t*)take(sizeof(int32_t) * (size_t)w.R_cap);
+  w.pair_prow = (int32_t*)take(sizeof(int32_t) * (size_t)(pairs > 0 ? pairs : 1));
+  w.bytes = off;
+  return w;
+}
+
+// ---- saved activations (fwd -> bwd) and scratch ----
+struct ActWs {
+  void* xp;   // [R_cap, d]   gathered token rows (zero for padding rows)
+  void* a;    // [R_cap, F]   W_gate x
+  void* u;    // [R_cap, F]   W_up x
+  void* h;    // [R_cap, F]   silu(a) * u
+  void* o;    // [R_cap, d]   W_down h
+  void* sa;   // [T, n_sh*F_sh] shared experts: a
+  void* su;   // [T, n_sh*F_sh]
+  void* sh;   // [T, n_sh*F_sh]
+  size_t bytes;
+};
+inline ActWs carve_act_ws(const fomoe_config& c, int R_cap, void* base) {
+  ActWs w{};
+  size_t es = c.dtype == FOMOE_BF16 ? 2 : 4;
+  char* p = (char*)base;
+  size_t off = 0;
+  auto take = [&](size_t n) { void* r = p ? p + off : nullptr; off = align_up(off + n, 256); return r; };
+  w.xp = take(es * (size_t)R_cap * c.d_model);
+  w.a = take(es * (size_t)R_cap * c.d_ff);
+  w.u = take(es * (size_t)R_cap * c.d_ff);
+  w.h = take(es * (size_t)R_cap * c.d_ff);
+  w.o = take(es * (size_t)R_cap * c.d_model);
+  size_t fs = (size_t)c.n_shared * c.d_ff_shared;
+  w.sa = take(es * (size_t)c.T * fs);
+  w.su = take(es * (size_t)c.T * fs);
+  w.sh = take(es * (size_t)c.T * fs);
+  w.bytes = off;
+  return w;
+}
+
+struct ScratchWs {
+  // forward
+  void* y_sh;      // [T, d]  shared-expert output (element type)
+  // backward
+  void* dop;       // [R_cap, d]  g * dy per padded row
+  void* da;        // [R_cap, F]
+  void* du;        // [R_cap, F]
+  void* dxp;       // [R_cap, d]
+  float* dgate;    // [T*k] fp32
+  float* dz;       // [T, E] fp32
+  float* dx_r;     // [T, d] fp32  router term dz W_r^T
+  void* dsa;       // [T, n_sh*F_sh]
+  void* dsu;       // [T, n_sh*F_sh]
+  void* dx_sh;     // [T, d]
+  float* dwr_part; // [kRouterSplit, d, E] fp32 split-K partials of dW_r
+  size_t bytes;
+};
+constexpr int kRouterSplit = 32;
+inline ScratchWs carve_scratch_ws(const fomoe_config& c, int R_cap, void* base) {
+  ScratchWs w{};
+  size_t es = c.dtype == FOMOE_BF16 ? 2 : 4;
+  char* p = (char*)base;
+  size_t off = 0;
+  auto take = [&](size_t n) { void* r = p ? p + off : nullptr; off = align_up(off + n, 256); return r; };
+  size_t fs = (size_t)c.n_shared * c.d_ff_shared;
+  w.y_sh = take(es * (size_t)c.T * c.d_model);
+  w.dop = take(es * (size_t)R_cap * c.d_model);
+  w.da = take(es * (size_t)R_cap * c.d_ff);
+  w.du = take(es * (size_t)R_cap * c.d_ff);
+  w.dxp = take(es * (size_t)R_cap * c.d_model);
+  w.dgate = (float*)take(sizeof(float) * (size_t)c.T * c.top_k);
+  w.dz = (float*)take(sizeof(float) * (size_t)c.T * c.E);
+  w.dx_r = (float*)take(sizeof(float) * (size_t)c.T * c.d_model);
+  w.dsa = take(es * (size_t)c.T * fs);
+  w.dsu = take(es * (size_t)c.T * fs);
+  w.dx_sh = take(es * (size_t)c.T * c.d_model);
+  w.dwr_part = (float*)take(sizeof(float) * (size_t)kRouterSplit * c.d_model * c.E);
+  w.bytes = off;
+  return w;
+}
+
+// ---- launchers implemented in the other translation units (all enqueue on `st`, return FOMOE_* status) ----
+int launch_route(const fomoe_config& c, const void* x, const float* w_router, const float* bias,
+                 const int32_t* resident_ids, int n_res, const fomoe_route_state& out, const RouteWs& ws, cudaStream_t st);
+
+// row-wise (bandwidth) kernels, rows.cu
+int launch_gather_rows(const fomoe_config& c, const void* x, const RouteWs& ws, void* xp, cudaStream_t st);
+int launch_combine(const fomoe_config& c, const fomoe_route_state& r, const RouteWs& ws, const void* o, const void* y_sh,
+                   void* y, cudaStream_t st);
+int launch_combine_bwd(const fomoe_config& c, const void* dy, const void* o, const RouteWs& ws, void* dop, float* dgate,
+                       cudaStream_t st);
+int launch_gate_bwd(const fomoe_config& c, const fomoe_route_state& r, const RouteWs& ws, const float* dgate, float* dz,
+                    cudaStream_t st);
+int launch_dx_sum(const fomoe_config& c, const RouteWs& ws, const void* dxp, const void* dx_sh, const float* dx_r, void* dx,
+                  cudaStream_t st);
+
+// fp32-accumulate SIMT GEMM path, simt_gemm.cu (all shapes, both dtypes)
+struct FfnPtrs {
+  const void *w_gate, *w_up, *w_down, *sh_gate, *sh_up, *sh_down;
+};
+int simt_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs& rws, const ActWs& aws, const ScratchWs& sws,
+                 const FfnPtrs& w, cudaStream_t st);
+int simt_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy, const RouteWs& rws, const ActWs& aws,
+                 const ScratchWs& sws, const FfnPtrs& w, void* dw_gate, void* dw_up, void* dw_down, void* d_sh_gate,
+                 void* d_sh_up, void* d_sh_down, cudaStream_t st);
+int simt_router_bwd(const fomoe_config& c, const void* x, const float* w_router, const ScratchWs& sws, float* dw_router,
+                    cudaStream_t st);
+
+// tcgen05 / TMA grouped GEMM path, umma_gemm.cu (bf16, d % 64 == 0, F % 64 == 0)
+bool umma_supported(const fomoe_config& c);
+int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs& rws, const ActWs& aws, const ScratchWs& sws,
+                 const FfnPtrs& w, cudaStream_t st);
+int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy, const RouteWs& rws, const ActWs& aws,
+                 const ScratchWs& sws, const FfnPtrs& w, void* dw_gate, void* dw_up, void* dw_down, void* d_sh_gate,
+                 void* d_sh_up, void* d_sh_down, cudaStream_t st);
+
+int launch_pack(const float* const w_now[3], const float* const w_start[3], int n_res, int64_t eg, int64_t eu, int64_t ed,
+                const int32_t* pack_slots, int n_pack, float* payload, cudaStream_t st);
+
+}  // namespace fomoe
