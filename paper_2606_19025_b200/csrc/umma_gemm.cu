@@ -1,13 +1,639 @@
-// tcgen05 / TMA grouped GEMM path (placeholder until the kernels land; the SIMT path serves every shape meanwhile).
+// tcgen05 / TMEM / TMA grouped GEMMs for the resident-expert SwiGLU FFN, forward and backward
+// (rows F6, F6s, F7, B2, B3, B4 of SURVEY.md §8(a)); bf16 operands, fp32 accumulation in tensor memory.
+//
+// One persistent, warp-specialised kernel template (one CTA per SM, 256 threads):
+//   warp 0  : TMA producer   (cp.async.bulk.tensor.2d -> 128B-swizzled shared-memory stages, mbarrier complete_tx)
+//   warp 1  : MMA issuer     (one elected lane issues tcgen05.mma.cta_group::1.kind::f16, M=128 N=256 K=16)
+//   warp 2  : TMEM allocator (512 columns = two 128x256 fp32 accumulator stages)
+//   warps 4-7: epilogue      (tcgen05.ld 32x32b -> registers -> fused math -> 16-byte global stores)
+// Three pipelines: shared-memory full/empty (TMA <-> MMA), TMEM full/empty (MMA <-> epilogue), static round-robin
+// tile scheduler.  The number of row tiles is data dependent and is read from device memory (route workspace): the
+// host never learns P.
+//
+// Modes (all with a 128 x 256 accumulator tile, K staged 64 at a time):
+//   FWD1  [a|u] = X W_gate^T | X W_up^T   (A, B K-major; epilogue: a, u, h = silu(a)*u)
+//   FWD2  o = H W_down^T                  (A, B K-major)
+//   DH    dh = dO W_down                  (A K-major, B MN-major; epilogue: SwiGLU backward -> da, du)
+//   DX    dxp = dA W_gate + dU W_up       (A K-major, B MN-major; two K segments into one accumulator)
+//   WGRAD dW[g] = A[rows(g)]^T B[rows(g)] (A, B MN-major; K = the group's (padded) rows)
+// Row space is either the tile-padded routed rows (slot per 128-row tile) or dense rows (shared experts).
+#include <cuda.h>
+
 #include "common.cuh"
 
 namespace fomoe {
-bool umma_supported(const fomoe_config&) { return false; }
-int umma_ffn_fwd(const fomoe_config&, int, const void*, const RouteWs&, const ActWs&, const ScratchWs&, const FfnPtrs&, cudaStream_t) {
-  return FOMOE_ERR_UNSUPPORTED;
+namespace {
+
+using bf16 = __nv_bfloat16;
+
+constexpr int BM = 128, BN = 256, BK = 64, kStages = 4, kAccStages = 2;
+constexpr int kABytes = BM * BK * 2, kBBytes = BN * BK * 2, kStageBytes = kABytes + kBBytes;
+constexpr int kThreads = 256;
+constexpr int kSmemBytes = kStages * kStageBytes + 1024 /*align*/ + 256 /*barriers*/;
+constexpr int kTmemCols = 512;
+
+enum Mode { FWD1 = 0, FWD2 = 1, DH = 2, DX = 3, WGRAD = 4 };
+
+struct TmaMaps {
+  CUtensorMap m[4];
+};
+
+struct UmmaParams {
+  const int32_t* n_mtiles;     // routed: device, [0] = row tiles in use; nullptr = dense rows
+  const int32_t* tile_slot;    // routed: slot of row tile
+  const int32_t* pad_offsets;  // routed WGRAD: padded row range of group g
+  int dense_rows;              // dense: number of rows (T)
+  int parts;                   // dense: number of shared experts (1 for routed)
+  int n_groups;                // WGRAD: number of groups (n_res or n_shared)
+  int d, F;                    // model width; per-expert hidden width
+  int ld;                      // leading dimension of the [rows, hidden] activations (F, or parts*F for dense)
+  int M, N;                    // WGRAD: output rows / cols per group
+  int a_gcol, b_gcol;          // WGRAD dense: per-group column offset into A / B
+  bf16 *out0, *out1, *out2;    // FWD1: a,u,h | FWD2/DX: out | DH: da,du | WGRAD: dW
+  const bf16 *in0, *in1;       // DH: a,u
+};
+
+// ---------------------------------------------------------------------------------------------------------
+// PTX wrappers
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
-int umma_ffn_bwd(const fomoe_config&, int, const void*, const void*, const RouteWs&, const ActWs&, const ScratchWs&, const FfnPtrs&,
-                 void*, void*, void*, void*, void*, void*, cudaStream_t) {
-  return FOMOE_ERR_UNSUPPORTED;
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  do {
+    asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+               ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(bar), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void prefetch_tmap(const CUtensorMap* map) {
+  asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(map)) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// shared-memory matrix descriptor, 128-byte swizzle, Blackwell version field = 1
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  uint64_t dsc = 0;
+  dsc |= (uint64_t)((saddr & 0x3FFFFu) >> 4);
+  dsc |= (uint64_t)(lbo_bytes >> 4) << 16;
+  dsc |= (uint64_t)(sbo_bytes >> 4) << 32;
+  dsc |= (uint64_t)1 << 46;
+  dsc |= (uint64_t)2 << 61;
+  return dsc;
+}
+__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}"
+               ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32]) {
+  uint32_t* r = reinterpret_cast<uint32_t*>(v);
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+        "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]),
+        "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]),
+        "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+__device__ __forceinline__ void store_bf16x32(bf16* dst, const float (&v)[32]) {
+  uint4* p = reinterpret_cast<uint4*>(dst);
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    uint4 w;
+    __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&w);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) h[i] = __floats2bfloat162_rn(v[q * 8 + 2 * i], v[q * 8 + 2 * i + 1]);
+    p[q] = w;
+  }
+}
+__device__ __forceinline__ void load_bf16x32(const bf16* src, float (&v)[32]) {
+  const uint4* p = reinterpret_cast<const uint4*>(src);
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    uint4 w = p[q];
+    const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&w);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      float2 f = __bfloat1622float2(h[i]);
+      v[q * 8 + 2 * i] = f.x;
+      v[q * 8 + 2 * i + 1] = f.y;
+    }
+  }
+}
+
+// instruction descriptor: D fp32, A/B bf16, M=128, N=256, majorness per operand (0 = K-major, 1 = MN-major)
+__host__ __device__ constexpr uint32_t make_idesc(int a_mn, int b_mn) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)a_mn << 15) | ((uint32_t)b_mn << 16) | ((uint32_t)(BN >> 3) << 17) |
+         ((uint32_t)(BM >> 4) << 24);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// tile decode shared by the three roles
+// ---------------------------------------------------------------------------------------------------------
+struct Tile {
+  int m_tile, n_tile, slot, part, group;  // group: WGRAD only
+  int num_kb;                             // 64-wide K blocks
+  int k_row0;                             // WGRAD: first row of the K range
+};
+
+template <int MODE>
+struct Sched {
+  const UmmaParams& p;
+  int n_tiles_n, ntn_total, m_tiles;
+  long total;
+  __device__ Sched(const UmmaParams& p_) : p(p_) {
+    const bool dense = p.n_mtiles == nullptr;
+    if (MODE == WGRAD) {
+      m_tiles = (p.M + BM - 1) / BM;
+      n_tiles_n = (p.N + BN - 1) / BN;
+      ntn_total = n_tiles_n;
+      total = (long)p.n_groups * m_tiles * n_tiles_n;
+    } else {
+      m_tiles = dense ? (p.dense_rows + BM - 1) / BM : p.n_mtiles[0];
+      const int n_extent = (MODE == FWD1 || MODE == DH) ? p.F : p.d;
+      const int bn = MODE == FWD1 ? BN / 2 : BN;
+      n_tiles_n = (n_extent + bn - 1) / bn;
+      ntn_total = n_tiles_n * ((dense && (MODE == FWD1 || MODE == DH)) ? p.parts : 1);
+      total = (long)m_tiles * ntn_total;
+    }
+  }
+  __device__ Tile decode(long id) const {
+    Tile t;
+    const bool dense = p.n_mtiles == nullptr;
+    if (MODE == WGRAD) {
+      t.group = (int)(id / ((long)m_tiles * n_tiles_n));
+      int rem = (int)(id % ((long)m_tiles * n_tiles_n));
+      t.m_tile = rem / n_tiles_n;
+      t.n_tile = rem % n_tiles_n;
+      t.slot = t.part = t.group;
+      int r0, r1;
+      if (p.pad_offsets) { r0 = p.pad_offsets[t.group]; r1 = p.pad_offsets[t.group + 1]; }
+      else { r0 = 0; r1 = p.dense_rows; }
+      t.k_row0 = r0;
+      t.num_kb = (r1 - r0 + BK - 1) / BK;
+    } else {
+      t.m_tile = (int)(id / ntn_total);
+      int nidx = (int)(id % ntn_total);
+      t.part = nidx / n_tiles_n;
+      t.n_tile = nidx % n_tiles_n;
+      t.slot = dense ? t.part : p.tile_slot[t.m_tile];
+      t.group = 0;
+      t.k_row0 = 0;
+      const int kparts = dense ? p.parts : 1;
+      if (MODE == FWD1 || MODE == DH) t.num_kb = p.d / BK;
+      else if (MODE == FWD2) t.num_kb = kparts * (p.F / BK);
+      else t.num_kb = 2 * kparts * (p.F / BK);  // DX
+    }
+    return t;
+  }
+};
+
+// ---------------------------------------------------------------------------------------------------------
+// the kernel
+// ---------------------------------------------------------------------------------------------------------
+template <int MODE>
+__global__ void __launch_bounds__(kThreads, 1)
+umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kStages * kStageBytes);
+  uint64_t* full_bar = bars;                          // [kStages]
+  uint64_t* empty_bar = bars + kStages;               // [kStages]
+  uint64_t* tfull_bar = bars + 2 * kStages;           // [kAccStages]
+  uint64_t* tempty_bar = bars + 2 * kStages + kAccStages;  // [kAccStages]
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * kStages + 2 * kAccStages);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  constexpr bool kAMn = (MODE == WGRAD), kBMn = (MODE == DH || MODE == DX || MODE == WGRAD);
+
+  if (warp == 0 && lane == 0) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) prefetch_tmap(&maps.m[i]);
+  }
+  if (warp == 1 && lane == 0) {
+    for (int i = 0; i < kStages; ++i) { mbar_init(smem_u32(&full_bar[i]), 1); mbar_init(smem_u32(&empty_bar[i]), 1); }
+    for (int i = 0; i < kAccStages; ++i) { mbar_init(smem_u32(&tfull_bar[i]), 1); mbar_init(smem_u32(&tempty_bar[i]), 4); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 2) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "n"(kTmemCols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  const Sched<MODE> sched(p);
+  const bool dense = p.n_mtiles == nullptr;
+
+  if (warp == 0) {
+    // ===================== TMA producer =====================
+    if (lane == 0) {
+      int stage = 0;
+      uint32_t phase = 0;
+      for (long id = blockIdx.x; id < sched.total; id += gridDim.x) {
+        const Tile t = sched.decode(id);
+        const int m0 = t.m_tile * BM;
+        for (int kb = 0; kb < t.num_kb; ++kb) {
+          mbar_wait(smem_u32(&empty_bar[stage]), phase ^ 1);
+          const uint32_t sa = smem_u32(smem + stage * kStageBytes), sb = sa + kABytes, fb = smem_u32(&full_bar[stage]);
+          mbar_expect_tx(fb, kStageBytes);
+          if (MODE == FWD1) {
+            tma_load_2d(sa, &maps.m[0], fb, kb * BK, m0);
+            const int brow = t.slot * p.F + t.n_tile * (BN / 2);
+            tma_load_2d(sb, &maps.m[1], fb, kb * BK, brow);
+            tma_load_2d(sb + kBBytes / 2, &maps.m[2], fb, kb * BK, brow);
+          } else if (MODE == FWD2) {
+            const int kpp = p.F / BK, part = kb / kpp, kk = kb % kpp;
+            tma_load_2d(sa, &maps.m[0], fb, part * p.F + kk * BK, m0);
+            tma_load_2d(sb, &maps.m[1], fb, kk * BK, (dense ? part : t.slot) * p.d + t.n_tile * BN);
+          } else if (MODE == DH) {
+            tma_load_2d(sa, &maps.m[0], fb, kb * BK, m0);
+#pragma unroll
+            for (int j = 0; j < BN / 64; ++j)
+              tma_load_2d(sb + j * 8192, &maps.m[1], fb, t.n_tile * BN + 64 * j, t.slot * p.d + kb * BK);
+          } else if (MODE == DX) {
+            const int kseg = (dense ? p.parts : 1) * (p.F / BK), seg = kb / kseg, kk = kb % kseg;
+            tma_load_2d(sa, &maps.m[seg], fb, kk * BK, m0);
+            const int brow = (dense ? 0 : t.slot * p.F) + kk * BK;
+#pragma unroll
+            for (int j = 0; j < BN / 64; ++j) tma_load_2d(sb + j * 8192, &maps.m[2 + seg], fb, t.n_tile * BN + 64 * j, brow);
+          } else {  // WGRAD
+            const int r = t.k_row0 + kb * BK;
+#pragma unroll
+            for (int i = 0; i < BM / 64; ++i) tma_load_2d(sa + i * 8192, &maps.m[0], fb, t.group * p.a_gcol + m0 + 64 * i, r);
+#pragma unroll
+            for (int j = 0; j < BN / 64; ++j)
+              tma_load_2d(sb + j * 8192, &maps.m[1], fb, t.group * p.b_gcol + t.n_tile * BN + 64 * j, r);
+          }
+          if (++stage == kStages) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer =====================
+    constexpr uint32_t idesc = make_idesc(kAMn ? 1 : 0, kBMn ? 1 : 0);
+    int stage = 0, as = 0;
+    uint32_t phase = 0, aphase = 0;
+    for (long id = blockIdx.x; id < sched.total; id += gridDim.x) {
+      const Tile t = sched.decode(id);
+      if (t.num_kb == 0) continue;  // empty WGRAD group: the epilogue writes zeros without touching TMEM
+      mbar_wait(smem_u32(&tempty_bar[as]), aphase ^ 1);
+      tc_fence_after();
+      const uint32_t tmem_d = tmem_base + as * BN;
+      for (int kb = 0; kb < t.num_kb; ++kb) {
+        mbar_wait(smem_u32(&full_bar[stage]), phase);
+        tc_fence_after();
+        if (lane == 0) {
+          const uint32_t sa = smem_u32(smem + stage * kStageBytes), sb = sa + kABytes;
+#pragma unroll
+          for (int k = 0; k < BK / 16; ++k) {
+            // K-major: 16 K-elements = 32 bytes inside the 128-byte swizzle row, row groups 1024 B apart.
+            // MN-major: 16 K-rows = two 8-row swizzle atoms (2 x 1024 B); 64-element MN chunks 8192 B apart.
+            const uint64_t adesc = kAMn ? make_desc(sa + k * 2048, 8192, 1024) : make_desc(sa + k * 32, 16, 1024);
+            const uint64_t bdesc = kBMn ? make_desc(sb + k * 2048, 8192, 1024) : make_desc(sb + k * 32, 16, 1024);
+            umma_bf16(tmem_d, adesc, bdesc, idesc, (kb | k) != 0 ? 1u : 0u);
+          }
+          umma_commit(smem_u32(&empty_bar[stage]));                       // frees the smem stage when these MMAs retire
+          if (kb == t.num_kb - 1) umma_commit(smem_u32(&tfull_bar[as]));  // accumulator complete
+        }
+        __syncwarp();
+        if (++stage == kStages) { stage = 0; phase ^= 1; }
+      }
+      if (++as == kAccStages) { as = 0; aphase ^= 1; }
+    }
+  } else if (warp >= 4) {
+    // ===================== epilogue =====================
+    const int q = warp & 3;             // TMEM lane quarter of this warp
+    const int r_in_tile = q * 32 + lane;
+    int as = 0;
+    uint32_t aphase = 0;
+    for (long id = blockIdx.x; id < sched.total; id += gridDim.x) {
+      const Tile t = sched.decode(id);
+      const bool have_acc = t.num_kb > 0;
+      if (have_acc) {
+        mbar_wait(smem_u32(&tfull_bar[as]), aphase);
+        tc_fence_after();
+      }
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * BN;
+      if (MODE == WGRAD) {
+        const int m = t.m_tile * BM + r_in_tile;
+        bf16* orow = p.out0 + ((size_t)t.group * p.M + m) * p.N;
+#pragma unroll 1
+        for (int cc = 0; cc < BN / 32; ++cc) {
+          float v[32];
+          if (have_acc) { tmem_ld32(taddr + cc * 32, v); tmem_ld_wait(); }
+          else {
+#pragma unroll
+            for (int i = 0; i < 32; ++i) v[i] = 0.f;
+          }
+          const int n = t.n_tile * BN + cc * 32;
+          if (m < p.M && n < p.N) store_bf16x32(orow + n, v);
+        }
+      } else {
+        const int row = t.m_tile * BM + r_in_tile;
+        const bool row_ok = dense ? row < p.dense_rows : true;
+        if (MODE == FWD1) {
+          const size_t base = (size_t)row * p.ld + (size_t)t.part * p.F;
+#pragma unroll 1
+          for (int cc = 0; cc < (BN / 2) / 32; ++cc) {
+            float a[32], u[32];
+            tmem_ld32(taddr + cc * 32, a);
+            tmem_ld32(taddr + BN / 2 + cc * 32, u);
+            tmem_ld_wait();
+            const int n = t.n_tile * (BN / 2) + cc * 32;
+            if (row_ok && n < p.F) {
+              store_bf16x32(p.out0 + base + n, a);
+              store_bf16x32(p.out1 + base + n, u);
+#pragma unroll
+              for (int i = 0; i < 32; ++i) a[i] = __fdividef(a[i], 1.0f + __expf(-a[i])) * u[i];
+              store_bf16x32(p.out2 + base + n, a);
+            }
+          }
+        } else if (MODE == DH) {
+          const size_t base = (size_t)row * p.ld + (size_t)t.part * p.F;
+#pragma unroll 1
+          for (int cc = 0; cc < BN / 32; ++cc) {
+            float dh[32];
+            tmem_ld32(taddr + cc * 32, dh);
+            tmem_ld_wait();
+            const int n = t.n_tile * BN + cc * 32;
+            if (row_ok && n < p.F) {
+              float a[32], u[32];
+              load_bf16x32(p.in0 + base + n, a);
+              load_bf16x32(p.in1 + base + n, u);
+#pragma unroll
+              for (int i = 0; i < 32; ++i) {
+                const float s = __fdividef(1.0f, 1.0f + __expf(-a[i]));
+                const float da = dh[i] * u[i] * s * (1.0f + a[i] * (1.0f - s));
+                u[i] = dh[i] * a[i] * s;  // du
+                a[i] = da;
+              }
+              store_bf16x32(p.out0 + base + n, a);
+              store_bf16x32(p.out1 + base + n, u);
+            }
+          }
+        } else {  // FWD2, DX: plain store of a [rows, d] tile
+#pragma unroll 1
+          for (int cc = 0; cc < BN / 32; ++cc) {
+            float v[32];
+            tmem_ld32(taddr + cc * 32, v);
+            tmem_ld_wait();
+            const int n = t.n_tile * BN + cc * 32;
+            if (row_ok && n < p.d) store_bf16x32(p.out0 + (size_t)row * p.d + n, v);
+          }
+        }
+      }
+      if (have_acc) {
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&tempty_bar[as]));
+        if (++as == kAccStages) { as = 0; aphase ^= 1; }
+      }
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 2) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kTmemCols) : "memory");
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// host side: tensor maps and launches
+// ---------------------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode() {
+  static EncodeTiledFn fn = [] {
+    void* ptr = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
+      ptr = nullptr;
+    return (EncodeTiledFn)ptr;
+  }();
+  return fn;
+}
+
+// 2D bf16 tensor [rows, inner] row-major with row stride `ld` elements; box = 64 inner elements x box_rows rows; 128B swizzle.
+bool make_map(CUtensorMap* m, const void* ptr, uint64_t inner, uint64_t rows, uint64_t ld, uint32_t box_rows) {
+  EncodeTiledFn enc = get_encode();
+  if (!enc) return false;
+  if (rows == 0) rows = 1;
+  cuuint64_t gdim[2] = {inner, rows};
+  cuuint64_t gstride[1] = {ld * 2};
+  cuuint32_t box[2] = {64, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS;
+}
+
+int num_sms() {
+  static int n = [] {
+    int dev = 0, v = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
+    return v;
+  }();
+  return n;
+}
+
+template <int MODE>
+int launch(const TmaMaps& maps, const UmmaParams& p, cudaStream_t st, const char* name) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    FOMOE_CUDA_OK(cudaFuncSetAttribute(umma_grouped_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
+    attr_set = true;
+  }
+  umma_grouped_kernel<MODE><<<num_sms(), kThreads, kSmemBytes, st>>>(maps, p);
+  FOMOE_LAUNCH_OK(name);
+  return FOMOE_OK;
+}
+
+#define MAP_OK(expr) \
+  do { if (!(expr)) return set_cuda_error(cudaErrorInvalidValue, "cuTensorMapEncodeTiled " #expr); } while (0)
+
+}  // namespace
+
+bool umma_supported(const fomoe_config& c) {
+  if (c.dtype != FOMOE_BF16) return false;
+  if (c.d_model % 64 || c.d_ff % 64) return false;
+  if (c.n_shared > 0 && c.d_ff_shared % 64) return false;
+  return true;
+}
+
+int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs& rws, const ActWs& aws, const ScratchWs& sws,
+                 const FfnPtrs& w, cudaStream_t st) {
+  const int d = c.d_model, F = c.d_ff;
+  if (n_res > 0 && c.T > 0) {
+    const uint64_t R = (uint64_t)rws.R_cap;
+    UmmaParams p{};
+    p.n_mtiles = rws.n_mtiles; p.tile_slot = rws.tile_slot; p.parts = 1; p.d = d; p.F = F; p.ld = F;
+    {
+      TmaMaps m{};
+      MAP_OK(make_map(&m.m[0], aws.xp, d, R, d, 128));
+      MAP_OK(make_map(&m.m[1], w.w_gate, d, (uint64_t)n_res * F, d, 128));
+      MAP_OK(make_map(&m.m[2], w.w_up, d, (uint64_t)n_res * F, d, 128));
+      m.m[3] = m.m[0];
+      UmmaParams q = p;
+      q.out0 = (bf16*)aws.a; q.out1 = (bf16*)aws.u; q.out2 = (bf16*)aws.h;
+      int rc = launch<FWD1>(m, q, st, "umma_grouped_kernel<FWD1>");
+      if (rc != FOMOE_OK) return rc;
+    }
+    {
+      TmaMaps m{};
+      MAP_OK(make_map(&m.m[0], aws.h, F, R, F, 128));
+      MAP_OK(make_map(&m.m[1], w.w_down, F, (uint64_t)n_res * d, F, 256));
+      m.m[2] = m.m[3] = m.m[0];
+      UmmaParams q = p;
+      q.out0 = (bf16*)aws.o;
+      int rc = launch<FWD2>(m, q, st, "umma_grouped_kernel<FWD2>");
+      if (rc != FOMOE_OK) return rc;
+    }
+  }
+  if (c.n_shared > 0 && c.T > 0) {
+    const int Fs = c.d_ff_shared, ns = c.n_shared, ld = ns * Fs;
+    UmmaParams p{};
+    p.dense_rows = c.T; p.parts = ns; p.d = d; p.F = Fs; p.ld = ld;
+    {
+      TmaMaps m{};
+      MAP_OK(make_map(&m.m[0], x, d, c.T, d, 128));
+      MAP_OK(make_map(&m.m[1], w.sh_gate, d, (uint64_t)ns * Fs, d, 128));
+      MAP_OK(make_map(&m.m[2], w.sh_up, d, (uint64_t)ns * Fs, d, 128));
+      m.m[3] = m.m[0];
+      UmmaParams q = p;
+      q.out0 = (bf16*)aws.sa; q.out1 = (bf16*)aws.su; q.out2 = (bf16*)aws.sh;
+      int rc = launch<FWD1>(m, q, st, "umma_grouped_kernel<FWD1,shared>");
+      if (rc != FOMOE_OK) return rc;
+    }
+    {
+      TmaMaps m{};
+      MAP_OK(make_map(&m.m[0], aws.sh, ld, c.T, ld, 128));
+      MAP_OK(make_map(&m.m[1], w.sh_down, Fs, (uint64_t)ns * d, Fs, 256));
+      m.m[2] = m.m[3] = m.m[0];
+      UmmaParams q = p;
+      q.out0 = (bf16*)sws.y_sh;
+      int rc = launch<FWD2>(m, q, st, "umma_grouped_kernel<FWD2,shared>");
+      if (rc != FOMOE_OK) return rc;
+    }
+  }
+  return FOMOE_OK;
+}
+
+int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy, const RouteWs& rws, const ActWs& aws,
+                 const ScratchWs& sws, const FfnPtrs& w, void* dw_gate, void* dw_up, void* dw_down, void* d_sh_gate,
+                 void* d_sh_up, void* d_sh_down, cudaStream_t st) {
+  const int d = c.d_model, F = c.d_ff;
+  if (n_res > 0) {
+    const uint64_t R = (uint64_t)rws.R_cap;
+    UmmaParams p{};
+    p.n_mtiles = rws.n_mtiles; p.tile_slot = rws.tile_slot; p.pad_offsets = rws.pad_offsets; p.parts = 1; p.d = d; p.F = F; p.ld = F;
+    if (c.T > 0) {
+      {  // dh = dO W_down, fused SwiGLU backward
+        TmaMaps m{};
+        MAP_OK(make_map(&m.m[0], sws.dop, d, R, d, 128));
+        MAP_OK(make_map(&m.m[1], w.w_down, F, (uint64_t)n_res * d, F, 64));
+        m.m[2] = m.m[3] = m.m[0];
+        UmmaParams q = p;
+        q.in0 = (const bf16*)aws.a; q.in1 = (const bf16*)aws.u; q.out0 = (bf16*)sws.da; q.out1 = (bf16*)sws.du;
+        int rc = launch<DH>(m, q, st, "umma_grouped_kernel<DH>");
+        if (rc != FOMOE_OK) return rc;
+      }
+      {  // dxp = dA W_gate + dU W_up
+        TmaMaps m{};
+        MAP_OK(make_map(&m.m[0], sws.da, F, R, F, 128));
+        MAP_OK(make_map(&m.m[1], sws.du, F, R, F, 128));
+        MAP_OK(make_map(&m.m[2], w.w_gate, d, (uint64_t)n_res * F, d, 64));
+        MAP_OK(make_map(&m.m[3], w.w_up, d, (uint64_t)n_res * F, d, 64));
+        UmmaParams q = p;
+        q.out0 = (bf16*)sws.dxp;
+        int rc = launch<DX>(m, q, st, "umma_grouped_kernel<DX>");
+        if (rc != FOMOE_OK) return rc;
+      }
+    }
+    // weight gradients, K = the slot's padded rows (padding rows are zero)
+    struct WG { const void* A; int lda; const void* B; int ldb; int M, N; void* out; };
+    const WG jobs[3] = {{sws.dop, d, aws.h, F, d, F, dw_down}, {sws.da, F, aws.xp, d, F, d, dw_gate}, {sws.du, F, aws.xp, d, F, d, dw_up}};
+    for (const WG& j : jobs) {
+      TmaMaps m{};
+      MAP_OK(make_map(&m.m[0], j.A, j.lda, R, j.lda, 64));
+      MAP_OK(make_map(&m.m[1], j.B, j.ldb, R, j.ldb, 64));
+      m.m[2] = m.m[3] = m.m[0];
+      UmmaParams q = p;
+      q.n_groups = n_res; q.M = j.M; q.N = j.N; q.a_gcol = 0; q.b_gcol = 0; q.out0 = (bf16*)j.out;
+      int rc = launch<WGRAD>(m, q, st, "umma_grouped_kernel<WGRAD>");
+      if (rc != FOMOE_OK) return rc;
+    }
+  }
+  if (c.n_shared > 0 && c.T == 0) {  // empty batch: exact zeros
+    const size_t n = sizeof(bf16) * (size_t)c.n_shared * c.d_ff_shared * d;
+    FOMOE_CUDA_OK(cudaMemsetAsync(d_sh_gate, 0, n, st));
+    FOMOE_CUDA_OK(cudaMemsetAsync(d_sh_up, 0, n, st));
+    FOMOE_CUDA_OK(cudaMemsetAsync(d_sh_down, 0, n, st));
+  } else if (c.n_shared > 0) {
+    const int Fs = c.d_ff_shared, ns = c.n_shared, ld = ns * Fs;
+    UmmaParams p{};
+    p.dense_rows = c.T; p.parts = ns; p.d = d; p.F = Fs; p.ld = ld;
+    if (c.T > 0) {
+      {
+        TmaMaps m{};
+        MAP_OK(make_map(&m.m[0], dy, d, c.T, d, 128));
+        MAP_OK(make_map(&m.m[1], w.sh_down, Fs, (uint64_t)ns * d, Fs, 64));
+        m.m[2] = m.m[3] = m.m[0];
+        UmmaParams q = p;
+        q.in0 = (const bf16*)aws.sa; q.in1 = (const bf16*)aws.su; q.out0 = (bf16*)sws.dsa; q.out1 = (bf16*)sws.dsu;
+        int rc = launch<DH>(m, q, st, "umma_grouped_kernel<DH,shared>");
+        if (rc != FOMOE_OK) return rc;
+      }
+      {
+        TmaMaps m{};
+        MAP_OK(make_map(&m.m[0], sws.dsa, ld, c.T, ld, 128));
+        MAP_OK(make_map(&m.m[1], sws.dsu, ld, c.T, ld, 128));
+        MAP_OK(make_map(&m.m[2], w.sh_gate, d, (uint64_t)ns * Fs, d, 64));
+        MAP_OK(make_map(&m.m[3], w.sh_up, d, (uint64_t)ns * Fs, d, 64));
+        UmmaParams q = p;
+        q.out0 = (bf16*)sws.dx_sh;
+        int rc = launch<DX>(m, q, st, "umma_grouped_kernel<DX,shared>");
+        if (rc != FOMOE_OK) return rc;
+      }
+    }
+    struct WG { const void* A; int lda; int a_gcol; const void* B; int ldb; int b_gcol; int M, N; void* out; };
+    const WG jobs[3] = {{dy, d, 0, aws.sh, ld, Fs, d, Fs, d_sh_down},
+                        {sws.dsa, ld, Fs, x, d, 0, Fs, d, d_sh_gate},
+                        {sws.dsu, ld, Fs, x, d, 0, Fs, d, d_sh_up}};
+    for (const WG& j : jobs) {
+      TmaMaps m{};
+      MAP_OK(make_map(&m.m[0], j.A, j.lda, c.T, j.lda, 64));
+      MAP_OK(make_map(&m.m[1], j.B, j.ldb, c.T, j.ldb, 64));
+      m.m[2] = m.m[3] = m.m[0];
+      UmmaParams q = p;
+      q.n_groups = ns; q.M = j.M; q.N = j.N; q.a_gcol = j.a_gcol; q.b_gcol = j.b_gcol; q.out0 = (bf16*)j.out;
+      int rc = launch<WGRAD>(m, q, st, "umma_grouped_kernel<WGRAD,shared>");
+      if (rc != FOMOE_OK) return rc;
+    }
+  }
+  return FOMOE_OK;
+}
+
 }  // namespace fomoe
