@@ -1,0 +1,341 @@
+#!/usr/bin/env python
+"""bench.py — skip-token MoE layer tokens/s, forward + backward, on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2] [--impl reference]
+
+A "step" is one pass of the hot path over one batch resident in HBM: fomoe_route + fomoe_moe_fwd + fomoe_moe_bwd
+(rows F1-F8, B1-B7 of SURVEY.md §8(a)).  The resident-delta pack (row S1) runs once per K local steps at a round
+boundary, so it is timed beside the step and reported under "pack", not inside tokens/s.
+Prints ONE JSON line (see DESIGN.md "Measurement" for every key).  --impl reference times the CPU oracle instead.
+N > 1: one process per GPU (torchrun), independent replicas, no collective on the data path ("scaling": "weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+from paper_2606_19025_b200 import workloads as W  # noqa: E402
+
+METRIC = "skip-token MoE layer tokens/s fwd+bwd"
+UNIT = "tokens/s"
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}  # B200_PROFILING.md fallback
+
+
+def workload_desc(w: W.MoEWorkload, n_res: int) -> str:
+    sh = f" + {w.n_sh} shared (d_ff {w.F_sh})" if w.n_sh else ""
+    return (f"{w.name}: T={w.T}, d_model={w.d}, E={w.E}{sh}, top-{w.k}, SwiGLU d_ff={w.F}, {n_res} of {w.E} resident, "
+            f"{w.dtype}, fp32 router, x~N(0,1), weights~N(0,0.02), seed {w.seed}"
+            + (f", Zipf(alpha={w.zipf_alpha}) router bias" if w.zipf_alpha else ""))
+
+
+def load_peaks():
+    f = ROOT / "MEASURED_PEAKS.json"
+    if f.exists():
+        try:
+            d = json.loads(f.read_text())
+            return {k: float(d[k]) for k in FALLBACK_PEAKS}, "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return dict(FALLBACK_PEAKS), "fallback (B200_PROFILING.md)"
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# clocks sampled DURING the timed region
+# ------------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+                for nm, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                continue
+        # under load = samples in the upper half of what was seen (idle samples at the edges are dropped)
+        load = [v for v in sm if v >= 0.5 * max(sm)] if sm else []
+        return {"sm_mhz": statistics.median(load) if load else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# the CPU oracle legs (cpu_baseline, --impl reference): the only places bench.py executes oracle/
+# ------------------------------------------------------------------------------------------------------------------
+def oracle_sample_time(w: W.MoEWorkload, n_res: int, sample_tokens: int, reps: int = 1):
+    """Times the f32 oracle, as it stands, on the first `sample_tokens` tokens of the workload (same weights)."""
+    from oracle.oracle import Oracle
+    o = Oracle("f32")
+    ws = w.with_(T=sample_tokens)
+    S = W.resident_set(w, n_res)
+    x, dy = W.make_x(w)[:sample_tokens].copy(), W.make_dy(w)[:sample_tokens].copy()
+    w_r, bias = W.make_router(w), W.router_bias(w)
+    wg, wu, wd = W.make_resident_experts(w, S)
+    shared = W.make_shared_experts(w)
+    times = []
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        r = o.route(x, w_r, S, ws.k, ws.gate_fn, ws.gate_rule, ws.temperature, bias)
+        o.moe_fwd(x, r, S, wg, wu, wd, shared)
+        o.moe_bwd(x, dy, w_r, r, S, wg, wu, wd, shared, ws.gate_fn, ws.gate_rule, ws.temperature)
+        times.append(time.perf_counter() - t0)
+    return times, o.threads()
+
+
+def run_reference(args, w, n_res):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    sample = min(w.T, args.ref_tokens)
+    times, cores = oracle_sample_time(w, n_res, sample, reps=args.warmup + args.steps)
+    timed = times[args.warmup:]
+    ms = 1e3 * sum(timed) / len(timed)
+    val = sample / (ms / 1e3)
+    sample_desc = f"first {sample} of {w.T} tokens per step, all {n_res} resident experts' weights, route+fwd+bwd, f32 oracle"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic", "config": {"workload": workload_desc(w, n_res), "sample": sample_desc},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample_desc},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# GPU arm
+# ------------------------------------------------------------------------------------------------------------------
+def gemm_flops(mode: str, P: int, T: int, w: W.MoEWorkload) -> float:
+    """Algorithmic flops of one launch: 2*rows*d*F per GEMM; FWD1 and DX are two GEMMs."""
+    shared = "shared" in mode
+    rows, F = (T * w.n_sh, w.F_sh) if shared else (P, w.F)
+    mult = 4 if ("FWD1" in mode or "DX" in mode) else 2
+    return float(mult) * rows * w.d * F
+
+
+def run_gpu(args, w, n_res):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2606_19025_b200 import binding as B
+    from paper_2606_19025_b200.layer import SkipTokenMoE, pack_resident_deltas
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the CPU oracle")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    B.lib()
+
+    def build_layer(nr):
+        S = W.resident_set(w, nr)
+        wg, wu, wd = W.make_resident_experts(w, S)
+        return SkipTokenMoE(w, S, W.make_router(w), wg, wu, wd, W.make_shared_experts(w), W.router_bias(w))
+
+    layer = build_layer(n_res)
+    x_np, dy_np = W.make_x(w), W.make_dy(w)
+    x, dy = layer.to_dev(x_np), layer.to_dev(dy_np)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
+
+    def barrier_all():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed_steps(fn, steps, warmup, collective=False):
+        """Per-step CUDA events on the launching stream; L2 flushed between steps, outside the event pairs.
+        collective=True brackets the region with a barrier over all ranks (the headline measurement)."""
+        barrier = barrier_all if collective else torch.cuda.synchronize
+        for _ in range(warmup):
+            fn()
+        barrier()
+        evs = []
+        for _ in range(steps):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn()
+            e1.record()
+            evs.append((e0, e1))
+        barrier()
+        return [a.elapsed_time(b) for a, b in evs]
+
+    launches = [0]
+
+    def step():
+        launches[0] = layer.step(x, dy)
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    ms_list = timed_steps(step, args.steps, args.warmup, collective=True)
+    clocks = sampler.stop()
+    ms = sum(ms_list) / len(ms_list)
+    if world > 1:
+        t = torch.tensor([ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * w.T / (ms / 1e3)
+
+    routing = layer.routing_numpy()
+    P = routing["P"]
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": w.dtype,
+        "data": "synthetic",
+        "config": {"workload": workload_desc(w, n_res), "parallelism": f"{world} independent replica(s), no collective",
+                   "l2": "512 MiB flush write between timed steps (outside the per-step CUDA-event pairs)",
+                   "timing": "per-step CUDA events on the launching stream, mean over steps, max over ranks"},
+        "clocks": clocks, "gpu_launches": launches[0] * args.steps,
+        "kept_pairs": P, "kept_fraction": P / max(1, w.T * w.k), "ms_min": min(ms_list),
+    }
+    flops_step = 18.0 * P * w.d * w.F + 18.0 * w.T * w.n_sh * w.d * w.F_sh
+    out["tflops"] = flops_step / (ms / 1e3) / 1e12
+
+    if rank == 0:
+        peaks, peak_src = load_peaks()
+        # ---- per-kernel timing: a second pass of the same steps with one CUDA event after every launch ----
+        B.fomoe_profile_enable(True)
+        for _ in range(args.steps):
+            flush.zero_()
+            step()
+        recs = B.fomoe_profile_collect(65536)
+        B.fomoe_profile_enable(False)
+        agg = {}
+        for name, t in recs:
+            a = agg.setdefault(name, [0.0, 0])
+            a[0] += t
+            a[1] += 1
+        total = sum(a[0] for a in agg.values())
+        kernels = []
+        for name, (tt, n) in sorted(agg.items(), key=lambda kv: -kv[1][0]):
+            k = {"name": name, "launches_per_step": n / args.steps, "ms_per_launch": tt / n, "share": tt / total}
+            if name.startswith("umma_grouped_kernel"):
+                fl = gemm_flops(name, P, w.T, w)
+                k.update(bound="tensor", achieved=fl / (tt / n / 1e3) / 1e12, unit="TFLOP/s")
+                k["frac"] = k["achieved"] / peaks["bf16_tflops_sustained"]
+            kernels.append(k)
+        out["kernels"] = kernels
+        traffic = None
+        tf = ROOT / "profiles" / "traffic.json"
+        gemms = [k for k in kernels if k.get("bound") == "tensor"]
+        if gemms:
+            dom = gemms[0]
+            if tf.exists():
+                traffic = json.loads(tf.read_text()).get(w.name, {}).get(dom["name"])
+            out["roofline"] = {"kernel": dom["name"], "bound": "tensor", "achieved": dom["achieved"],
+                               "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s", "frac": dom["frac"], "traffic": traffic,
+                               "peak_source": peak_src + ", bf16 sustained (kernel timed inside a long step)",
+                               "frac_of_nominal_2250": dom["achieved"] / 2250.0, "share_of_step": dom["share"],
+                               "kernel_timing": "second pass of the same steps with one CUDA event after every launch"}
+            gt = sum(k["ms_per_launch"] * k["launches_per_step"] for k in gemms)
+            out["gemm_family"] = {"tflops": flops_step / (gt / 1e3) / 1e12, "share_of_step": gt * args.steps / total,
+                                  "frac_of_measured_sustained": flops_step / (gt / 1e3) / 1e12 / peaks["bf16_tflops_sustained"]}
+
+        # ---- end to end through the C ABI with HOST buffers (uploads x, dy; downloads y, dx every step) ----
+        xh, dyh = x.cpu().pin_memory(), dy.cpu().pin_memory()
+        yh, dxh = torch.empty_like(xh).pin_memory(), torch.empty_like(xh).pin_memory()
+        xd, dyd = torch.empty_like(x), torch.empty_like(dy)
+        cs = torch.cuda.Stream()
+        e2e_ms = timed_steps(lambda: layer.step_host(xh, dyh, yh, dxh, xd, dyd, copy_stream=cs), args.steps, args.warmup)
+        e2e = sum(e2e_ms) / len(e2e_ms)
+        nbytes = xh.numel() * xh.element_size()
+        out["e2e"] = {"value": world * w.T / (e2e / 1e3), "unit": UNIT, "h2d_bytes_per_step": 2 * nbytes,
+                      "d2h_bytes_per_step": 2 * nbytes, "ms_per_step": e2e,
+                      "api": "fomoe_moe_step_host (pinned host x, dy -> y, dx; dy upload and y download overlap compute)"}
+
+        # ---- resident-delta pack (row S1), HBM bound: 12 B per parameter ----
+        S = W.resident_set(w, n_res)
+        now = [torch.from_numpy(np.stack(t)).cuda() for t in zip(*(W.make_expert_master(w, int(e)) for e in S))]
+        start = [t + 1e-3 * torch.randn_like(t) for t in now]
+        payload = torch.empty((n_res, sum(int(t[0].numel()) for t in now)), dtype=torch.float32, device="cuda")
+        pk = timed_steps(lambda: pack_resident_deltas(now, start, None, payload), max(args.steps, 10), 3)
+        pbytes = 12.0 * payload.numel()
+        pms = sum(pk) / len(pk)
+        out["pack"] = {"bound": "hbm", "achieved": pbytes / (pms / 1e3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                       "frac": pbytes / (pms / 1e3) / 1e9 / peaks["hbm_gbs"], "ms": pms, "bytes": pbytes,
+                       "frac_of_nominal_8000": pbytes / (pms / 1e3) / 1e9 / 8000.0}
+        del now, start, payload
+
+        # ---- skip-token speed-up against the same kernels with every expert resident ----
+        if not args.no_all_resident and n_res < w.E:
+            del layer
+            torch.cuda.empty_cache()
+            full = build_layer(w.E)
+            ms_full = timed_steps(lambda: full.step(x, dy), args.steps, args.warmup)
+            mf = sum(ms_full) / len(ms_full)
+            out["skip_token"] = {"ms_all_resident": mf, "speedup_vs_all_resident": mf / ms,
+                                 "ideal_flop_ratio": (w.k * 18.0 * w.d * w.F * w.T + 18.0 * w.T * w.n_sh * w.d * w.F_sh) / flops_step}
+            del full
+
+        # ---- the oracle, as it stands, on the host cores (reported baseline, not the target) ----
+        if not args.no_cpu_baseline:
+            sample = min(w.T, args.ref_tokens)
+            times, cores = oracle_sample_time(w, n_res, sample)
+            out["cpu_baseline"] = {"value": sample / times[0], "unit": UNIT, "cores": cores, "kind": "oracle",
+                                   "sample": f"first {sample} of {w.T} tokens, all {n_res} resident experts' weights, "
+                                             f"route+fwd+bwd, f32 oracle, 1 repetition, {times[0]:.1f} s"}
+        print(json.dumps(out))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C2", choices=sorted(W.CONFIGS))
+    ap.add_argument("--n-res", type=int, default=None)
+    ap.add_argument("--ref-tokens", type=int, default=1024, help="tokens per step of the CPU oracle sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-all-resident", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    w = W.config(args.workload)
+    n_res = w.n_res if args.n_res is None else args.n_res
+    if args.impl == "reference":
+        run_reference(args, w, n_res)
+    else:
+        run_gpu(args, w, n_res)
+
+
+if __name__ == "__main__":
+    main()

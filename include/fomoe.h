@@ -189,6 +189,16 @@ FOMOE_API int fomoe_abi_version(void);
  * Debug / A-B testing only. */
 FOMOE_API int fomoe_set_force_simt(int on);
 
+/*
+ * Per-kernel timing for bench.py's roofline figures.  fomoe_profile_enable(1) clears and starts recording on the
+ * calling thread: every kernel the library launches is followed by a CUDA event on its stream.  fomoe_profile_collect
+ * synchronises the last event and returns the number of kernel records; for i < min(count, cap) it stores the
+ * kernel's name (a static string) and the milliseconds since the previous event on the stream.  Recording adds an
+ * event per launch, so timed throughput runs keep it off (fomoe_profile_enable(0)).
+ */
+FOMOE_API int fomoe_profile_enable(int on);
+FOMOE_API int fomoe_profile_collect(const char** names, float* ms, int cap);
+
 #ifdef __cplusplus
 }
 #endif

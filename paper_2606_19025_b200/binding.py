@@ -24,7 +24,7 @@ FOMOE_DROP_ONLY, FOMOE_RENORM_TOPK, FOMOE_RENORM_RESIDENT = 0, 1, 2
 
 EXPORTS = ("fomoe_workspace_bytes", "fomoe_route", "fomoe_moe_fwd", "fomoe_moe_bwd", "fomoe_pack_resident_deltas",
            "fomoe_moe_step_host", "fomoe_last_launch_count", "fomoe_last_cuda_error", "fomoe_abi_version",
-           "fomoe_set_force_simt")
+           "fomoe_set_force_simt", "fomoe_profile_enable", "fomoe_profile_collect")
 
 
 class fomoe_config(C.Structure):
@@ -173,3 +173,15 @@ def fomoe_last_launch_count() -> int:
 
 def fomoe_set_force_simt(on: bool) -> bool:
     return bool(lib().fomoe_set_force_simt(C.c_int(1 if on else 0)))
+
+
+def fomoe_profile_enable(on: bool) -> None:
+    _check(lib().fomoe_profile_enable(C.c_int(1 if on else 0)), "fomoe_profile_enable")
+
+
+def fomoe_profile_collect(cap: int = 4096):
+    """Returns [(kernel name, ms), ...] recorded since fomoe_profile_enable(True)."""
+    names = (C.c_char_p * cap)()
+    ms = (C.c_float * cap)()
+    n = lib().fomoe_profile_collect(names, ms, C.c_int(cap))
+    return [(names[i].decode(), float(ms[i])) for i in range(min(n, cap))]

@@ -2,6 +2,8 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <vector>
+
 #include "common.cuh"
 
 namespace fomoe {
@@ -10,7 +12,24 @@ static thread_local char g_err[512] = "";
 static thread_local int g_launches = 0;
 static int g_force_simt = 0;
 
-void note_launch() { ++g_launches; }
+// optional per-kernel timing: one event after every launch (+ a marker at each entry point); kernel i's time is the
+// interval since the previous event on the same stream
+struct ProfRec { const char* name; cudaEvent_t ev; };
+static thread_local std::vector<ProfRec> g_prof;
+static thread_local bool g_prof_on = false;
+static void prof_push(const char* name, cudaStream_t st) {
+  cudaEvent_t e;
+  if (cudaEventCreate(&e) != cudaSuccess) return;
+  cudaEventRecord(e, st);
+  g_prof.push_back({name, e});
+}
+void note_launch(const char* name, cudaStream_t st) {
+  ++g_launches;
+  if (g_prof_on) prof_push(name, st);
+}
+void note_api_entry(const char* name, cudaStream_t st) {
+  if (g_prof_on) prof_push(name, st);
+}
 int set_cuda_error(cudaError_t e, const char* where) {
   snprintf(g_err, sizeof(g_err), "%s: %s (%s)", where, cudaGetErrorName(e), cudaGetErrorString(e));
   return FOMOE_ERR_CUDA;
@@ -45,6 +64,28 @@ const char* fomoe_last_cuda_error(void) { return g_err; }
 int fomoe_last_launch_count(void) { return g_launches; }
 int fomoe_set_force_simt(int on) { int p = g_force_simt; g_force_simt = on ? 1 : 0; return p; }
 
+int fomoe_profile_enable(int on) {
+  for (auto& r : g_prof) cudaEventDestroy(r.ev);
+  g_prof.clear();
+  g_prof_on = on != 0;
+  return FOMOE_OK;
+}
+
+int fomoe_profile_collect(const char** names, float* ms, int cap) {
+  int n = 0;
+  if (!g_prof.empty()) cudaEventSynchronize(g_prof.back().ev);
+  for (size_t i = 1; i < g_prof.size(); ++i) {
+    if (g_prof[i].name[0] == '@') continue;  // entry marker: the gap before it is not kernel time
+    float t = 0.f;
+    if (cudaEventElapsedTime(&t, g_prof[i - 1].ev, g_prof[i].ev) != cudaSuccess) t = -1.f;
+    if (n < cap) { names[n] = g_prof[i].name; ms[n] = t; }
+    ++n;
+  }
+  for (auto& r : g_prof) cudaEventDestroy(r.ev);
+  g_prof.clear();
+  return n;
+}
+
 int fomoe_workspace_bytes(const fomoe_config* cfg, int32_t n_res, size_t* route_internal, size_t* saved_acts, size_t* scratch) {
   int rc = check_cfg(cfg, n_res);
   if (rc != FOMOE_OK) return rc;
@@ -65,6 +106,7 @@ int fomoe_route(const fomoe_config* cfg, const void* x, const float* w_router, c
   if (cfg->T > 0 && (!out->topk_idx || !out->gate || !out->probs || !out->row_token || !out->pair_row)) return FOMOE_ERR_BADARG;
   if (!aligned16(x) || !aligned16(w_router) || !aligned16(out->internal)) return FOMOE_ERR_BADARG;
   RouteWs ws = carve_route_ws(*cfg, n_res, out->internal);
+  note_api_entry("@fomoe_route", (cudaStream_t)stream);
   return launch_route(*cfg, x, w_router, router_bias, resident_ids, n_res, *out, ws, (cudaStream_t)stream);
 }
 
@@ -85,6 +127,7 @@ int fomoe_moe_fwd(const fomoe_config* cfg, const void* x, const fomoe_route_stat
   ActWs aws = carve_act_ws(*cfg, rws.R_cap, saved_acts);
   ScratchWs sws = carve_scratch_ws(*cfg, rws.R_cap, scratch);
   FfnPtrs w{w_gate, w_up, w_down, sh_gate, sh_up, sh_down};
+  note_api_entry("@fomoe_moe_fwd", st);
   if (cfg->T == 0) return FOMOE_OK;
   if (n_res > 0) {
     rc = launch_gather_rows(*cfg, x, rws, aws.xp, st);
@@ -115,6 +158,7 @@ int fomoe_moe_bwd(const fomoe_config* cfg, const void* dy, const void* x, const 
   ActWs aws = carve_act_ws(*cfg, rws.R_cap, const_cast<void*>(saved_acts));
   ScratchWs sws = carve_scratch_ws(*cfg, rws.R_cap, scratch);
   FfnPtrs w{w_gate, w_up, w_down, sh_gate, sh_up, sh_down};
+  note_api_entry("@fomoe_moe_bwd", st);
   // B1: do = g dy per row, dgate = <dy, o>
   if (n_res > 0 && cfg->T > 0) {
     rc = launch_combine_bwd(*cfg, dy, aws.o, rws, sws.dop, sws.dgate, st);
@@ -146,6 +190,7 @@ int fomoe_pack_resident_deltas(const float* const w_now[3], const float* const w
   for (int i = 0; i < 3; ++i)
     if (!w_now[i] || !w_start[i] || !aligned16(w_now[i]) || !aligned16(w_start[i])) return FOMOE_ERR_BADARG;
   if (elems_gate % 4 || elems_up % 4 || elems_down % 4) return FOMOE_ERR_UNSUPPORTED;
+  note_api_entry("@fomoe_pack_resident_deltas", (cudaStream_t)stream);
   return launch_pack(w_now, w_start, n_res, elems_gate, elems_up, elems_down, pack_slots, n_pack, payload, (cudaStream_t)stream);
 }
 

@@ -14,7 +14,8 @@ constexpr int kMaxE = 512;
 constexpr int kMaxK = 32;
 
 // ---- per-thread error / launch bookkeeping (api.cu) ----
-void note_launch();
+void note_launch(const char* name, cudaStream_t st);   // counts the launch; records a profiling event when enabled
+void note_api_entry(const char* name, cudaStream_t st);  // profiling marker at the start of an entry point
 int set_cuda_error(cudaError_t e, const char* where);
 #define FOMOE_CUDA_OK(expr)                                          \
   do {                                                               \
@@ -23,7 +24,7 @@ int set_cuda_error(cudaError_t e, const char* where);
   } while (0)
 #define FOMOE_LAUNCH_OK(name)                                        \
   do {                                                               \
-    fomoe::note_launch();                                            \
+    fomoe::note_launch(name, st);                                    \
     cudaError_t e__ = cudaGetLastError();                            \
     if (e__ != cudaSuccess) return fomoe::set_cuda_error(e__, name);  \
   } while (0)
