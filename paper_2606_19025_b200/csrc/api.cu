@@ -51,6 +51,7 @@ static int check_cfg(const fomoe_config* c, int n_res) {
   return FOMOE_OK;
 }
 
+bool force_simt() { return g_force_simt != 0; }
 static bool use_umma(const fomoe_config& c) { return !g_force_simt && umma_supported(c); }
 
 }  // namespace fomoe

@@ -9,7 +9,7 @@
 namespace fomoe {
 
 constexpr int kTileM = 128;      // rows of one expert-GEMM tile; every slot's row group is padded to this
-constexpr int kPermChunk = 1024; // (token, expert) pairs handled by one block of the permutation kernels
+constexpr int kPermTokens = 128; // tokens (x top_k pairs) handled by one block of the permutation kernels = one router tile
 constexpr int kMaxE = 512;
 constexpr int kMaxK = 32;
 
@@ -53,6 +53,7 @@ struct RouteWs {
   float* prow_gate;     // [R_cap]        gate of padded row r
   int32_t* prow_pair;   // [R_cap]        t*k+j of padded row r
   int32_t* pair_prow;   // [T*k]          padded row of pair, -1 if skipped
+  void* wr_split;       // [d, 256] bf16  W_r split into bf16 pieces for the tensor-core router
   int n_blk, max_mtiles, R_cap;
   size_t bytes;
 };
@@ -60,7 +61,7 @@ struct RouteWs {
 inline RouteWs carve_route_ws(const fomoe_config& c, int n_res, void* base) {
   RouteWs w{};
   long pairs = (long)c.T * c.top_k;
-  w.n_blk = (int)((pairs + kPermChunk - 1) / kPermChunk);
+  w.n_blk = (c.T + kPermTokens - 1) / kPermTokens;
   if (w.n_blk < 1) w.n_blk = 1;
   w.max_mtiles = (int)((pairs + kTileM - 1) / kTileM) + n_res;
   if (w.max_mtiles < 1) w.max_mtiles = 1;
@@ -77,6 +78,7 @@ inline RouteWs carve_route_ws(const fomoe_config& c, int n_res, void* base) {
   w.prow_gate = (float*)take(sizeof(float) * (size_t)w.R_cap);
   w.prow_pair = (int32_t*)take(sizeof(int32_t) * (size_t)w.R_cap);
   w.pair_prow = (int32_t*)take(sizeof(int32_t) * (size_t)(pairs > 0 ? pairs : 1));
+  w.wr_split = take(sizeof(__nv_bfloat16) * (size_t)c.d_model * 256);
   w.bytes = off;
   return w;
 }
@@ -156,6 +158,11 @@ inline ScratchWs carve_scratch_ws(const fomoe_config& c, int R_cap, void* base) 
 // ---- launchers implemented in the other translation units (all enqueue on `st`, return FOMOE_* status) ----
 int launch_route(const fomoe_config& c, const void* x, const float* w_router, const float* bias,
                  const int32_t* resident_ids, int n_res, const fomoe_route_state& out, const RouteWs& ws, cudaStream_t st);
+// tensor-core router (route_umma.cu): bf16 tokens, d % 64 == 0, E <= 128, k <= 8
+bool route_umma_supported(const fomoe_config& c);
+int launch_route_umma(const fomoe_config& c, const void* x, const float* w_router, const float* bias, const int32_t* resident_ids,
+                      int n_res, const fomoe_route_state& out, const RouteWs& ws, cudaStream_t st);
+bool force_simt();
 
 // row-wise (bandwidth) kernels, rows.cu
 int launch_gather_rows(const fomoe_config& c, const void* x, const RouteWs& ws, void* xp, cudaStream_t st);

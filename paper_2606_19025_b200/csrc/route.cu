@@ -149,15 +149,15 @@ route_kernel(const XT* __restrict__ x, const float* __restrict__ w_r, const floa
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// Permutation.  Pairs are numbered p = t*k + j; a block owns kPermChunk consecutive pairs.
+// Permutation.  Pairs are numbered p = t*k + j; a block owns the kPermTokens * k pairs of one 128-token router tile.
 // ---------------------------------------------------------------------------------------------------------
 __global__ void perm_hist_kernel(const int32_t* __restrict__ topk_idx, const int32_t* __restrict__ slot_of, long n_pairs,
-                                 int n_res, int32_t* __restrict__ blk_hist) {
+                                 int pairs_per_blk, int n_res, int32_t* __restrict__ blk_hist) {
   extern __shared__ int32_t hist[];
   for (int i = threadIdx.x; i < n_res; i += blockDim.x) hist[i] = 0;
   __syncthreads();
-  long p0 = (long)blockIdx.x * kPermChunk;
-  for (int i = threadIdx.x; i < kPermChunk; i += blockDim.x) {
+  long p0 = (long)blockIdx.x * pairs_per_blk;
+  for (int i = threadIdx.x; i < pairs_per_blk; i += blockDim.x) {
     long p = p0 + i;
     if (p < n_pairs) {
       int s = slot_of[topk_idx[p]];
@@ -208,7 +208,7 @@ constexpr int kPermThreads = 256;
 __global__ void __launch_bounds__(kPermThreads)
 perm_scatter_kernel(const int32_t* __restrict__ topk_idx, const float* __restrict__ gate, const int32_t* __restrict__ slot_of,
                     const int32_t* __restrict__ blk_base, const int32_t* __restrict__ offsets,
-                    const int32_t* __restrict__ pad_offsets, long n_pairs, int k, int n_res,
+                    const int32_t* __restrict__ pad_offsets, long n_pairs, int pairs_per_blk, int k, int n_res,
                     int32_t* __restrict__ row_token, int32_t* __restrict__ pair_row, int32_t* __restrict__ prow_token,
                     float* __restrict__ prow_gate, int32_t* __restrict__ prow_pair, int32_t* __restrict__ pair_prow) {
   extern __shared__ int32_t sm[];
@@ -218,9 +218,10 @@ perm_scatter_kernel(const int32_t* __restrict__ topk_idx, const float* __restric
   for (int i = threadIdx.x; i < n_res; i += kPermThreads) running[i] = blk_base[(size_t)blockIdx.x * n_res + i];
   for (int i = threadIdx.x; i < 8 * n_res; i += kPermThreads) warp_cnt[i] = 0;
   __syncthreads();
-  const long p0 = (long)blockIdx.x * kPermChunk;
-  for (int it = 0; it < kPermChunk / kPermThreads; ++it) {
-    const long p = p0 + it * kPermThreads + threadIdx.x;
+  const long p0 = (long)blockIdx.x * pairs_per_blk;
+  for (int it = 0; it < (pairs_per_blk + kPermThreads - 1) / kPermThreads; ++it) {
+    const int ip = it * kPermThreads + threadIdx.x;
+    const long p = ip < pairs_per_blk ? p0 + ip : n_pairs;   // out of this block's range -> inactive
     int s = -1;
     if (p < n_pairs) s = slot_of[topk_idx[p]];
     unsigned m = __match_any_sync(0xffffffffu, s);
@@ -284,8 +285,8 @@ static int launch_route_t(const fomoe_config& c, const XT* x, const float* w_rou
 int launch_route(const fomoe_config& c, const void* x, const float* w_router, const float* bias, const int32_t* resident_ids,
                  int n_res, const fomoe_route_state& out, const RouteWs& ws, cudaStream_t st) {
   const long n_pairs = (long)c.T * c.top_k;
-  slot_map_kernel<<<ceil_div(c.E, 128), 128, 0, st>>>(resident_ids, n_res, c.E, ws.slot_of);
-  FOMOE_LAUNCH_OK("slot_map_kernel");
+  const int pairs_per_blk = kPermTokens * c.top_k;
+  const int nr = n_res > 0 ? n_res : 1;
   FOMOE_CUDA_OK(cudaMemsetAsync(out.row_token, 0xFF, sizeof(int32_t) * (size_t)n_pairs, st));
   FOMOE_CUDA_OK(cudaMemsetAsync(ws.prow_token, 0xFF, sizeof(int32_t) * (size_t)ws.R_cap, st));
   if (c.T == 0) {  // empty batch: all counts and offsets are zero, no tile in use
@@ -295,18 +296,25 @@ int launch_route(const fomoe_config& c, const void* x, const float* w_router, co
     FOMOE_CUDA_OK(cudaMemsetAsync(ws.n_mtiles, 0, sizeof(int32_t) * 4, st));
     return FOMOE_OK;
   }
-  int rc = c.dtype == FOMOE_BF16 ? launch_route_t<__nv_bfloat16>(c, (const __nv_bfloat16*)x, w_router, bias, ws, out, st)
-                                 : launch_route_t<float>(c, (const float*)x, w_router, bias, ws, out, st);
-  if (rc != FOMOE_OK) return rc;
-  const int nr = n_res > 0 ? n_res : 1;
-  perm_hist_kernel<<<ws.n_blk, 256, sizeof(int32_t) * nr, st>>>(out.topk_idx, ws.slot_of, n_pairs, n_res, ws.blk_hist);
-  FOMOE_LAUNCH_OK("perm_hist_kernel");
+  if (!force_simt() && route_umma_supported(c)) {
+    // tensor-core router: logits + gate + top-k + mask + per-block histogram in one kernel
+    int rc = launch_route_umma(c, x, w_router, bias, resident_ids, n_res, out, ws, st);
+    if (rc != FOMOE_OK) return rc;
+  } else {
+    slot_map_kernel<<<ceil_div(c.E, 128), 128, 0, st>>>(resident_ids, n_res, c.E, ws.slot_of);
+    FOMOE_LAUNCH_OK("slot_map_kernel");
+    int rc = c.dtype == FOMOE_BF16 ? launch_route_t<__nv_bfloat16>(c, (const __nv_bfloat16*)x, w_router, bias, ws, out, st)
+                                   : launch_route_t<float>(c, (const float*)x, w_router, bias, ws, out, st);
+    if (rc != FOMOE_OK) return rc;
+    perm_hist_kernel<<<ws.n_blk, 256, sizeof(int32_t) * nr, st>>>(out.topk_idx, ws.slot_of, n_pairs, pairs_per_blk, n_res, ws.blk_hist);
+    FOMOE_LAUNCH_OK("perm_hist_kernel");
+  }
   perm_scan_kernel<<<1, 256, 0, st>>>(ws.blk_hist, ws.n_blk, n_res, out.counts, out.offsets, ws.pad_offsets, ws.n_mtiles,
                                       ws.tile_slot);
   FOMOE_LAUNCH_OK("perm_scan_kernel");
   perm_scatter_kernel<<<ws.n_blk, kPermThreads, sizeof(int32_t) * 9 * nr, st>>>(
-      out.topk_idx, out.gate, ws.slot_of, ws.blk_hist, out.offsets, ws.pad_offsets, n_pairs, c.top_k, n_res, out.row_token,
-      out.pair_row, ws.prow_token, ws.prow_gate, ws.prow_pair, ws.pair_prow);
+      out.topk_idx, out.gate, ws.slot_of, ws.blk_hist, out.offsets, ws.pad_offsets, n_pairs, pairs_per_blk, c.top_k, n_res,
+      out.row_token, out.pair_row, ws.prow_token, ws.prow_gate, ws.prow_pair, ws.pair_prow);
   FOMOE_LAUNCH_OK("perm_scatter_kernel");
   return FOMOE_OK;
 }

@@ -20,19 +20,27 @@
 #include <cuda.h>
 
 #include "common.cuh"
+#include "umma_ptx.cuh"
 
 namespace fomoe {
 namespace {
 
-using bf16 = __nv_bfloat16;
-
-constexpr int BM = 128, BN = 256, BK = 64, kStages = 4, kAccStages = 2;
+constexpr int BM = 128, BN = 256, BK = 64, kAccStages = 2;
 constexpr int kABytes = BM * BK * 2, kBBytes = BN * BK * 2, kStageBytes = kABytes + kBBytes;
 constexpr int kThreads = 256;
-constexpr int kSmemBytes = kStages * kStageBytes + 1024 /*align*/ + 256 /*barriers*/;
-constexpr int kTmemCols = 512;
-
+// epilogue staging: per epilogue warp, up to 3 swizzled tiles of 32 rows x 32 bf16 (2 KB each) used to turn the
+// row-per-thread TMEM layout into coalesced 16-byte global accesses
+constexpr int kStgTile = 2048;
+constexpr int kDhDepth = 4;  // DH epilogue: chunks of (a, u) kept in flight per warp with cp.async
 enum Mode { FWD1 = 0, FWD2 = 1, DH = 2, DX = 3, WGRAD = 4 };
+// DH trades one TMA stage for a deep epilogue prefetch ring: its epilogue must stream a and u back in
+__host__ __device__ constexpr int stages_of(int mode) { return mode == DH ? 3 : 4; }
+__host__ __device__ constexpr int stg_tiles_per_warp(int mode) { return mode == DH ? 2 * kDhDepth + 2 : 3; }
+__host__ __device__ constexpr int stg_bytes_of(int mode) { return 4 * stg_tiles_per_warp(mode) * kStgTile; }
+__host__ __device__ constexpr int smem_bytes_of(int mode) {
+  return stages_of(mode) * kStageBytes + stg_bytes_of(mode) + 1024 /*align*/ + 256 /*barriers*/;
+}
+constexpr int kTmemCols = 512;
 
 struct TmaMaps {
   CUtensorMap m[4];
@@ -53,81 +61,32 @@ struct UmmaParams {
   const bf16 *in0, *in1;       // DH: a,u
 };
 
-// ---------------------------------------------------------------------------------------------------------
-// PTX wrappers
-// ---------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, bool valid) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(valid ? 16 : 0) : "memory");
 }
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  uint32_t done;
-  do {
-    asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
-                 : "=r"(done) : "r"(bar), "r"(parity) : "memory");
-  } while (!done);
-}
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1) {
-  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
-               ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(bar), "r"(c0), "r"(c1) : "memory");
-}
-__device__ __forceinline__ void prefetch_tmap(const CUtensorMap* map) {
-  asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(map)) : "memory");
-}
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void umma_commit(uint32_t bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
-}
-// shared-memory matrix descriptor, 128-byte swizzle, Blackwell version field = 1
-__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
-  uint64_t dsc = 0;
-  dsc |= (uint64_t)((saddr & 0x3FFFFu) >> 4);
-  dsc |= (uint64_t)(lbo_bytes >> 4) << 16;
-  dsc |= (uint64_t)(sbo_bytes >> 4) << 32;
-  dsc |= (uint64_t)1 << 46;
-  dsc |= (uint64_t)2 << 61;
-  return dsc;
-}
-__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
-  asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}"
-               ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
-}
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32]) {
-  uint32_t* r = reinterpret_cast<uint32_t*>(v);
-  asm volatile(
-      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-      "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
-      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
-        "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]),
-        "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]),
-        "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
-      : "r"(taddr));
-}
-__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-__device__ __forceinline__ void store_bf16x32(bf16* dst, const float (&v)[32]) {
-  uint4* p = reinterpret_cast<uint4*>(dst);
+// ---- per-warp staging tile: 32 rows x 64 B, two rows per 128-byte line, 16-byte chunks XOR-swizzled so that both the
+// row-per-lane accesses and the 8-rows-x-4-chunks global-side accesses are bank-conflict free ----
+__device__ __forceinline__ uint32_t stg_off(int r, int q) { return (uint32_t)((r >> 1) * 128 + (((((r & 1) << 2) | q) ^ ((r >> 1) & 7)) * 16)); }
+
+// lane = row: write 32 fp32 as bf16 into the staging tile
+__device__ __forceinline__ void stg_put_row(uint8_t* stg, int lane, const float (&v)[32]) {
 #pragma unroll
   for (int q = 0; q < 4; ++q) {
     uint4 w;
     __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&w);
 #pragma unroll
     for (int i = 0; i < 4; ++i) h[i] = __floats2bfloat162_rn(v[q * 8 + 2 * i], v[q * 8 + 2 * i + 1]);
-    p[q] = w;
+    *reinterpret_cast<uint4*>(stg + stg_off(lane, q)) = w;
   }
 }
-__device__ __forceinline__ void load_bf16x32(const bf16* src, float (&v)[32]) {
-  const uint4* p = reinterpret_cast<const uint4*>(src);
+// lane = row: read 32 bf16 from the staging tile as fp32
+__device__ __forceinline__ void stg_get_row(const uint8_t* stg, int lane, float (&v)[32]) {
 #pragma unroll
   for (int q = 0; q < 4; ++q) {
-    uint4 w = p[q];
+    uint4 w = *reinterpret_cast<const uint4*>(stg + stg_off(lane, q));
     const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&w);
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
@@ -135,6 +94,30 @@ __device__ __forceinline__ void load_bf16x32(const bf16* src, float (&v)[32]) {
       v[q * 8 + 2 * i] = f.x;
       v[q * 8 + 2 * i + 1] = f.y;
     }
+  }
+}
+// whole warp: staging tile -> global rows [0, rows_valid) x 32 columns at g (row stride ld elements); 4 lanes per row
+__device__ __forceinline__ void stg_to_global(const uint8_t* stg, bf16* g, size_t ld, int lane, int rows_valid) {
+#pragma unroll
+  for (int it = 0; it < 4; ++it) {
+    const int r = it * 8 + (lane >> 2), c = lane & 3;
+    const uint4 w = *reinterpret_cast<const uint4*>(stg + stg_off(r, c));
+    if (r < rows_valid) *reinterpret_cast<uint4*>(g + (size_t)r * ld + c * 8) = w;
+  }
+}
+// whole warp: global -> registers (issue early), then registers -> staging tile
+__device__ __forceinline__ void global_to_regs(const bf16* g, size_t ld, int lane, int rows_valid, uint4 (&w)[4]) {
+#pragma unroll
+  for (int it = 0; it < 4; ++it) {
+    const int r = it * 8 + (lane >> 2), c = lane & 3;
+    w[it] = r < rows_valid ? *reinterpret_cast<const uint4*>(g + (size_t)r * ld + c * 8) : make_uint4(0, 0, 0, 0);
+  }
+}
+__device__ __forceinline__ void regs_to_stg(uint8_t* stg, int lane, const uint4 (&w)[4]) {
+#pragma unroll
+  for (int it = 0; it < 4; ++it) {
+    const int r = it * 8 + (lane >> 2), c = lane & 3;
+    *reinterpret_cast<uint4*>(stg + stg_off(r, c)) = w[it];
   }
 }
 
@@ -213,7 +196,10 @@ __global__ void __launch_bounds__(kThreads, 1)
 umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kStages * kStageBytes);
+  constexpr int kStages = stages_of(MODE);
+  constexpr int kStgTilesPerWarp = stg_tiles_per_warp(MODE);
+  uint8_t* stg_base = smem + kStages * kStageBytes;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(stg_base + stg_bytes_of(MODE));
   uint64_t* full_bar = bars;                          // [kStages]
   uint64_t* empty_bar = bars + kStages;               // [kStages]
   uint64_t* tfull_bar = bars + 2 * kStages;           // [kAccStages]
@@ -323,82 +309,160 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
   } else if (warp >= 4) {
     // ===================== epilogue =====================
     const int q = warp & 3;             // TMEM lane quarter of this warp
-    const int r_in_tile = q * 32 + lane;
+    uint8_t* stg0 = stg_base + q * (kStgTilesPerWarp * kStgTile);
+    uint8_t* stg1 = stg0 + kStgTile;
+    uint8_t* stg2 = stg1 + kStgTile;
+    if (MODE == DH) {
+      // SwiGLU backward needs a and u for every output element.  They are streamed global -> shared with cp.async,
+      // kDhDepth 32-column chunks ahead of the consumer and across tile boundaries (the schedule is static), so the
+      // loads never sit on the critical path of the accumulator drain.
+      uint8_t* ring = stg0;                                   // kDhDepth slots of (a tile | u tile)
+      uint8_t* out_a = stg0 + 2 * kDhDepth * kStgTile;
+      uint8_t* out_u = out_a + kStgTile;
+      long pid = blockIdx.x;                                  // prefetch cursor
+      int pcc = 0;
+      bool pvalid = pid < sched.total;
+      Tile pt = pvalid ? sched.decode(pid) : Tile{};
+      auto issue = [&](int slot) {
+        if (pvalid) {
+          const int prow0 = pt.m_tile * BM + q * 32;
+          const int prows = dense ? min(32, p.dense_rows - prow0) : 32;
+          const size_t off = (size_t)prow0 * p.ld + (size_t)pt.part * p.F + pt.n_tile * BN + pcc * 32;
+          const uint32_t sa = smem_u32(ring + slot * 2 * kStgTile), su = sa + kStgTile;
+#pragma unroll
+          for (int it = 0; it < 4; ++it) {
+            const int r = it * 8 + (lane >> 2), c = lane & 3;
+            const bool ok = r < prows;
+            const size_t g = off + (size_t)(ok ? r : 0) * p.ld + c * 8;
+            cp_async16(sa + stg_off(r, c), p.in0 + g, ok);
+            cp_async16(su + stg_off(r, c), p.in1 + g, ok);
+          }
+          ++pcc;
+          if (pcc == BN / 32 || pt.n_tile * BN + pcc * 32 >= p.F) {
+            pcc = 0;
+            pid += gridDim.x;
+            pvalid = pid < sched.total;
+            if (pvalid) pt = sched.decode(pid);
+          }
+        }
+        cp_async_commit();
+      };
+#pragma unroll
+      for (int sidx = 0; sidx < kDhDepth; ++sidx) issue(sidx);
+      int slot = 0, as = 0;
+      uint32_t aphase = 0;
+      for (long id = blockIdx.x; id < sched.total; id += gridDim.x) {
+        const Tile t = sched.decode(id);
+        const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * BN;
+        const int row0 = t.m_tile * BM + q * 32;
+        const int rows_valid = dense ? min(32, p.dense_rows - row0) : 32;
+        const size_t base = (size_t)row0 * p.ld + (size_t)t.part * p.F;
+        mbar_wait(smem_u32(&tfull_bar[as]), aphase);
+        tc_fence_after();
+#pragma unroll 1
+        for (int cc = 0; cc < BN / 32; ++cc) {
+          const int n = t.n_tile * BN + cc * 32;
+          if (n >= p.F) break;
+          float dh[32], a[32], u[32];
+          tmem_ld32(taddr + cc * 32, dh);
+          cp_async_wait<kDhDepth - 1>();
+          __syncwarp();
+          stg_get_row(ring + slot * 2 * kStgTile, lane, a);
+          stg_get_row(ring + slot * 2 * kStgTile + kStgTile, lane, u);
+          __syncwarp();
+          issue(slot);                                        // refill the slot just drained
+          tmem_ld_wait();
+#pragma unroll
+          for (int i = 0; i < 32; ++i) {
+            const float sg = __fdividef(1.0f, 1.0f + __expf(-a[i]));
+            const float da = dh[i] * u[i] * sg * (1.0f + a[i] * (1.0f - sg));
+            u[i] = dh[i] * a[i] * sg;  // du
+            a[i] = da;
+          }
+          stg_put_row(out_a, lane, a);
+          stg_put_row(out_u, lane, u);
+          __syncwarp();
+          if (rows_valid > 0) {
+            stg_to_global(out_a, p.out0 + base + n, p.ld, lane, rows_valid);
+            stg_to_global(out_u, p.out1 + base + n, p.ld, lane, rows_valid);
+          }
+          __syncwarp();
+          if (++slot == kDhDepth) slot = 0;
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&tempty_bar[as]));
+        if (++as == kAccStages) { as = 0; aphase ^= 1; }
+      }
+      cp_async_wait<0>();
+    } else {
     int as = 0;
     uint32_t aphase = 0;
     for (long id = blockIdx.x; id < sched.total; id += gridDim.x) {
       const Tile t = sched.decode(id);
       const bool have_acc = t.num_kb > 0;
-      if (have_acc) {
-        mbar_wait(smem_u32(&tfull_bar[as]), aphase);
-        tc_fence_after();
-      }
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * BN;
+      const int row0 = t.m_tile * BM + q * 32;   // first row (or WGRAD output row m) of this warp
       if (MODE == WGRAD) {
-        const int m = t.m_tile * BM + r_in_tile;
-        bf16* orow = p.out0 + ((size_t)t.group * p.M + m) * p.N;
+        if (have_acc) { mbar_wait(smem_u32(&tfull_bar[as]), aphase); tc_fence_after(); }
+        const int rows_valid = min(32, p.M - row0);
+        bf16* obase = p.out0 + ((size_t)t.group * p.M + row0) * p.N;
 #pragma unroll 1
         for (int cc = 0; cc < BN / 32; ++cc) {
+          const int n = t.n_tile * BN + cc * 32;
+          if (n >= p.N) break;
           float v[32];
           if (have_acc) { tmem_ld32(taddr + cc * 32, v); tmem_ld_wait(); }
           else {
 #pragma unroll
             for (int i = 0; i < 32; ++i) v[i] = 0.f;
           }
-          const int n = t.n_tile * BN + cc * 32;
-          if (m < p.M && n < p.N) store_bf16x32(orow + n, v);
+          stg_put_row(stg0, lane, v);
+          __syncwarp();
+          if (rows_valid > 0) stg_to_global(stg0, obase + n, p.N, lane, rows_valid);
+          __syncwarp();
         }
       } else {
-        const int row = t.m_tile * BM + r_in_tile;
-        const bool row_ok = dense ? row < p.dense_rows : true;
+        const int rows_valid = dense ? min(32, p.dense_rows - row0) : 32;
         if (MODE == FWD1) {
-          const size_t base = (size_t)row * p.ld + (size_t)t.part * p.F;
+          mbar_wait(smem_u32(&tfull_bar[as]), aphase);
+          tc_fence_after();
+          const size_t base = (size_t)row0 * p.ld + (size_t)t.part * p.F;
 #pragma unroll 1
           for (int cc = 0; cc < (BN / 2) / 32; ++cc) {
+            const int n = t.n_tile * (BN / 2) + cc * 32;
+            if (n >= p.F) break;
             float a[32], u[32];
             tmem_ld32(taddr + cc * 32, a);
             tmem_ld32(taddr + BN / 2 + cc * 32, u);
             tmem_ld_wait();
-            const int n = t.n_tile * (BN / 2) + cc * 32;
-            if (row_ok && n < p.F) {
-              store_bf16x32(p.out0 + base + n, a);
-              store_bf16x32(p.out1 + base + n, u);
+            stg_put_row(stg0, lane, a);
+            stg_put_row(stg1, lane, u);
 #pragma unroll
-              for (int i = 0; i < 32; ++i) a[i] = __fdividef(a[i], 1.0f + __expf(-a[i])) * u[i];
-              store_bf16x32(p.out2 + base + n, a);
+            for (int i = 0; i < 32; ++i) a[i] = __fdividef(a[i], 1.0f + __expf(-a[i])) * u[i];
+            stg_put_row(stg2, lane, a);
+            __syncwarp();
+            if (rows_valid > 0) {
+              stg_to_global(stg0, p.out0 + base + n, p.ld, lane, rows_valid);
+              stg_to_global(stg1, p.out1 + base + n, p.ld, lane, rows_valid);
+              stg_to_global(stg2, p.out2 + base + n, p.ld, lane, rows_valid);
             }
-          }
-        } else if (MODE == DH) {
-          const size_t base = (size_t)row * p.ld + (size_t)t.part * p.F;
-#pragma unroll 1
-          for (int cc = 0; cc < BN / 32; ++cc) {
-            float dh[32];
-            tmem_ld32(taddr + cc * 32, dh);
-            tmem_ld_wait();
-            const int n = t.n_tile * BN + cc * 32;
-            if (row_ok && n < p.F) {
-              float a[32], u[32];
-              load_bf16x32(p.in0 + base + n, a);
-              load_bf16x32(p.in1 + base + n, u);
-#pragma unroll
-              for (int i = 0; i < 32; ++i) {
-                const float s = __fdividef(1.0f, 1.0f + __expf(-a[i]));
-                const float da = dh[i] * u[i] * s * (1.0f + a[i] * (1.0f - s));
-                u[i] = dh[i] * a[i] * s;  // du
-                a[i] = da;
-              }
-              store_bf16x32(p.out0 + base + n, a);
-              store_bf16x32(p.out1 + base + n, u);
-            }
+            __syncwarp();
           }
         } else {  // FWD2, DX: plain store of a [rows, d] tile
+          mbar_wait(smem_u32(&tfull_bar[as]), aphase);
+          tc_fence_after();
 #pragma unroll 1
           for (int cc = 0; cc < BN / 32; ++cc) {
+            const int n = t.n_tile * BN + cc * 32;
+            if (n >= p.d) break;
             float v[32];
             tmem_ld32(taddr + cc * 32, v);
             tmem_ld_wait();
-            const int n = t.n_tile * BN + cc * 32;
-            if (row_ok && n < p.d) store_bf16x32(p.out0 + (size_t)row * p.d + n, v);
+            stg_put_row(stg0, lane, v);
+            __syncwarp();
+            if (rows_valid > 0) stg_to_global(stg0, p.out0 + (size_t)row0 * p.d + n, p.d, lane, rows_valid);
+            __syncwarp();
           }
         }
       }
@@ -408,6 +472,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
         if (lane == 0) mbar_arrive(smem_u32(&tempty_bar[as]));
         if (++as == kAccStages) { as = 0; aphase ^= 1; }
       }
+    }
     }
   }
 
@@ -421,58 +486,17 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
 // ---------------------------------------------------------------------------------------------------------
 // host side: tensor maps and launches
 // ---------------------------------------------------------------------------------------------------------
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-EncodeTiledFn get_encode() {
-  static EncodeTiledFn fn = [] {
-    void* ptr = nullptr;
-    cudaDriverEntryPointQueryResult q;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
-      ptr = nullptr;
-    return (EncodeTiledFn)ptr;
-  }();
-  return fn;
-}
-
-// 2D bf16 tensor [rows, inner] row-major with row stride `ld` elements; box = 64 inner elements x box_rows rows; 128B swizzle.
-bool make_map(CUtensorMap* m, const void* ptr, uint64_t inner, uint64_t rows, uint64_t ld, uint32_t box_rows) {
-  EncodeTiledFn enc = get_encode();
-  if (!enc) return false;
-  if (rows == 0) rows = 1;
-  cuuint64_t gdim[2] = {inner, rows};
-  cuuint64_t gstride[1] = {ld * 2};
-  cuuint32_t box[2] = {64, box_rows};
-  cuuint32_t estr[2] = {1, 1};
-  CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                   CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  return r == CUDA_SUCCESS;
-}
-
-int num_sms() {
-  static int n = [] {
-    int dev = 0, v = 148;
-    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
-    return v;
-  }();
-  return n;
-}
-
 template <int MODE>
 int launch(const TmaMaps& maps, const UmmaParams& p, cudaStream_t st, const char* name) {
   static bool attr_set = false;
   if (!attr_set) {
-    FOMOE_CUDA_OK(cudaFuncSetAttribute(umma_grouped_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
+    FOMOE_CUDA_OK(cudaFuncSetAttribute(umma_grouped_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes_of(MODE)));
     attr_set = true;
   }
-  umma_grouped_kernel<MODE><<<num_sms(), kThreads, kSmemBytes, st>>>(maps, p);
+  umma_grouped_kernel<MODE><<<num_sms(), kThreads, smem_bytes_of(MODE), st>>>(maps, p);
   FOMOE_LAUNCH_OK(name);
   return FOMOE_OK;
 }
-
-#define MAP_OK(expr) \
-  do { if (!(expr)) return set_cuda_error(cudaErrorInvalidValue, "cuTensorMapEncodeTiled " #expr); } while (0)
 
 }  // namespace
 
