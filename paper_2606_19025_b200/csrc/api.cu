@@ -172,12 +172,14 @@ int fomoe_moe_bwd(const fomoe_config* cfg, const void* dy, const void* x, const 
                       : simt_ffn_bwd(*cfg, n_res, x, dy, rws, aws, sws, w, dw_gate, dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, st);
   if (rc != FOMOE_OK) return rc;
   // B6, B7
-  rc = launch_gate_bwd(*cfg, *route, rws, sws.dgate, sws.dz, st);
+  const bool tc_router = use_umma(*cfg) && cfg->T > 0;
+  rc = launch_gate_bwd(*cfg, *route, rws, sws.dgate, sws.dz, tc_router ? sws.dz_bf : nullptr, sws.Ez, st);
   if (rc != FOMOE_OK) return rc;
-  rc = simt_router_bwd(*cfg, x, w_router, sws, dw_router, st);
+  rc = tc_router ? umma_router_bwd(*cfg, x, w_router, sws, dw_router, st) : simt_router_bwd(*cfg, x, w_router, sws, dw_router, st);
   if (rc != FOMOE_OK) return rc;
   // B5
-  return launch_dx_sum(*cfg, rws, sws.dxp, cfg->n_shared > 0 ? sws.dx_sh : nullptr, sws.dx_r, dx, st);
+  return launch_dx_sum(*cfg, rws, sws.dxp, cfg->n_shared > 0 ? sws.dx_sh : nullptr, tc_router ? nullptr : sws.dx_r,
+                       tc_router ? (const void*)sws.dx_r : nullptr, dx, st);
 }
 
 int fomoe_pack_resident_deltas(const float* const w_now[3], const float* const w_start[3], int32_t n_res, int64_t elems_gate,

@@ -128,7 +128,10 @@ struct ScratchWs {
   void* dsa;       // [T, n_sh*F_sh]
   void* dsu;       // [T, n_sh*F_sh]
   void* dx_sh;     // [T, d]
-  float* dwr_part; // [kRouterSplit, d, E] fp32 split-K partials of dW_r
+  float* dwr_part; // [kRouterSplit, d, Ez] fp32 split-K partials of dW_r
+  void* dz_bf;     // [T, Ez] bf16 dz, Ez = E rounded up to 64 (tensor-core router backward)
+  void* wr_bf;     // [d, Ez] bf16 W_r
+  int Ez;
   size_t bytes;
 };
 constexpr int kRouterSplit = 32;
@@ -150,7 +153,10 @@ inline ScratchWs carve_scratch_ws(const fomoe_config& c, int R_cap, void* base) 
   w.dsa = take(es * (size_t)c.T * fs);
   w.dsu = take(es * (size_t)c.T * fs);
   w.dx_sh = take(es * (size_t)c.T * c.d_model);
-  w.dwr_part = (float*)take(sizeof(float) * (size_t)kRouterSplit * c.d_model * c.E);
+  w.Ez = (c.E + 63) / 64 * 64;
+  w.dwr_part = (float*)take(sizeof(float) * (size_t)kRouterSplit * c.d_model * w.Ez);
+  w.dz_bf = take(sizeof(__nv_bfloat16) * (size_t)c.T * w.Ez);
+  w.wr_bf = take(sizeof(__nv_bfloat16) * (size_t)c.d_model * w.Ez);
   w.bytes = off;
   return w;
 }
@@ -171,9 +177,9 @@ int launch_combine(const fomoe_config& c, const fomoe_route_state& r, const Rout
 int launch_combine_bwd(const fomoe_config& c, const void* dy, const void* o, const RouteWs& ws, void* dop, float* dgate,
                        cudaStream_t st);
 int launch_gate_bwd(const fomoe_config& c, const fomoe_route_state& r, const RouteWs& ws, const float* dgate, float* dz,
-                    cudaStream_t st);
-int launch_dx_sum(const fomoe_config& c, const RouteWs& ws, const void* dxp, const void* dx_sh, const float* dx_r, void* dx,
-                  cudaStream_t st);
+                    void* dz_bf, int ldz_bf, cudaStream_t st);
+int launch_dx_sum(const fomoe_config& c, const RouteWs& ws, const void* dxp, const void* dx_sh, const float* dx_r, const void* dx_r_t,
+                  void* dx, cudaStream_t st);
 
 // fp32-accumulate SIMT GEMM path, simt_gemm.cu (all shapes, both dtypes)
 struct FfnPtrs {
@@ -194,6 +200,9 @@ int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs&
 int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy, const RouteWs& rws, const ActWs& aws,
                  const ScratchWs& sws, const FfnPtrs& w, void* dw_gate, void* dw_up, void* dw_down, void* d_sh_gate,
                  void* d_sh_up, void* d_sh_down, cudaStream_t st);
+
+// B7 on tensor cores: dx_r (bf16, into sws.dx_r reinterpreted) = dz W_r^T and dW_r = x^T dz (split-K, fp32 partials)
+int umma_router_bwd(const fomoe_config& c, const void* x, const float* w_router, const ScratchWs& sws, float* dw_router, cudaStream_t st);
 
 int launch_pack(const float* const w_now[3], const float* const w_start[3], int n_res, int64_t eg, int64_t eu, int64_t ed,
                 const int32_t* pack_slots, int n_pack, float* payload, cudaStream_t st);

@@ -122,10 +122,12 @@ combine_bwd_kernel(const T* __restrict__ dy, const T* __restrict__ o, const int3
 }
 
 // Gate rule + gate function backward (row B6): dz[t,:] from dgate[t,:].  One warp per token.
+// DZ = float (row stride E) or bf16 (row stride ldz >= E, padding columns zeroed: K-operand of the tensor-core router backward)
+template <typename DZ>
 __global__ void gate_bwd_kernel(const float* __restrict__ probs, const int32_t* __restrict__ topk_idx,
                                 const float* __restrict__ gate, const int32_t* __restrict__ pair_prow,
                                 const float* __restrict__ dgate, int T_, int E, int k, int gate_fn, int gate_rule,
-                                float inv_tau, float* __restrict__ dz) {
+                                float inv_tau, DZ* __restrict__ dz, int ldz) {
   const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (warp >= T_) return;
   const int t = warp;
@@ -154,23 +156,24 @@ __global__ void gate_bwd_kernel(const float* __restrict__ probs, const int32_t* 
     dp = (in_norm && ssum > 0.f) ? ((kept ? dg : 0.f) - dgg) / ssum : 0.f;
   }
   if (gate_fn == FOMOE_GATE_SIGMOID) {
-    for (int ee = lane; ee < E; ee += 32) dz[(size_t)t * E + ee] = 0.f;
+    for (int ee = lane; ee < ldz; ee += 32) dz[(size_t)t * ldz + ee] = from_f32<DZ>(0.f);
     __syncwarp();
-    if (lane < k) dz[(size_t)t * E + e] = dp * p * (1.f - p) * inv_tau;
+    if (lane < k) dz[(size_t)t * ldz + e] = from_f32<DZ>(dp * p * (1.f - p) * inv_tau);
   } else {
     float pd = lane < k ? p * dp : 0.f;
 #pragma unroll
     for (int s = 16; s > 0; s >>= 1) pd += __shfl_xor_sync(0xffffffffu, pd, s);
-    for (int ee = lane; ee < E; ee += 32) dz[(size_t)t * E + ee] = probs[(size_t)t * E + ee] * (0.f - pd) * inv_tau;
+    for (int ee = lane; ee < ldz; ee += 32)
+      dz[(size_t)t * ldz + ee] = from_f32<DZ>(ee < E ? probs[(size_t)t * E + ee] * (0.f - pd) * inv_tau : 0.f);
     __syncwarp();
-    if (lane < k) dz[(size_t)t * E + e] = p * (dp - pd) * inv_tau;
+    if (lane < k) dz[(size_t)t * ldz + e] = from_f32<DZ>(p * (dp - pd) * inv_tau);
   }
 }
 
-// dx[t] = sum_{j ascending} dxp[pair_prow[t,j]] + dx_sh[t] + dx_r[t]
+// dx[t] = sum_{j ascending} dxp[pair_prow[t,j]] + dx_sh[t] + dx_r[t]   (router term as fp32 or in the element type)
 template <typename T, int V>
 __global__ void __launch_bounds__(kRowThreads)
-dx_sum_kernel(const T* __restrict__ dxp, const T* __restrict__ dx_sh, const float* __restrict__ dx_r,
+dx_sum_kernel(const T* __restrict__ dxp, const T* __restrict__ dx_sh, const float* __restrict__ dx_r, const T* __restrict__ dx_r_t,
               const int32_t* __restrict__ pair_prow, int T_, int d, int k, T* __restrict__ dx) {
   for (int t = blockIdx.x; t < T_; t += gridDim.x) {
     for (int c = threadIdx.x * V; c < d; c += kRowThreads * V) {
@@ -187,6 +190,12 @@ dx_sum_kernel(const T* __restrict__ dxp, const T* __restrict__ dx_sh, const floa
       if (dx_r) {
 #pragma unroll
         for (int i = 0; i < V; ++i) acc.v[i] += dx_r[(size_t)t * d + c + i];
+      }
+      if (dx_r_t) {
+        Vec<T, V> a;
+        a.load(dx_r_t + (size_t)t * d + c);
+#pragma unroll
+        for (int i = 0; i < V; ++i) acc.v[i] += a.v[i];
       }
       acc.store(dx + (size_t)t * d + c);
     }
@@ -231,19 +240,23 @@ int launch_combine_bwd(const fomoe_config& c, const void* dy, const void* o, con
 }
 
 int launch_gate_bwd(const fomoe_config& c, const fomoe_route_state& r, const RouteWs& ws, const float* dgate, float* dz,
-                    cudaStream_t st) {
+                    void* dz_bf, int ldz_bf, cudaStream_t st) {
   if (c.T == 0) return FOMOE_OK;
-  gate_bwd_kernel<<<ceil_div(c.T, 8), 256, 0, st>>>(r.probs, r.topk_idx, r.gate, ws.pair_prow, dgate, c.T, c.E, c.top_k,
-                                                    c.gate_fn, c.gate_rule, 1.0f / c.temperature, dz);
+  if (dz_bf)
+    gate_bwd_kernel<__nv_bfloat16><<<ceil_div(c.T, 8), 256, 0, st>>>(r.probs, r.topk_idx, r.gate, ws.pair_prow, dgate, c.T, c.E, c.top_k,
+                                                                     c.gate_fn, c.gate_rule, 1.0f / c.temperature, (__nv_bfloat16*)dz_bf, ldz_bf);
+  else
+    gate_bwd_kernel<float><<<ceil_div(c.T, 8), 256, 0, st>>>(r.probs, r.topk_idx, r.gate, ws.pair_prow, dgate, c.T, c.E, c.top_k,
+                                                             c.gate_fn, c.gate_rule, 1.0f / c.temperature, dz, c.E);
   FOMOE_LAUNCH_OK("gate_bwd_kernel");
   return FOMOE_OK;
 }
 
-int launch_dx_sum(const fomoe_config& c, const RouteWs& ws, const void* dxp, const void* dx_sh, const float* dx_r, void* dx,
-                  cudaStream_t st) {
+int launch_dx_sum(const fomoe_config& c, const RouteWs& ws, const void* dxp, const void* dx_sh, const float* dx_r, const void* dx_r_t,
+                  void* dx, cudaStream_t st) {
   if (c.T == 0) return FOMOE_OK;
-  ROWS_DISPATCH(c, (dx_sum_kernel<T, V><<<row_grid(c.T), kRowThreads, 0, st>>>((const T*)dxp, (const T*)dx_sh, dx_r, ws.pair_prow,
-                                                                               c.T, c.d_model, c.top_k, (T*)dx)));
+  ROWS_DISPATCH(c, (dx_sum_kernel<T, V><<<row_grid(c.T), kRowThreads, 0, st>>>((const T*)dxp, (const T*)dx_sh, dx_r, (const T*)dx_r_t,
+                                                                               ws.pair_prow, c.T, c.d_model, c.top_k, (T*)dx)));
   FOMOE_LAUNCH_OK("dx_sum_kernel");
   return FOMOE_OK;
 }

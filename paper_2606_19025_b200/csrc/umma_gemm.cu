@@ -57,6 +57,8 @@ struct UmmaParams {
   int ld;                      // leading dimension of the [rows, hidden] activations (F, or parts*F for dense)
   int M, N;                    // WGRAD: output rows / cols per group
   int a_gcol, b_gcol;          // WGRAD dense: per-group column offset into A / B
+  int k_chunk;                 // WGRAD dense: > 0 = split-K, group g reduces rows [g*k_chunk, (g+1)*k_chunk)
+  float* out_f32;              // WGRAD: if set, fp32 output [n_groups, M, N] instead of out0
   bf16 *out0, *out1, *out2;    // FWD1: a,u,h | FWD2/DX: out | DH: da,du | WGRAD: dW
   const bf16 *in0, *in1;       // DH: a,u
 };
@@ -168,6 +170,7 @@ struct Sched {
       t.slot = t.part = t.group;
       int r0, r1;
       if (p.pad_offsets) { r0 = p.pad_offsets[t.group]; r1 = p.pad_offsets[t.group + 1]; }
+      else if (p.k_chunk > 0) { r0 = min(t.group * p.k_chunk, p.dense_rows); r1 = min(r0 + p.k_chunk, p.dense_rows); }
       else { r0 = 0; r1 = p.dense_rows; }
       t.k_row0 = r0;
       t.num_kb = (r1 - r0 + BK - 1) / BK;
@@ -417,6 +420,14 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
 #pragma unroll
             for (int i = 0; i < 32; ++i) v[i] = 0.f;
           }
+          if (p.out_f32) {  // split-K partials (small): one 128-byte row segment per thread
+            if (lane < rows_valid) {
+              float4* dst = reinterpret_cast<float4*>(p.out_f32 + ((size_t)t.group * p.M + row0 + lane) * p.N + n);
+#pragma unroll
+              for (int i = 0; i < 8; ++i) dst[i] = make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
+            }
+            continue;
+          }
           stg_put_row(stg0, lane, v);
           __syncwarp();
           if (rows_valid > 0) stg_to_global(stg0, obase + n, p.N, lane, rows_valid);
@@ -656,6 +667,69 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
       int rc = launch<WGRAD>(m, q, st, "umma_grouped_kernel<WGRAD,shared>");
       if (rc != FOMOE_OK) return rc;
     }
+  }
+  return FOMOE_OK;
+}
+
+
+namespace {
+__global__ void wr_to_bf16_kernel(const float* __restrict__ w_r, int d, int E, int Ez, bf16* __restrict__ out) {
+  const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (long)d * Ez) return;
+  const int i = (int)(idx / Ez), e = (int)(idx % Ez);
+  out[idx] = __float2bfloat16_rn(e < E ? w_r[(size_t)i * E + e] : 0.f);
+}
+__global__ void reduce_wr_parts_kernel(const float* __restrict__ part, int n_parts, int d, int E, int Ez, float* __restrict__ out) {
+  const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (long)d * E) return;
+  const int i = (int)(idx / E), e = (int)(idx % E);
+  float s = 0.f;
+  for (int g = 0; g < n_parts; ++g) s += part[((size_t)g * d + i) * Ez + e];  // fixed order
+  out[idx] = s;
+}
+}  // namespace
+
+int umma_router_bwd(const fomoe_config& c, const void* x, const float* w_router, const ScratchWs& sws, float* dw_router, cudaStream_t st) {
+  const int d = c.d_model, E = c.E, Ez = sws.Ez, T = c.T;
+  {
+    const long n = (long)d * Ez;
+    wr_to_bf16_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(w_router, d, E, Ez, (bf16*)sws.wr_bf);
+    FOMOE_LAUNCH_OK("wr_to_bf16_kernel");
+  }
+  {  // dx_r [T,d] = dz [T,Ez] W_r^T : FWD2 shape on dense rows (A = dz, K = Ez; B = W_r [d,Ez] K-major)
+    UmmaParams p{};
+    p.dense_rows = T; p.parts = 1; p.d = d; p.F = Ez; p.ld = Ez;
+    TmaMaps m{};
+    MAP_OK(make_map(&m.m[0], sws.dz_bf, Ez, T, Ez, 128));
+    MAP_OK(make_map(&m.m[1], sws.wr_bf, Ez, d, Ez, 256));
+    m.m[2] = m.m[3] = m.m[0];
+    p.out0 = (bf16*)sws.dx_r;
+    int rc = launch<FWD2>(m, p, st, "umma_grouped_kernel<FWD2,router dx>");
+    if (rc != FOMOE_OK) return rc;
+  }
+  // dW_r [d,E] = x^T dz : WGRAD shape, split over tokens into G groups, fp32 partials, fixed-order reduce
+  const int m_tiles = (d + BM - 1) / BM;
+  int G = (2 * num_sms() + m_tiles - 1) / m_tiles;
+  if (G > kRouterSplit) G = kRouterSplit;
+  if (G > (T + 511) / 512) G = (T + 511) / 512;
+  if (G < 1) G = 1;
+  const int k_chunk = ((T + G - 1) / G + 63) / 64 * 64;
+  G = (T + k_chunk - 1) / k_chunk;
+  {
+    UmmaParams p{};
+    p.dense_rows = T; p.parts = 1; p.d = d; p.F = Ez; p.ld = Ez;
+    p.n_groups = G; p.M = d; p.N = Ez; p.k_chunk = k_chunk; p.out_f32 = sws.dwr_part;
+    TmaMaps m{};
+    MAP_OK(make_map(&m.m[0], x, d, T, d, 64));
+    MAP_OK(make_map(&m.m[1], sws.dz_bf, Ez, T, Ez, 64));
+    m.m[2] = m.m[3] = m.m[0];
+    int rc = launch<WGRAD>(m, p, st, "umma_grouped_kernel<WGRAD,router dW>");
+    if (rc != FOMOE_OK) return rc;
+  }
+  {
+    const long n = (long)d * E;
+    reduce_wr_parts_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(sws.dwr_part, G, d, E, Ez, dw_router);
+    FOMOE_LAUNCH_OK("reduce_wr_parts_kernel");
   }
   return FOMOE_OK;
 }

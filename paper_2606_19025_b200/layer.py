@@ -79,6 +79,21 @@ class SkipTokenMoE:
         self.launches = n
         return n
 
+    def capture_step(self, x: torch.Tensor, dy: torch.Tensor):
+        """Captures route + forward + backward on (x, dy) into a CUDA graph (no entry point syncs or reads back, so the
+        whole step is capturable).  Returns a callable that replays it; inputs are read from the captured buffers."""
+        s = torch.cuda.Stream()
+        s.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(s):
+            for _ in range(2):  # warm up: first-call attribute setup must not happen during capture
+                n = self.step(x, dy)
+        torch.cuda.current_stream().wait_stream(s)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            self.step(x, dy)
+        self.launches = n
+        return g.replay
+
     def step_host(self, x_host, dy_host, y_host, dx_host, x_dev, dy_dev, stream=None, copy_stream=None) -> int:
         """Whole step from pinned HOST buffers through fomoe_moe_step_host (uploads x, dy; downloads y, dx)."""
         B.fomoe_moe_step_host(self.cfg, x_host, dy_host, y_host, dx_host, x_dev, dy_dev, self.y, self.dx, self.w_router,
