@@ -387,6 +387,42 @@ int oracle_moe_bwd(int T, int d, int E, int k, int F, int n_sh, int F_sh,
 }
 
 /* ------------------------------------------------------------------------------------------------
+ * Sampled weight gradients for the full-size parity tests (outputs "the oracle can compute one by one"):
+ * for resident slot s and each sampled hidden index f = f_idx[q], over ALL rows of the slot,
+ *   dW_gate[s,f,:] = sum_r da_rf x_r,  dW_up[s,f,:] = sum_r du_rf x_r,  dW_down[s,:,f] = sum_r do_r h_rf
+ * with do_r = g_r dy_t(r), dh_rf = <do_r, W_down[:,f]>, a_rf = <W_gate[f,:], x_r>, u_rf = <W_up[f,:], x_r>,
+ * h_rf = silu(a_rf) u_rf, da = dh u s (1 + a (1 - s)), du = dh a s   (same formulas as expert_bwd_, one f at a time).
+ * Outputs [n_f, d] each.  Pinned against oracle_moe_bwd in tests/test_oracle_pins.py.
+ * ---------------------------------------------------------------------------------------------- */
+int oracle_dw_sample(int d, int k, int F, const REAL* x, const REAL* dy, const int32_t* topk_idx, const REAL* gate,
+                     int resident_id, int row_begin, int row_end, const int32_t* row_token,
+                     const REAL* wg, const REAL* wu, const REAL* wd, /* this slot's [F,d], [F,d], [d,F] */
+                     const int32_t* f_idx, int n_f, REAL* dwg_rows, REAL* dwu_rows, REAL* dwd_cols) {
+#pragma omp parallel for schedule(static)
+  for (int q = 0; q < n_f; ++q) {
+    const int f = f_idx[q];
+    REAL *og = dwg_rows + (size_t)q * d, *ou = dwu_rows + (size_t)q * d, *od = dwd_cols + (size_t)q * d;
+    for (int i = 0; i < d; ++i) og[i] = ou[i] = od[i] = 0;
+    for (int r = row_begin; r < row_end; ++r) {
+      const int t = row_token[r];
+      int j = -1;
+      for (int jj = 0; jj < k; ++jj)
+        if (topk_idx[(size_t)t * k + jj] == resident_id) j = jj;
+      const REAL g = gate[(size_t)t * k + j];
+      const REAL *xt = x + (size_t)t * d, *dyt = dy + (size_t)t * d;
+      REAL a = dot_(wg + (size_t)f * d, xt, d), u = dot_(wu + (size_t)f * d, xt, d);
+      REAL sg = sigmoid_(a), h = a * sg * u, dh = 0;
+      for (int i = 0; i < d; ++i) dh += g * dyt[i] * wd[(size_t)i * F + f];
+      REAL da = dh * u * sg * ((REAL)1 + a * ((REAL)1 - sg)), du = dh * a * sg;
+      axpy_(da, xt, og, d);
+      axpy_(du, xt, ou, d);
+      axpy_(g * h, dyt, od, d);
+    }
+  }
+  return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------
  * Step 10: resident-delta pack, always fp32 (BASELINE.json config 4 "fp32 resident-delta pack").
  * payload block b (b-th entry of pack_slots, or slot b if pack_slots == NULL) =
  *   [ w_start_gate - w_now_gate | w_start_up - w_now_up | w_start_down - w_now_down ]  of that slot

@@ -42,7 +42,7 @@ class Oracle:
         self.real = real
         self.lib = C.CDLL(str(_HERE / lib))
         assert self.lib.oracle_real_bytes() == np.dtype(self.dt).itemsize
-        for fn in ("oracle_route", "oracle_moe_fwd", "oracle_moe_bwd", "oracle_pack_resident_deltas"):
+        for fn in ("oracle_route", "oracle_moe_fwd", "oracle_moe_bwd", "oracle_pack_resident_deltas", "oracle_dw_sample"):
             getattr(self.lib, fn).restype = C.c_int
 
     @staticmethod
@@ -130,6 +130,24 @@ class Oracle:
         if rc != 0:
             raise ValueError(f"oracle_moe_bwd rc={rc}")
         return out
+
+    # ---- sampled weight gradients (full-size parity) -----------------------------------------------
+    def dw_sample(self, x, dy, route, resident, slot, f_idx, w_gate_s, w_up_s, w_down_s):
+        """dW_gate[slot, f, :], dW_up[slot, f, :], dW_down[slot, :, f] for f in f_idx; weights are that slot's matrices."""
+        x, dy = self._r(x), self._r(dy)
+        wg, wu, wd = self._r(w_gate_s), self._r(w_up_s), self._r(w_down_s)
+        F, d = wg.shape
+        k = route["topk_idx"].shape[1]
+        f_idx = np.ascontiguousarray(f_idx, dtype=np.int32)
+        outs = [np.empty((len(f_idx), d), self.dt) for _ in range(3)]
+        rc = self.lib.oracle_dw_sample(C.c_int(d), C.c_int(k), C.c_int(F), _ptr(x), _ptr(dy), _ptr(route["topk_idx"]),
+                                       _ptr(self._r(route["gate"])), C.c_int(int(resident[slot])),
+                                       C.c_int(int(route["offsets"][slot])), C.c_int(int(route["offsets"][slot + 1])),
+                                       _ptr(route["row_token"]), _ptr(wg), _ptr(wu), _ptr(wd), _ptr(f_idx), C.c_int(len(f_idx)),
+                                       _ptr(outs[0]), _ptr(outs[1]), _ptr(outs[2]))
+        if rc != 0:
+            raise ValueError(f"oracle_dw_sample rc={rc}")
+        return outs
 
     # ---- step 10 ---------------------------------------------------------------------------------
     def pack(self, w_now, w_start, pack_slots=None):

@@ -284,6 +284,19 @@ def test_f32_build_matches_f64(oracle32, oracle64):
         assert np.abs(b32[key] - b64[key]).max() <= 1e-5 * np.abs(b64[key]).max(), key
 
 
+def test_dw_sample_matches_full_backward(oracle64):
+    """The sampled-row weight-gradient helper used by the full-size GPU tests equals the (autograd-pinned) full backward."""
+    prob = refs.tiny_problem(21, T=90, d=10, E=6, k=2, F=9, n_res=3)
+    wg, wu, wd = refs.resident_stacks(prob)
+    r, _, b = run_oracle(oracle64, prob)
+    f_idx = np.array([0, 4, 8], np.int32)
+    for slot in range(3):
+        g, u, dn = oracle64.dw_sample(prob["x"], prob["dy"], r, prob["resident"], slot, f_idx, wg[slot], wu[slot], wd[slot])
+        np.testing.assert_allclose(g, b["dw_gate"][slot][f_idx], rtol=1e-11, atol=1e-13)
+        np.testing.assert_allclose(u, b["dw_up"][slot][f_idx], rtol=1e-11, atol=1e-13)
+        np.testing.assert_allclose(dn, b["dw_down"][slot][:, f_idx].T, rtol=1e-11, atol=1e-13)
+
+
 def test_pack_bit_exact_and_layout(oracle64):
     rng = np.random.default_rng(2)
     n_res, F, d = 5, 6, 4
