@@ -153,6 +153,7 @@ def run_gpu(args, w, n_res):
     import torch.distributed as dist
 
     from paper_2606_19025_b200 import binding as B
+    from paper_2606_19025_b200 import replicas
     from paper_2606_19025_b200.layer import SkipTokenMoE, pack_resident_deltas
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -176,8 +177,7 @@ def run_gpu(args, w, n_res):
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
 
     def barrier_all():
-        if world > 1:
-            dist.barrier()
+        replicas.barrier()
         torch.cuda.synchronize()
 
     def timed_steps(fn, steps, warmup, collective=False):
@@ -212,12 +212,8 @@ def run_gpu(args, w, n_res):
     sampler.start()
     ms_list = timed_steps(step, args.steps, args.warmup, collective=True)
     clocks = sampler.stop()
-    ms = sum(ms_list) / len(ms_list)
-    if world > 1:
-        t = torch.tensor([ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * w.T / (ms / 1e3)
+    ms = replicas.max_over_ranks(sum(ms_list) / len(ms_list), "cuda")
+    value = replicas.whole_job_tokens_per_s(w.T, ms)
 
     routing = layer.routing_numpy()
     P = routing["P"]
