@@ -47,8 +47,9 @@ struct RouteWs {
   int32_t* slot_of;     // [E]            resident slot of expert e or -1 (ghost)
   int32_t* blk_hist;    // [n_blk, n_res] kept pairs per (permutation block, slot); then exclusive over blocks
   int32_t* pad_offsets; // [n_res+1]      first padded row of slot s (multiples of kTileM)
-  int32_t* n_mtiles;    // [4]            [0] = number of kTileM-row tiles in use, [1] = padded rows in use
+  int32_t* n_mtiles;    // [4]            [0] = number of kTileM-row tiles in use, [1] = padded rows in use, [2] = tile pairs
   int32_t* tile_slot;   // [max_mtiles]   slot of row tile i
+  int32_t* pair_info;   // [max_mtiles]   CTA-pair work items: 2 * first row tile + (second tile belongs to the same slot)
   int32_t* prow_token;  // [R_cap]        token of padded row r, -1 for padding rows
   float* prow_gate;     // [R_cap]        gate of padded row r
   int32_t* prow_pair;   // [R_cap]        t*k+j of padded row r
@@ -74,6 +75,7 @@ inline RouteWs carve_route_ws(const fomoe_config& c, int n_res, void* base) {
   w.pad_offsets = (int32_t*)take(sizeof(int32_t) * (size_t)(n_res + 1));
   w.n_mtiles = (int32_t*)take(sizeof(int32_t) * 4);
   w.tile_slot = (int32_t*)take(sizeof(int32_t) * (size_t)w.max_mtiles);
+  w.pair_info = (int32_t*)take(sizeof(int32_t) * (size_t)w.max_mtiles);
   w.prow_token = (int32_t*)take(sizeof(int32_t) * (size_t)w.R_cap);
   w.prow_gate = (float*)take(sizeof(float) * (size_t)w.R_cap);
   w.prow_pair = (int32_t*)take(sizeof(int32_t) * (size_t)w.R_cap);

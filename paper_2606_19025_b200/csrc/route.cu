@@ -172,8 +172,9 @@ __global__ void perm_hist_kernel(const int32_t* __restrict__ topk_idx, const int
 // offsets, the row-tile -> slot map and the number of tiles in use.
 __global__ void perm_scan_kernel(int32_t* __restrict__ blk_hist, int n_blk, int n_res, int32_t* __restrict__ counts,
                                  int32_t* __restrict__ offsets, int32_t* __restrict__ pad_offsets,
-                                 int32_t* __restrict__ n_mtiles, int32_t* __restrict__ tile_slot) {
+                                 int32_t* __restrict__ n_mtiles, int32_t* __restrict__ tile_slot, int32_t* __restrict__ pair_info) {
   __shared__ int32_t s_pad[kMaxE + 1];
+  __shared__ int32_t s_pair[kMaxE + 1];  // first tile pair of slot s (a pair = two row tiles of ONE slot, the last may be single)
   for (int s = threadIdx.x; s < n_res; s += blockDim.x) {
     int run = 0;
     for (int b = 0; b < n_blk; ++b) {
@@ -185,23 +186,32 @@ __global__ void perm_scan_kernel(int32_t* __restrict__ blk_hist, int n_blk, int 
   }
   __syncthreads();
   if (threadIdx.x == 0) {
-    int off = 0, pad = 0;
+    int off = 0, pad = 0, pairs = 0;
     for (int s = 0; s < n_res; ++s) {
       offsets[s] = off;
       pad_offsets[s] = pad;
       s_pad[s] = pad;
+      s_pair[s] = pairs;
       off += counts[s];
-      pad += (counts[s] + kTileM - 1) / kTileM * kTileM;
+      const int tiles = (counts[s] + kTileM - 1) / kTileM;
+      pad += tiles * kTileM;
+      pairs += (tiles + 1) / 2;
     }
     offsets[n_res] = off;
     pad_offsets[n_res] = pad;
     s_pad[n_res] = pad;
+    s_pair[n_res] = pairs;
     n_mtiles[0] = pad / kTileM;
     n_mtiles[1] = pad;
+    n_mtiles[2] = pairs;
   }
   __syncthreads();
-  for (int s = 0; s < n_res; ++s)
-    for (int i = s_pad[s] / kTileM + threadIdx.x; i < s_pad[s + 1] / kTileM; i += blockDim.x) tile_slot[i] = s;
+  for (int s = 0; s < n_res; ++s) {
+    const int t0 = s_pad[s] / kTileM, t1 = s_pad[s + 1] / kTileM;
+    for (int i = t0 + threadIdx.x; i < t1; i += blockDim.x) tile_slot[i] = s;
+    for (int i = threadIdx.x; i < s_pair[s + 1] - s_pair[s]; i += blockDim.x)
+      pair_info[s_pair[s] + i] = 2 * (t0 + 2 * i) + (t0 + 2 * i + 1 < t1 ? 1 : 0);
+  }
 }
 
 constexpr int kPermThreads = 256;
@@ -310,7 +320,7 @@ int launch_route(const fomoe_config& c, const void* x, const float* w_router, co
     FOMOE_LAUNCH_OK("perm_hist_kernel");
   }
   perm_scan_kernel<<<1, 256, 0, st>>>(ws.blk_hist, ws.n_blk, n_res, out.counts, out.offsets, ws.pad_offsets, ws.n_mtiles,
-                                      ws.tile_slot);
+                                      ws.tile_slot, ws.pair_info);
   FOMOE_LAUNCH_OK("perm_scan_kernel");
   perm_scatter_kernel<<<ws.n_blk, kPermThreads, sizeof(int32_t) * 9 * nr, st>>>(
       out.topk_idx, out.gate, ws.slot_of, ws.blk_hist, out.offsets, ws.pad_offsets, n_pairs, pairs_per_blk, c.top_k, n_res,

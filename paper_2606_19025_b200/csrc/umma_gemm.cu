@@ -1,22 +1,27 @@
 // tcgen05 / TMEM / TMA grouped GEMMs for the resident-expert SwiGLU FFN, forward and backward
 // (rows F6, F6s, F7, B2, B3, B4 of SURVEY.md §8(a)); bf16 operands, fp32 accumulation in tensor memory.
 //
-// One persistent, warp-specialised kernel template (one CTA per SM, 256 threads):
-//   warp 0  : TMA producer   (cp.async.bulk.tensor.2d -> 128B-swizzled shared-memory stages, mbarrier complete_tx)
-//   warp 1  : MMA issuer     (one elected lane issues tcgen05.mma.cta_group::1.kind::f16, M=128 N=256 K=16)
-//   warp 2  : TMEM allocator (512 columns = two 128x256 fp32 accumulator stages)
-//   warps 4-7: epilogue      (tcgen05.ld 32x32b -> registers -> fused math -> 16-byte global stores)
+// One persistent, warp-specialised kernel template.  CTAs run as PAIRS (cluster of 2 on one TPC, cta_group::2): one
+// tcgen05.mma covers 256 rows x 256 columns, each CTA staging its own 128 rows of A and HALF of the columns of B, so
+// shared-memory and L2 operand traffic per flop is 2/3 of the single-CTA 128 x 256 tile.  Per CTA, 256 threads:
+//   warp 0  : TMA producer   (cp.async.bulk.tensor.2d -> 128B-swizzled shared-memory stages; both CTAs' loads signal
+//                             the LEADER's mbarrier with complete_tx)
+//   warp 1  : MMA issuer     (leader CTA only: one elected lane issues tcgen05.mma.cta_group::2.kind::f16, M=256 N<=256
+//                             K=16; tcgen05.commit multicasts stage release / accumulator-full to both CTAs)
+//   warp 2  : TMEM allocator (512 columns = two 128x256 fp32 accumulator stages per CTA)
+//   warps 4-7: epilogue      (tcgen05.ld 32x32b -> registers -> fused math -> 16-byte global stores of this CTA's rows)
 // Three pipelines: shared-memory full/empty (TMA <-> MMA), TMEM full/empty (MMA <-> epilogue), static round-robin
-// tile scheduler.  The number of row tiles is data dependent and is read from device memory (route workspace): the
-// host never learns P.
+// tile scheduler over clusters.  The number of row tiles is data dependent and is read from device memory (route
+// workspace): the host never learns P.
 //
-// Modes (all with a 128 x 256 accumulator tile, K staged 64 at a time):
-//   FWD1  [a|u] = X W_gate^T | X W_up^T   (A, B K-major; epilogue: a, u, h = silu(a)*u)
+// Modes (pair tile 256 x 256, K staged 64 at a time):
+//   FWD1  [a|u] = X W_gate^T | X W_up^T   (A, B K-major; CTA0 stages W_gate, CTA1 W_up; epilogue: a, u, h = silu(a)*u)
 //   FWD2  o = H W_down^T                  (A, B K-major)
 //   DH    dh = dO W_down                  (A K-major, B MN-major; epilogue: SwiGLU backward -> da, du)
 //   DX    dxp = dA W_gate + dU W_up       (A K-major, B MN-major; two K segments into one accumulator)
 //   WGRAD dW[g] = A[rows(g)]^T B[rows(g)] (A, B MN-major; K = the group's (padded) rows)
-// Row space is either the tile-padded routed rows (slot per 128-row tile) or dense rows (shared experts).
+// Row space is either the tile-padded routed rows (pairs of 128-row tiles of ONE slot; the last pair of a slot may hold a
+// single tile, then CTA 1 computes rows nobody stores) or dense rows (shared experts).
 #include <cuda.h>
 
 #include "common.cuh"
@@ -25,16 +30,18 @@
 namespace fomoe {
 namespace {
 
-constexpr int BM = 128, BN = 256, BK = 64, kAccStages = 2;
-constexpr int kABytes = BM * BK * 2, kBBytes = BN * BK * 2, kStageBytes = kABytes + kBBytes;
+constexpr int BM = 128;   // rows per CTA (256 per pair)
+constexpr int BN = 256;   // accumulator columns (each CTA stages BN/2 columns of B)
+constexpr int BK = 64, kAccStages = 2;
+constexpr int kABytes = BM * BK * 2, kBBytes = (BN / 2) * BK * 2, kStageBytes = kABytes + kBBytes;
 constexpr int kThreads = 256;
 // epilogue staging: per epilogue warp, up to 3 swizzled tiles of 32 rows x 32 bf16 (2 KB each) used to turn the
 // row-per-thread TMEM layout into coalesced 16-byte global accesses
 constexpr int kStgTile = 2048;
 constexpr int kDhDepth = 4;  // DH epilogue: chunks of (a, u) kept in flight per warp with cp.async
 enum Mode { FWD1 = 0, FWD2 = 1, DH = 2, DX = 3, WGRAD = 4 };
-// DH trades one TMA stage for a deep epilogue prefetch ring: its epilogue must stream a and u back in
-__host__ __device__ constexpr int stages_of(int mode) { return mode == DH ? 3 : 4; }
+// DH trades TMA stages for a deep epilogue prefetch ring: its epilogue must stream a and u back in
+__host__ __device__ constexpr int stages_of(int mode) { return mode == DH ? 4 : 6; }
 __host__ __device__ constexpr int stg_tiles_per_warp(int mode) { return mode == DH ? 2 * kDhDepth + 2 : 3; }
 __host__ __device__ constexpr int stg_bytes_of(int mode) { return 4 * stg_tiles_per_warp(mode) * kStgTile; }
 __host__ __device__ constexpr int smem_bytes_of(int mode) {
@@ -47,8 +54,9 @@ struct TmaMaps {
 };
 
 struct UmmaParams {
-  const int32_t* n_mtiles;     // routed: device, [0] = row tiles in use; nullptr = dense rows
+  const int32_t* n_mtiles;     // routed: device, [2] = tile pairs in use; nullptr = dense rows
   const int32_t* tile_slot;    // routed: slot of row tile
+  const int32_t* pair_info;    // routed: 2 * first row tile + (second tile in the same slot)
   const int32_t* pad_offsets;  // routed WGRAD: padded row range of group g
   int dense_rows;              // dense: number of rows (T)
   int parts;                   // dense: number of shared experts (1 for routed)
@@ -107,66 +115,58 @@ __device__ __forceinline__ void stg_to_global(const uint8_t* stg, bf16* g, size_
     if (r < rows_valid) *reinterpret_cast<uint4*>(g + (size_t)r * ld + c * 8) = w;
   }
 }
-// whole warp: global -> registers (issue early), then registers -> staging tile
-__device__ __forceinline__ void global_to_regs(const bf16* g, size_t ld, int lane, int rows_valid, uint4 (&w)[4]) {
-#pragma unroll
-  for (int it = 0; it < 4; ++it) {
-    const int r = it * 8 + (lane >> 2), c = lane & 3;
-    w[it] = r < rows_valid ? *reinterpret_cast<const uint4*>(g + (size_t)r * ld + c * 8) : make_uint4(0, 0, 0, 0);
-  }
-}
-__device__ __forceinline__ void regs_to_stg(uint8_t* stg, int lane, const uint4 (&w)[4]) {
-#pragma unroll
-  for (int it = 0; it < 4; ++it) {
-    const int r = it * 8 + (lane >> 2), c = lane & 3;
-    *reinterpret_cast<uint4*>(stg + stg_off(r, c)) = w[it];
-  }
-}
 
-// instruction descriptor: D fp32, A/B bf16, M=128, N=256, majorness per operand (0 = K-major, 1 = MN-major)
-__host__ __device__ constexpr uint32_t make_idesc(int a_mn, int b_mn) {
-  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)a_mn << 15) | ((uint32_t)b_mn << 16) | ((uint32_t)(BN >> 3) << 17) |
-         ((uint32_t)(BM >> 4) << 24);
+// instruction descriptor: D fp32, A/B bf16, M = 256 (pair), N = n, majorness per operand (0 = K-major, 1 = MN-major)
+__host__ __device__ constexpr uint32_t make_idesc(int a_mn, int b_mn, int n) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)a_mn << 15) | ((uint32_t)b_mn << 16) | ((uint32_t)(n >> 3) << 17) |
+         ((uint32_t)((2 * BM) >> 4) << 24);
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// tile decode shared by the three roles
+// tile decode shared by the three roles (identical in both CTAs of a pair except for the rank-dependent fields)
 // ---------------------------------------------------------------------------------------------------------
 struct Tile {
-  int m_tile, n_tile, slot, part, group;  // group: WGRAD only
-  int num_kb;                             // 64-wide K blocks
-  int k_row0;                             // WGRAD: first row of the K range
+  int row0;        // first of THIS CTA's 128 rows (row modes) / output rows (WGRAD)
+  bool live;       // this CTA's rows exist (false: second half of a single-tile pair, or beyond the row count)
+  int n_tile;      // column tile
+  int n_mma;       // N of the MMA: 256, or 128 when at most 128 columns of the tile exist
+  int slot, part, group;  // group: WGRAD only
+  int num_kb;      // 64-wide K blocks
+  int k_row0;      // WGRAD: first row of the K range
 };
 
 template <int MODE>
 struct Sched {
   const UmmaParams& p;
-  int n_tiles_n, ntn_total, m_tiles;
+  const int rank;
+  int n_tiles_n, ntn_total, m_pairs;
   long total;
-  __device__ Sched(const UmmaParams& p_) : p(p_) {
+  __device__ Sched(const UmmaParams& p_, int rank_) : p(p_), rank(rank_) {
     const bool dense = p.n_mtiles == nullptr;
     if (MODE == WGRAD) {
-      m_tiles = (p.M + BM - 1) / BM;
+      m_pairs = (p.M + 2 * BM - 1) / (2 * BM);
       n_tiles_n = (p.N + BN - 1) / BN;
       ntn_total = n_tiles_n;
-      total = (long)p.n_groups * m_tiles * n_tiles_n;
+      total = (long)p.n_groups * m_pairs * n_tiles_n;
     } else {
-      m_tiles = dense ? (p.dense_rows + BM - 1) / BM : p.n_mtiles[0];
+      m_pairs = dense ? (p.dense_rows + 2 * BM - 1) / (2 * BM) : p.n_mtiles[2];
       const int n_extent = (MODE == FWD1 || MODE == DH) ? p.F : p.d;
       const int bn = MODE == FWD1 ? BN / 2 : BN;
       n_tiles_n = (n_extent + bn - 1) / bn;
       ntn_total = n_tiles_n * ((dense && (MODE == FWD1 || MODE == DH)) ? p.parts : 1);
-      total = (long)m_tiles * ntn_total;
+      total = (long)m_pairs * ntn_total;
     }
   }
   __device__ Tile decode(long id) const {
     Tile t;
     const bool dense = p.n_mtiles == nullptr;
     if (MODE == WGRAD) {
-      t.group = (int)(id / ((long)m_tiles * n_tiles_n));
-      int rem = (int)(id % ((long)m_tiles * n_tiles_n));
-      t.m_tile = rem / n_tiles_n;
+      t.group = (int)(id / ((long)m_pairs * n_tiles_n));
+      int rem = (int)(id % ((long)m_pairs * n_tiles_n));
+      t.row0 = (rem / n_tiles_n) * 2 * BM + rank * BM;
+      t.live = t.row0 < p.M;
       t.n_tile = rem % n_tiles_n;
+      t.n_mma = (p.N - t.n_tile * BN <= BN / 2) ? BN / 2 : BN;
       t.slot = t.part = t.group;
       int r0, r1;
       if (p.pad_offsets) { r0 = p.pad_offsets[t.group]; r1 = p.pad_offsets[t.group + 1]; }
@@ -175,14 +175,26 @@ struct Sched {
       t.k_row0 = r0;
       t.num_kb = (r1 - r0 + BK - 1) / BK;
     } else {
-      t.m_tile = (int)(id / ntn_total);
+      const int pair = (int)(id / ntn_total);
       int nidx = (int)(id % ntn_total);
       t.part = nidx / n_tiles_n;
       t.n_tile = nidx % n_tiles_n;
-      t.slot = dense ? t.part : p.tile_slot[t.m_tile];
+      if (dense) {
+        t.row0 = pair * 2 * BM + rank * BM;
+        t.live = t.row0 < p.dense_rows;
+        t.slot = t.part;
+      } else {
+        const int info = p.pair_info[pair];
+        const int first = info >> 1;
+        t.row0 = (first + rank) * BM;
+        t.live = rank == 0 || (info & 1);
+        t.slot = p.tile_slot[first];
+      }
       t.group = 0;
       t.k_row0 = 0;
       const int kparts = dense ? p.parts : 1;
+      const int n_extent = (MODE == DH) ? p.F : p.d;
+      t.n_mma = (MODE != FWD1 && n_extent - t.n_tile * BN <= BN / 2) ? BN / 2 : BN;
       if (MODE == FWD1 || MODE == DH) t.num_kb = p.d / BK;
       else if (MODE == FWD2) t.num_kb = kparts * (p.F / BK);
       else t.num_kb = 2 * kparts * (p.F / BK);  // DX
@@ -195,7 +207,7 @@ struct Sched {
 // the kernel
 // ---------------------------------------------------------------------------------------------------------
 template <int MODE>
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
@@ -203,13 +215,15 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
   constexpr int kStgTilesPerWarp = stg_tiles_per_warp(MODE);
   uint8_t* stg_base = smem + kStages * kStageBytes;
   uint64_t* bars = reinterpret_cast<uint64_t*>(stg_base + stg_bytes_of(MODE));
-  uint64_t* full_bar = bars;                          // [kStages]
-  uint64_t* empty_bar = bars + kStages;               // [kStages]
-  uint64_t* tfull_bar = bars + 2 * kStages;           // [kAccStages]
-  uint64_t* tempty_bar = bars + 2 * kStages + kAccStages;  // [kAccStages]
+  uint64_t* full_bar = bars;                          // [kStages]   used in the leader CTA only
+  uint64_t* empty_bar = bars + kStages;               // [kStages]   one per CTA, released by the leader's commits
+  uint64_t* tfull_bar = bars + 2 * kStages;           // [kAccStages] one per CTA
+  uint64_t* tempty_bar = bars + 2 * kStages + kAccStages;  // [kAccStages] leader only: 4 epilogue warps x 2 CTAs
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * kStages + 2 * kAccStages);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int rank = (int)cluster_ctarank();
+  const int cluster_id = blockIdx.x >> 1, n_clusters = gridDim.x >> 1;
   constexpr bool kAMn = (MODE == WGRAD), kBMn = (MODE == DH || MODE == DX || MODE == WGRAD);
 
   if (warp == 0 && lane == 0) {
@@ -218,103 +232,108 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
   }
   if (warp == 1 && lane == 0) {
     for (int i = 0; i < kStages; ++i) { mbar_init(smem_u32(&full_bar[i]), 1); mbar_init(smem_u32(&empty_bar[i]), 1); }
-    for (int i = 0; i < kAccStages; ++i) { mbar_init(smem_u32(&tfull_bar[i]), 1); mbar_init(smem_u32(&tempty_bar[i]), 4); }
+    for (int i = 0; i < kAccStages; ++i) { mbar_init(smem_u32(&tfull_bar[i]), 1); mbar_init(smem_u32(&tempty_bar[i]), 8); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 2) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "n"(kTmemCols) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "n"(kTmemCols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
   }
   tc_fence_before();
-  __syncthreads();
+  cluster_sync_all();   // barriers of both CTAs initialised, tensor memory allocated in both
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
 
-  const Sched<MODE> sched(p);
+  const Sched<MODE> sched(p, rank);
   const bool dense = p.n_mtiles == nullptr;
 
   if (warp == 0) {
-    // ===================== TMA producer =====================
+    // ===================== TMA producer (both CTAs; completion bytes land on the leader's barrier) =====================
     if (lane == 0) {
       int stage = 0;
       uint32_t phase = 0;
-      for (long id = blockIdx.x; id < sched.total; id += gridDim.x) {
+      for (long id = cluster_id; id < sched.total; id += n_clusters) {
         const Tile t = sched.decode(id);
-        const int m0 = t.m_tile * BM;
+        const int m0 = t.row0;
+        const int nh = t.n_mma / 2;                 // B columns staged by each CTA
         for (int kb = 0; kb < t.num_kb; ++kb) {
           mbar_wait(smem_u32(&empty_bar[stage]), phase ^ 1);
-          const uint32_t sa = smem_u32(smem + stage * kStageBytes), sb = sa + kABytes, fb = smem_u32(&full_bar[stage]);
-          mbar_expect_tx(fb, kStageBytes);
+          const uint32_t sa = smem_u32(smem + stage * kStageBytes), sb = sa + kABytes;
+          const uint32_t fb = mapa_u32(smem_u32(&full_bar[stage]), 0);
+          if (rank == 0) mbar_expect_tx(smem_u32(&full_bar[stage]), 2 * kStageBytes);
           if (MODE == FWD1) {
-            tma_load_2d(sa, &maps.m[0], fb, kb * BK, m0);
-            const int brow = t.slot * p.F + t.n_tile * (BN / 2);
-            tma_load_2d(sb, &maps.m[1], fb, kb * BK, brow);
-            tma_load_2d(sb + kBBytes / 2, &maps.m[2], fb, kb * BK, brow);
+            tma_load_2d_2sm(sa, &maps.m[0], fb, kb * BK, m0);
+            // N columns [0,128) = a (W_gate rows, staged by CTA 0), [128,256) = u (W_up rows, CTA 1)
+            tma_load_2d_2sm(sb, &maps.m[1 + rank], fb, kb * BK, t.slot * p.F + t.n_tile * (BN / 2));
           } else if (MODE == FWD2) {
             const int kpp = p.F / BK, part = kb / kpp, kk = kb % kpp;
-            tma_load_2d(sa, &maps.m[0], fb, part * p.F + kk * BK, m0);
-            tma_load_2d(sb, &maps.m[1], fb, kk * BK, (dense ? part : t.slot) * p.d + t.n_tile * BN);
+            tma_load_2d_2sm(sa, &maps.m[0], fb, part * p.F + kk * BK, m0);
+            tma_load_2d_2sm(sb, &maps.m[1], fb, kk * BK, (dense ? part : t.slot) * p.d + t.n_tile * BN + rank * nh);
           } else if (MODE == DH) {
-            tma_load_2d(sa, &maps.m[0], fb, kb * BK, m0);
+            tma_load_2d_2sm(sa, &maps.m[0], fb, kb * BK, m0);
 #pragma unroll
-            for (int j = 0; j < BN / 64; ++j)
-              tma_load_2d(sb + j * 8192, &maps.m[1], fb, t.n_tile * BN + 64 * j, t.slot * p.d + kb * BK);
+            for (int j = 0; j < BN / 128; ++j)
+              tma_load_2d_2sm(sb + j * 8192, &maps.m[1], fb, t.n_tile * BN + rank * nh + 64 * j, t.slot * p.d + kb * BK);
           } else if (MODE == DX) {
             const int kseg = (dense ? p.parts : 1) * (p.F / BK), seg = kb / kseg, kk = kb % kseg;
-            tma_load_2d(sa, &maps.m[seg], fb, kk * BK, m0);
+            tma_load_2d_2sm(sa, &maps.m[seg], fb, kk * BK, m0);
             const int brow = (dense ? 0 : t.slot * p.F) + kk * BK;
 #pragma unroll
-            for (int j = 0; j < BN / 64; ++j) tma_load_2d(sb + j * 8192, &maps.m[2 + seg], fb, t.n_tile * BN + 64 * j, brow);
+            for (int j = 0; j < BN / 128; ++j)
+              tma_load_2d_2sm(sb + j * 8192, &maps.m[2 + seg], fb, t.n_tile * BN + rank * nh + 64 * j, brow);
           } else {  // WGRAD
             const int r = t.k_row0 + kb * BK;
 #pragma unroll
-            for (int i = 0; i < BM / 64; ++i) tma_load_2d(sa + i * 8192, &maps.m[0], fb, t.group * p.a_gcol + m0 + 64 * i, r);
+            for (int i = 0; i < BM / 64; ++i) tma_load_2d_2sm(sa + i * 8192, &maps.m[0], fb, t.group * p.a_gcol + m0 + 64 * i, r);
 #pragma unroll
-            for (int j = 0; j < BN / 64; ++j)
-              tma_load_2d(sb + j * 8192, &maps.m[1], fb, t.group * p.b_gcol + t.n_tile * BN + 64 * j, r);
+            for (int j = 0; j < BN / 128; ++j)
+              tma_load_2d_2sm(sb + j * 8192, &maps.m[1], fb, t.group * p.b_gcol + t.n_tile * BN + rank * nh + 64 * j, r);
           }
           if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
       }
     }
   } else if (warp == 1) {
-    // ===================== MMA issuer =====================
-    constexpr uint32_t idesc = make_idesc(kAMn ? 1 : 0, kBMn ? 1 : 0);
-    int stage = 0, as = 0;
-    uint32_t phase = 0, aphase = 0;
-    for (long id = blockIdx.x; id < sched.total; id += gridDim.x) {
-      const Tile t = sched.decode(id);
-      if (t.num_kb == 0) continue;  // empty WGRAD group: the epilogue writes zeros without touching TMEM
-      mbar_wait(smem_u32(&tempty_bar[as]), aphase ^ 1);
-      tc_fence_after();
-      const uint32_t tmem_d = tmem_base + as * BN;
-      for (int kb = 0; kb < t.num_kb; ++kb) {
-        mbar_wait(smem_u32(&full_bar[stage]), phase);
+    // ===================== MMA issuer (leader CTA) =====================
+    if (rank == 0) {
+      int stage = 0, as = 0;
+      uint32_t phase = 0, aphase = 0;
+      for (long id = cluster_id; id < sched.total; id += n_clusters) {
+        const Tile t = sched.decode(id);
+        if (t.num_kb == 0) continue;  // empty WGRAD group: the epilogue writes zeros without touching TMEM
+        const uint32_t idesc = make_idesc(kAMn ? 1 : 0, kBMn ? 1 : 0, t.n_mma);
+        mbar_wait(smem_u32(&tempty_bar[as]), aphase ^ 1);
         tc_fence_after();
-        if (lane == 0) {
-          const uint32_t sa = smem_u32(smem + stage * kStageBytes), sb = sa + kABytes;
+        const uint32_t tmem_d = tmem_base + as * BN;
+        for (int kb = 0; kb < t.num_kb; ++kb) {
+          mbar_wait(smem_u32(&full_bar[stage]), phase);
+          tc_fence_after();
+          if (lane == 0) {
+            const uint32_t sa = smem_u32(smem + stage * kStageBytes), sb = sa + kABytes;
 #pragma unroll
-          for (int k = 0; k < BK / 16; ++k) {
-            // K-major: 16 K-elements = 32 bytes inside the 128-byte swizzle row, row groups 1024 B apart.
-            // MN-major: 16 K-rows = two 8-row swizzle atoms (2 x 1024 B); 64-element MN chunks 8192 B apart.
-            const uint64_t adesc = kAMn ? make_desc(sa + k * 2048, 8192, 1024) : make_desc(sa + k * 32, 16, 1024);
-            const uint64_t bdesc = kBMn ? make_desc(sb + k * 2048, 8192, 1024) : make_desc(sb + k * 32, 16, 1024);
-            umma_bf16(tmem_d, adesc, bdesc, idesc, (kb | k) != 0 ? 1u : 0u);
+            for (int k = 0; k < BK / 16; ++k) {
+              // K-major: 16 K-elements = 32 bytes inside the 128-byte swizzle row, row groups 1024 B apart.
+              // MN-major: 16 K-rows = two 8-row swizzle atoms (2 x 1024 B); 64-element MN chunks 8192 B apart.
+              const uint64_t adesc = kAMn ? make_desc(sa + k * 2048, 8192, 1024) : make_desc(sa + k * 32, 16, 1024);
+              const uint64_t bdesc = kBMn ? make_desc(sb + k * 2048, 8192, 1024) : make_desc(sb + k * 32, 16, 1024);
+              umma_bf16_2sm(tmem_d, adesc, bdesc, idesc, (kb | k) != 0 ? 1u : 0u);
+            }
+            umma_commit_2sm(smem_u32(&empty_bar[stage]), 3);                       // frees the stage in both CTAs
+            if (kb == t.num_kb - 1) umma_commit_2sm(smem_u32(&tfull_bar[as]), 3);  // accumulator complete, both CTAs
           }
-          umma_commit(smem_u32(&empty_bar[stage]));                       // frees the smem stage when these MMAs retire
-          if (kb == t.num_kb - 1) umma_commit(smem_u32(&tfull_bar[as]));  // accumulator complete
+          __syncwarp();
+          if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
-        __syncwarp();
-        if (++stage == kStages) { stage = 0; phase ^= 1; }
+        if (++as == kAccStages) { as = 0; aphase ^= 1; }
       }
-      if (++as == kAccStages) { as = 0; aphase ^= 1; }
     }
   } else if (warp >= 4) {
-    // ===================== epilogue =====================
+    // ===================== epilogue (each CTA drains its own 128 accumulator rows) =====================
     const int q = warp & 3;             // TMEM lane quarter of this warp
     uint8_t* stg0 = stg_base + q * (kStgTilesPerWarp * kStgTile);
     uint8_t* stg1 = stg0 + kStgTile;
     uint8_t* stg2 = stg1 + kStgTile;
+    const uint32_t tempty_leader = mapa_u32(smem_u32(&tempty_bar[0]), 0);  // + 8 * stage
     if (MODE == DH) {
       // SwiGLU backward needs a and u for every output element.  They are streamed global -> shared with cp.async,
       // kDhDepth 32-column chunks ahead of the consumer and across tile boundaries (the schedule is static), so the
@@ -322,28 +341,30 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
       uint8_t* ring = stg0;                                   // kDhDepth slots of (a tile | u tile)
       uint8_t* out_a = stg0 + 2 * kDhDepth * kStgTile;
       uint8_t* out_u = out_a + kStgTile;
-      long pid = blockIdx.x;                                  // prefetch cursor
+      long pid = cluster_id;                                  // prefetch cursor
       int pcc = 0;
       bool pvalid = pid < sched.total;
       Tile pt = pvalid ? sched.decode(pid) : Tile{};
       auto issue = [&](int slot) {
         if (pvalid) {
-          const int prow0 = pt.m_tile * BM + q * 32;
-          const int prows = dense ? min(32, p.dense_rows - prow0) : 32;
+          const int prow0 = pt.row0 + q * 32;
+          const int prows = !pt.live ? 0 : dense ? min(32, p.dense_rows - prow0) : 32;
           const size_t off = (size_t)prow0 * p.ld + (size_t)pt.part * p.F + pt.n_tile * BN + pcc * 32;
           const uint32_t sa = smem_u32(ring + slot * 2 * kStgTile), su = sa + kStgTile;
+          if (prows > 0) {
 #pragma unroll
-          for (int it = 0; it < 4; ++it) {
-            const int r = it * 8 + (lane >> 2), c = lane & 3;
-            const bool ok = r < prows;
-            const size_t g = off + (size_t)(ok ? r : 0) * p.ld + c * 8;
-            cp_async16(sa + stg_off(r, c), p.in0 + g, ok);
-            cp_async16(su + stg_off(r, c), p.in1 + g, ok);
+            for (int it = 0; it < 4; ++it) {
+              const int r = it * 8 + (lane >> 2), c = lane & 3;
+              const bool ok = r < prows;
+              const size_t g = off + (size_t)(ok ? r : 0) * p.ld + c * 8;
+              cp_async16(sa + stg_off(r, c), p.in0 + g, ok);
+              cp_async16(su + stg_off(r, c), p.in1 + g, ok);
+            }
           }
           ++pcc;
           if (pcc == BN / 32 || pt.n_tile * BN + pcc * 32 >= p.F) {
             pcc = 0;
-            pid += gridDim.x;
+            pid += n_clusters;
             pvalid = pid < sched.total;
             if (pvalid) pt = sched.decode(pid);
           }
@@ -354,11 +375,11 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
       for (int sidx = 0; sidx < kDhDepth; ++sidx) issue(sidx);
       int slot = 0, as = 0;
       uint32_t aphase = 0;
-      for (long id = blockIdx.x; id < sched.total; id += gridDim.x) {
+      for (long id = cluster_id; id < sched.total; id += n_clusters) {
         const Tile t = sched.decode(id);
         const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * BN;
-        const int row0 = t.m_tile * BM + q * 32;
-        const int rows_valid = dense ? min(32, p.dense_rows - row0) : 32;
+        const int row0 = t.row0 + q * 32;
+        const int rows_valid = !t.live ? 0 : dense ? min(32, p.dense_rows - row0) : 32;
         const size_t base = (size_t)row0 * p.ld + (size_t)t.part * p.F;
         mbar_wait(smem_u32(&tfull_bar[as]), aphase);
         tc_fence_after();
@@ -367,51 +388,53 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
           const int n = t.n_tile * BN + cc * 32;
           if (n >= p.F) break;
           float dh[32], a[32], u[32];
-          tmem_ld32(taddr + cc * 32, dh);
+          if (rows_valid > 0) tmem_ld32(taddr + cc * 32, dh);
           cp_async_wait<kDhDepth - 1>();
           __syncwarp();
-          stg_get_row(ring + slot * 2 * kStgTile, lane, a);
-          stg_get_row(ring + slot * 2 * kStgTile + kStgTile, lane, u);
+          if (rows_valid > 0) {
+            stg_get_row(ring + slot * 2 * kStgTile, lane, a);
+            stg_get_row(ring + slot * 2 * kStgTile + kStgTile, lane, u);
+          }
           __syncwarp();
           issue(slot);                                        // refill the slot just drained
-          tmem_ld_wait();
-#pragma unroll
-          for (int i = 0; i < 32; ++i) {
-            const float sg = __fdividef(1.0f, 1.0f + __expf(-a[i]));
-            const float da = dh[i] * u[i] * sg * (1.0f + a[i] * (1.0f - sg));
-            u[i] = dh[i] * a[i] * sg;  // du
-            a[i] = da;
-          }
-          stg_put_row(out_a, lane, a);
-          stg_put_row(out_u, lane, u);
-          __syncwarp();
           if (rows_valid > 0) {
+            tmem_ld_wait();
+#pragma unroll
+            for (int i = 0; i < 32; ++i) {
+              const float sg = __fdividef(1.0f, 1.0f + __expf(-a[i]));
+              const float da = dh[i] * u[i] * sg * (1.0f + a[i] * (1.0f - sg));
+              u[i] = dh[i] * a[i] * sg;  // du
+              a[i] = da;
+            }
+            stg_put_row(out_a, lane, a);
+            stg_put_row(out_u, lane, u);
+            __syncwarp();
             stg_to_global(out_a, p.out0 + base + n, p.ld, lane, rows_valid);
             stg_to_global(out_u, p.out1 + base + n, p.ld, lane, rows_valid);
+            __syncwarp();
           }
-          __syncwarp();
           if (++slot == kDhDepth) slot = 0;
         }
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&tempty_bar[as]));
+        if (lane == 0) mbar_arrive_cluster(tempty_leader + 8 * as);
         if (++as == kAccStages) { as = 0; aphase ^= 1; }
       }
       cp_async_wait<0>();
     } else {
     int as = 0;
     uint32_t aphase = 0;
-    for (long id = blockIdx.x; id < sched.total; id += gridDim.x) {
+    for (long id = cluster_id; id < sched.total; id += n_clusters) {
       const Tile t = sched.decode(id);
       const bool have_acc = t.num_kb > 0;
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * BN;
-      const int row0 = t.m_tile * BM + q * 32;   // first row (or WGRAD output row m) of this warp
+      const int row0 = t.row0 + q * 32;   // first row (or WGRAD output row m) of this warp
+      if (have_acc) { mbar_wait(smem_u32(&tfull_bar[as]), aphase); tc_fence_after(); }
       if (MODE == WGRAD) {
-        if (have_acc) { mbar_wait(smem_u32(&tfull_bar[as]), aphase); tc_fence_after(); }
-        const int rows_valid = min(32, p.M - row0);
+        const int rows_valid = !t.live ? 0 : min(32, p.M - row0);
         bf16* obase = p.out0 + ((size_t)t.group * p.M + row0) * p.N;
 #pragma unroll 1
-        for (int cc = 0; cc < BN / 32; ++cc) {
+        for (int cc = 0; cc < BN / 32 && rows_valid > 0; ++cc) {
           const int n = t.n_tile * BN + cc * 32;
           if (n >= p.N) break;
           float v[32];
@@ -430,17 +453,15 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
           }
           stg_put_row(stg0, lane, v);
           __syncwarp();
-          if (rows_valid > 0) stg_to_global(stg0, obase + n, p.N, lane, rows_valid);
+          stg_to_global(stg0, obase + n, p.N, lane, rows_valid);
           __syncwarp();
         }
       } else {
-        const int rows_valid = dense ? min(32, p.dense_rows - row0) : 32;
+        const int rows_valid = !t.live ? 0 : dense ? min(32, p.dense_rows - row0) : 32;
         if (MODE == FWD1) {
-          mbar_wait(smem_u32(&tfull_bar[as]), aphase);
-          tc_fence_after();
           const size_t base = (size_t)row0 * p.ld + (size_t)t.part * p.F;
 #pragma unroll 1
-          for (int cc = 0; cc < (BN / 2) / 32; ++cc) {
+          for (int cc = 0; cc < (BN / 2) / 32 && rows_valid > 0; ++cc) {
             const int n = t.n_tile * (BN / 2) + cc * 32;
             if (n >= p.F) break;
             float a[32], u[32];
@@ -453,18 +474,14 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
             for (int i = 0; i < 32; ++i) a[i] = __fdividef(a[i], 1.0f + __expf(-a[i])) * u[i];
             stg_put_row(stg2, lane, a);
             __syncwarp();
-            if (rows_valid > 0) {
-              stg_to_global(stg0, p.out0 + base + n, p.ld, lane, rows_valid);
-              stg_to_global(stg1, p.out1 + base + n, p.ld, lane, rows_valid);
-              stg_to_global(stg2, p.out2 + base + n, p.ld, lane, rows_valid);
-            }
+            stg_to_global(stg0, p.out0 + base + n, p.ld, lane, rows_valid);
+            stg_to_global(stg1, p.out1 + base + n, p.ld, lane, rows_valid);
+            stg_to_global(stg2, p.out2 + base + n, p.ld, lane, rows_valid);
             __syncwarp();
           }
         } else {  // FWD2, DX: plain store of a [rows, d] tile
-          mbar_wait(smem_u32(&tfull_bar[as]), aphase);
-          tc_fence_after();
 #pragma unroll 1
-          for (int cc = 0; cc < BN / 32; ++cc) {
+          for (int cc = 0; cc < BN / 32 && rows_valid > 0; ++cc) {
             const int n = t.n_tile * BN + cc * 32;
             if (n >= p.d) break;
             float v[32];
@@ -472,7 +489,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
             tmem_ld_wait();
             stg_put_row(stg0, lane, v);
             __syncwarp();
-            if (rows_valid > 0) stg_to_global(stg0, p.out0 + (size_t)row0 * p.d + n, p.d, lane, rows_valid);
+            stg_to_global(stg0, p.out0 + (size_t)row0 * p.d + n, p.d, lane, rows_valid);
             __syncwarp();
           }
         }
@@ -480,17 +497,18 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
       if (have_acc) {
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&tempty_bar[as]));
+        if (lane == 0) mbar_arrive_cluster(tempty_leader + 8 * as);
         if (++as == kAccStages) { as = 0; aphase ^= 1; }
       }
     }
     }
   }
 
+  // neither CTA may leave (or free tensor memory) while its peer can still read its shared memory or signal its barriers
   tc_fence_before();
-  __syncthreads();
+  cluster_sync_all();
   if (warp == 2) {
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kTmemCols) : "memory");
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kTmemCols) : "memory");
   }
 }
 
@@ -504,7 +522,7 @@ int launch(const TmaMaps& maps, const UmmaParams& p, cudaStream_t st, const char
     FOMOE_CUDA_OK(cudaFuncSetAttribute(umma_grouped_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes_of(MODE)));
     attr_set = true;
   }
-  umma_grouped_kernel<MODE><<<num_sms(), kThreads, smem_bytes_of(MODE), st>>>(maps, p);
+  umma_grouped_kernel<MODE><<<num_sms() & ~1, kThreads, smem_bytes_of(MODE), st>>>(maps, p);
   FOMOE_LAUNCH_OK(name);
   return FOMOE_OK;
 }
@@ -524,7 +542,7 @@ int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs&
   if (n_res > 0 && c.T > 0) {
     const uint64_t R = (uint64_t)rws.R_cap;
     UmmaParams p{};
-    p.n_mtiles = rws.n_mtiles; p.tile_slot = rws.tile_slot; p.parts = 1; p.d = d; p.F = F; p.ld = F;
+    p.n_mtiles = rws.n_mtiles; p.tile_slot = rws.tile_slot; p.pair_info = rws.pair_info; p.parts = 1; p.d = d; p.F = F; p.ld = F;
     {
       TmaMaps m{};
       MAP_OK(make_map(&m.m[0], aws.xp, d, R, d, 128));
@@ -539,7 +557,7 @@ int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs&
     {
       TmaMaps m{};
       MAP_OK(make_map(&m.m[0], aws.h, F, R, F, 128));
-      MAP_OK(make_map(&m.m[1], w.w_down, F, (uint64_t)n_res * d, F, 256));
+      MAP_OK(make_map(&m.m[1], w.w_down, F, (uint64_t)n_res * d, F, 128));
       m.m[2] = m.m[3] = m.m[0];
       UmmaParams q = p;
       q.out0 = (bf16*)aws.o;
@@ -565,7 +583,7 @@ int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs&
     {
       TmaMaps m{};
       MAP_OK(make_map(&m.m[0], aws.sh, ld, c.T, ld, 128));
-      MAP_OK(make_map(&m.m[1], w.sh_down, Fs, (uint64_t)ns * d, Fs, 256));
+      MAP_OK(make_map(&m.m[1], w.sh_down, Fs, (uint64_t)ns * d, Fs, 128));
       m.m[2] = m.m[3] = m.m[0];
       UmmaParams q = p;
       q.out0 = (bf16*)sws.y_sh;
@@ -583,7 +601,7 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
   if (n_res > 0) {
     const uint64_t R = (uint64_t)rws.R_cap;
     UmmaParams p{};
-    p.n_mtiles = rws.n_mtiles; p.tile_slot = rws.tile_slot; p.pad_offsets = rws.pad_offsets; p.parts = 1; p.d = d; p.F = F; p.ld = F;
+    p.n_mtiles = rws.n_mtiles; p.tile_slot = rws.tile_slot; p.pair_info = rws.pair_info; p.pad_offsets = rws.pad_offsets; p.parts = 1; p.d = d; p.F = F; p.ld = F;
     if (c.T > 0) {
       {  // dh = dO W_down, fused SwiGLU backward
         TmaMaps m{};
@@ -701,7 +719,7 @@ int umma_router_bwd(const fomoe_config& c, const void* x, const float* w_router,
     p.dense_rows = T; p.parts = 1; p.d = d; p.F = Ez; p.ld = Ez;
     TmaMaps m{};
     MAP_OK(make_map(&m.m[0], sws.dz_bf, Ez, T, Ez, 128));
-    MAP_OK(make_map(&m.m[1], sws.wr_bf, Ez, d, Ez, 256));
+    MAP_OK(make_map(&m.m[1], sws.wr_bf, Ez, d, Ez, 128));
     m.m[2] = m.m[3] = m.m[0];
     p.out0 = (bf16*)sws.dx_r;
     int rc = launch<FWD2>(m, p, st, "umma_grouped_kernel<FWD2,router dx>");
