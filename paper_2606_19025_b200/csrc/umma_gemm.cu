@@ -34,16 +34,17 @@ constexpr int BM = 128;   // rows per CTA (256 per pair)
 constexpr int BN = 256;   // accumulator columns (each CTA stages BN/2 columns of B)
 constexpr int BK = 64, kAccStages = 2;
 constexpr int kABytes = BM * BK * 2, kBBytes = (BN / 2) * BK * 2, kStageBytes = kABytes + kBBytes;
-constexpr int kThreads = 256;
-// epilogue staging: per epilogue warp, up to 3 swizzled tiles of 32 rows x 32 bf16 (2 KB each) used to turn the
+constexpr int kThreads = 384;   // warps 0-3: TMA, MMA, TMEM allocator, idle; warps 4-11: epilogue
+constexpr int kEpiWarps = 8;    // two warps per TMEM lane quarter; they take alternate 32-column chunks of a tile
+// epilogue staging: per epilogue warp, swizzled tiles of 32 rows x 32 bf16 (2 KB each) used to turn the
 // row-per-thread TMEM layout into coalesced 16-byte global accesses
 constexpr int kStgTile = 2048;
-constexpr int kDhDepth = 4;  // DH epilogue: chunks of (a, u) kept in flight per warp with cp.async
+constexpr int kDhDepth = 3;  // DH epilogue: chunks of (a, u) kept in flight per warp with cp.async
 enum Mode { FWD1 = 0, FWD2 = 1, DH = 2, DX = 3, WGRAD = 4 };
-// DH trades TMA stages for a deep epilogue prefetch ring: its epilogue must stream a and u back in
-__host__ __device__ constexpr int stages_of(int mode) { return mode == DH ? 4 : 6; }
-__host__ __device__ constexpr int stg_tiles_per_warp(int mode) { return mode == DH ? 2 * kDhDepth + 2 : 3; }
-__host__ __device__ constexpr int stg_bytes_of(int mode) { return 4 * stg_tiles_per_warp(mode) * kStgTile; }
+// DH and FWD1 trade TMA stages for epilogue staging: DH streams a and u back in through a cp.async ring
+__host__ __device__ constexpr int stages_of(int mode) { return mode == DH ? 4 : mode == FWD1 ? 5 : 6; }
+__host__ __device__ constexpr int stg_tiles_per_warp(int mode) { return mode == DH ? 2 * kDhDepth : mode == FWD1 ? 3 : 1; }
+__host__ __device__ constexpr int stg_bytes_of(int mode) { return kEpiWarps * stg_tiles_per_warp(mode) * kStgTile; }
 __host__ __device__ constexpr int smem_bytes_of(int mode) {
   return stages_of(mode) * kStageBytes + stg_bytes_of(mode) + 1024 /*align*/ + 256 /*barriers*/;
 }
@@ -78,41 +79,46 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 // ---- per-warp staging tile: 32 rows x 64 B, two rows per 128-byte line, 16-byte chunks XOR-swizzled so that both the
-// row-per-lane accesses and the 8-rows-x-4-chunks global-side accesses are bank-conflict free ----
+// row-per-lane accesses and the 8-rows-x-4-chunks global-side accesses are bank-conflict free.  Addresses are
+// shared-state-space (ld.shared / st.shared), not generic ----
 __device__ __forceinline__ uint32_t stg_off(int r, int q) { return (uint32_t)((r >> 1) * 128 + (((((r & 1) << 2) | q) ^ ((r >> 1) & 7)) * 16)); }
+__device__ __forceinline__ void sts128(uint32_t addr, const uint4& v) {
+  asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
+  __nv_bfloat162 h = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&h);
+}
+__device__ __forceinline__ float2 unpack_bf16x2(uint32_t w) {
+  return __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&w));
+}
 
 // lane = row: write 32 fp32 as bf16 into the staging tile
-__device__ __forceinline__ void stg_put_row(uint8_t* stg, int lane, const float (&v)[32]) {
+__device__ __forceinline__ void stg_put_row(uint32_t stg, int lane, const float (&v)[32]) {
 #pragma unroll
   for (int q = 0; q < 4; ++q) {
     uint4 w;
-    __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&w);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) h[i] = __floats2bfloat162_rn(v[q * 8 + 2 * i], v[q * 8 + 2 * i + 1]);
-    *reinterpret_cast<uint4*>(stg + stg_off(lane, q)) = w;
-  }
-}
-// lane = row: read 32 bf16 from the staging tile as fp32
-__device__ __forceinline__ void stg_get_row(const uint8_t* stg, int lane, float (&v)[32]) {
-#pragma unroll
-  for (int q = 0; q < 4; ++q) {
-    uint4 w = *reinterpret_cast<const uint4*>(stg + stg_off(lane, q));
-    const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&w);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      float2 f = __bfloat1622float2(h[i]);
-      v[q * 8 + 2 * i] = f.x;
-      v[q * 8 + 2 * i + 1] = f.y;
-    }
+    w.x = pack_bf16x2(v[q * 8 + 0], v[q * 8 + 1]);
+    w.y = pack_bf16x2(v[q * 8 + 2], v[q * 8 + 3]);
+    w.z = pack_bf16x2(v[q * 8 + 4], v[q * 8 + 5]);
+    w.w = pack_bf16x2(v[q * 8 + 6], v[q * 8 + 7]);
+    sts128(stg + stg_off(lane, q), w);
   }
 }
 // whole warp: staging tile -> global rows [0, rows_valid) x 32 columns at g (row stride ld elements); 4 lanes per row
-__device__ __forceinline__ void stg_to_global(const uint8_t* stg, bf16* g, size_t ld, int lane, int rows_valid) {
+__device__ __forceinline__ void stg_to_global(uint32_t stg, bf16* g, size_t ld, int lane, int rows_valid) {
+  uint4 w[4];
+#pragma unroll
+  for (int it = 0; it < 4; ++it) w[it] = lds128(stg + stg_off(it * 8 + (lane >> 2), lane & 3));
 #pragma unroll
   for (int it = 0; it < 4; ++it) {
     const int r = it * 8 + (lane >> 2), c = lane & 3;
-    const uint4 w = *reinterpret_cast<const uint4*>(stg + stg_off(r, c));
-    if (r < rows_valid) *reinterpret_cast<uint4*>(g + (size_t)r * ld + c * 8) = w;
+    if (r < rows_valid) *reinterpret_cast<uint4*>(g + (size_t)r * ld + c * 8) = w[it];
   }
 }
 
@@ -218,7 +224,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
   uint64_t* full_bar = bars;                          // [kStages]   used in the leader CTA only
   uint64_t* empty_bar = bars + kStages;               // [kStages]   one per CTA, released by the leader's commits
   uint64_t* tfull_bar = bars + 2 * kStages;           // [kAccStages] one per CTA
-  uint64_t* tempty_bar = bars + 2 * kStages + kAccStages;  // [kAccStages] leader only: 4 epilogue warps x 2 CTAs
+  uint64_t* tempty_bar = bars + 2 * kStages + kAccStages;  // [kAccStages] leader only: 8 epilogue warps x 2 CTAs
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * kStages + 2 * kAccStages);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -232,7 +238,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
   }
   if (warp == 1 && lane == 0) {
     for (int i = 0; i < kStages; ++i) { mbar_init(smem_u32(&full_bar[i]), 1); mbar_init(smem_u32(&empty_bar[i]), 1); }
-    for (int i = 0; i < kAccStages; ++i) { mbar_init(smem_u32(&tfull_bar[i]), 1); mbar_init(smem_u32(&tempty_bar[i]), 8); }
+    for (int i = 0; i < kAccStages; ++i) { mbar_init(smem_u32(&tfull_bar[i]), 1); mbar_init(smem_u32(&tempty_bar[i]), 2 * kEpiWarps); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 2) {
@@ -295,31 +301,38 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
     }
   } else if (warp == 1) {
     // ===================== MMA issuer (leader CTA) =====================
+    // The whole warp walks the (warp-uniform) schedule and waits on the barriers; one elected lane issues.  What bounds
+    // this loop is the issuing thread's own instruction latency per MMA, so the per-stage descriptor words are
+    // precomputed (lane s holds stage s, fetched with one shuffle) and a K step is one 32-bit add.
     if (rank == 0) {
       int stage = 0, as = 0;
       uint32_t phase = 0, aphase = 0;
+      // K-major: 16 K-elements = 32 bytes inside the 128-byte swizzle row, row groups 1024 B apart.
+      // MN-major: 16 K-rows = two 8-row swizzle atoms (2 x 1024 B); 64-element MN chunks 8192 B apart.
+      const uint32_t sa0 = smem_u32(smem) + (uint32_t)(lane < kStages ? lane : 0) * kStageBytes, sb0 = sa0 + kABytes;
+      const uint64_t adesc_l = kAMn ? make_desc(sa0, 8192, 1024) : make_desc(sa0, 16, 1024);
+      const uint64_t bdesc_l = kBMn ? make_desc(sb0, 8192, 1024) : make_desc(sb0, 16, 1024);
+      const uint32_t a_hi = (uint32_t)(adesc_l >> 32), b_hi = (uint32_t)(bdesc_l >> 32);
+      const uint32_t my_alo = (uint32_t)adesc_l, my_blo = (uint32_t)bdesc_l;
+      constexpr uint32_t kAStep = (kAMn ? 2048 : 32) >> 4, kBStep = (kBMn ? 2048 : 32) >> 4;
       for (long id = cluster_id; id < sched.total; id += n_clusters) {
         const Tile t = sched.decode(id);
         if (t.num_kb == 0) continue;  // empty WGRAD group: the epilogue writes zeros without touching TMEM
         const uint32_t idesc = make_idesc(kAMn ? 1 : 0, kBMn ? 1 : 0, t.n_mma);
         mbar_wait(smem_u32(&tempty_bar[as]), aphase ^ 1);
-        tc_fence_after();
         const uint32_t tmem_d = tmem_base + as * BN;
-        for (int kb = 0; kb < t.num_kb; ++kb) {
+        const int num_kb = t.num_kb;
+        for (int kb = 0; kb < num_kb; ++kb) {
           mbar_wait(smem_u32(&full_bar[stage]), phase);
           tc_fence_after();
-          if (lane == 0) {
-            const uint32_t sa = smem_u32(smem + stage * kStageBytes), sb = sa + kABytes;
-#pragma unroll
-            for (int k = 0; k < BK / 16; ++k) {
-              // K-major: 16 K-elements = 32 bytes inside the 128-byte swizzle row, row groups 1024 B apart.
-              // MN-major: 16 K-rows = two 8-row swizzle atoms (2 x 1024 B); 64-element MN chunks 8192 B apart.
-              const uint64_t adesc = kAMn ? make_desc(sa + k * 2048, 8192, 1024) : make_desc(sa + k * 32, 16, 1024);
-              const uint64_t bdesc = kBMn ? make_desc(sb + k * 2048, 8192, 1024) : make_desc(sb + k * 32, 16, 1024);
-              umma_bf16_2sm(tmem_d, adesc, bdesc, idesc, (kb | k) != 0 ? 1u : 0u);
-            }
-            umma_commit_2sm(smem_u32(&empty_bar[stage]), 3);                       // frees the stage in both CTAs
-            if (kb == t.num_kb - 1) umma_commit_2sm(smem_u32(&tfull_bar[as]), 3);  // accumulator complete, both CTAs
+          const uint32_t alo = __shfl_sync(0xffffffffu, my_alo, stage), blo = __shfl_sync(0xffffffffu, my_blo, stage);
+          if (elect_one_sync()) {
+            umma_bf16_2sm_lohi(tmem_d, alo, a_hi, blo, b_hi, idesc, kb != 0 ? 1u : 0u);
+            umma_bf16_2sm_lohi(tmem_d, alo + kAStep, a_hi, blo + kBStep, b_hi, idesc, 1u);
+            umma_bf16_2sm_lohi(tmem_d, alo + 2 * kAStep, a_hi, blo + 2 * kBStep, b_hi, idesc, 1u);
+            umma_bf16_2sm_lohi(tmem_d, alo + 3 * kAStep, a_hi, blo + 3 * kBStep, b_hi, idesc, 1u);
+            umma_commit_2sm(smem_u32(&empty_bar[stage]), 3);                    // frees the stage in both CTAs
+            if (kb == num_kb - 1) umma_commit_2sm(smem_u32(&tfull_bar[as]), 3);  // accumulator complete, both CTAs
           }
           __syncwarp();
           if (++stage == kStages) { stage = 0; phase ^= 1; }
@@ -329,28 +342,31 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
     }
   } else if (warp >= 4) {
     // ===================== epilogue (each CTA drains its own 128 accumulator rows) =====================
-    const int q = warp & 3;             // TMEM lane quarter of this warp
-    uint8_t* stg0 = stg_base + q * (kStgTilesPerWarp * kStgTile);
-    uint8_t* stg1 = stg0 + kStgTile;
-    uint8_t* stg2 = stg1 + kStgTile;
+    const int q = warp & 3;               // TMEM lane quarter of this warp
+    const int half = (warp >> 2) - 1;     // which of the two warps of the quarter: takes chunks half, half + 2, ...
+    const uint32_t stg0 = smem_u32(stg_base) + (uint32_t)((warp - 4) * (kStgTilesPerWarp * kStgTile));
     const uint32_t tempty_leader = mapa_u32(smem_u32(&tempty_bar[0]), 0);  // + 8 * stage
     if (MODE == DH) {
       // SwiGLU backward needs a and u for every output element.  They are streamed global -> shared with cp.async,
       // kDhDepth 32-column chunks ahead of the consumer and across tile boundaries (the schedule is static), so the
-      // loads never sit on the critical path of the accumulator drain.
-      uint8_t* ring = stg0;                                   // kDhDepth slots of (a tile | u tile)
-      uint8_t* out_a = stg0 + 2 * kDhDepth * kStgTile;
-      uint8_t* out_u = out_a + kStgTile;
-      long pid = cluster_id;                                  // prefetch cursor
-      int pcc = 0;
+      // loads never sit on the critical path of the accumulator drain.  A ring slot (a tile | u tile) is overwritten in
+      // place with (da | du) and stored from there.
+      long pid = cluster_id;                                  // prefetch cursor: (tile, chunk) in consumption order
+      int pcc = half;
       bool pvalid = pid < sched.total;
       Tile pt = pvalid ? sched.decode(pid) : Tile{};
       auto issue = [&](int slot) {
+        while (pvalid && pt.n_tile * BN + pcc * 32 >= p.F) {  // this warp has no (more) chunk in the tile
+          pcc = half;
+          pid += n_clusters;
+          pvalid = pid < sched.total;
+          if (pvalid) pt = sched.decode(pid);
+        }
         if (pvalid) {
           const int prow0 = pt.row0 + q * 32;
           const int prows = !pt.live ? 0 : dense ? min(32, p.dense_rows - prow0) : 32;
           const size_t off = (size_t)prow0 * p.ld + (size_t)pt.part * p.F + pt.n_tile * BN + pcc * 32;
-          const uint32_t sa = smem_u32(ring + slot * 2 * kStgTile), su = sa + kStgTile;
+          const uint32_t sa = stg0 + slot * 2 * kStgTile, su = sa + kStgTile;
           if (prows > 0) {
 #pragma unroll
             for (int it = 0; it < 4; ++it) {
@@ -361,9 +377,9 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
               cp_async16(su + stg_off(r, c), p.in1 + g, ok);
             }
           }
-          ++pcc;
-          if (pcc == BN / 32 || pt.n_tile * BN + pcc * 32 >= p.F) {
-            pcc = 0;
+          pcc += 2;
+          if (pcc >= BN / 32) {
+            pcc = half;
             pid += n_clusters;
             pvalid = pid < sched.total;
             if (pvalid) pt = sched.decode(pid);
@@ -384,35 +400,39 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
         mbar_wait(smem_u32(&tfull_bar[as]), aphase);
         tc_fence_after();
 #pragma unroll 1
-        for (int cc = 0; cc < BN / 32; ++cc) {
+        for (int cc = half; cc < BN / 32; cc += 2) {
           const int n = t.n_tile * BN + cc * 32;
           if (n >= p.F) break;
-          float dh[32], a[32], u[32];
+          const uint32_t sa = stg0 + slot * 2 * kStgTile, su = sa + kStgTile;
+          float dh[32];
           if (rows_valid > 0) tmem_ld32(taddr + cc * 32, dh);
           cp_async_wait<kDhDepth - 1>();
           __syncwarp();
           if (rows_valid > 0) {
-            stg_get_row(ring + slot * 2 * kStgTile, lane, a);
-            stg_get_row(ring + slot * 2 * kStgTile + kStgTile, lane, u);
-          }
-          __syncwarp();
-          issue(slot);                                        // refill the slot just drained
-          if (rows_valid > 0) {
             tmem_ld_wait();
 #pragma unroll
-            for (int i = 0; i < 32; ++i) {
-              const float sg = __fdividef(1.0f, 1.0f + __expf(-a[i]));
-              const float da = dh[i] * u[i] * sg * (1.0f + a[i] * (1.0f - sg));
-              u[i] = dh[i] * a[i] * sg;  // du
-              a[i] = da;
+            for (int g8 = 0; g8 < 4; ++g8) {
+              const uint32_t o = stg_off(lane, g8);
+              uint4 wa = lds128(sa + o), wu = lds128(su + o);
+              uint32_t* pa = reinterpret_cast<uint32_t*>(&wa);
+              uint32_t* pu = reinterpret_cast<uint32_t*>(&wu);
+#pragma unroll
+              for (int i = 0; i < 4; ++i) {
+                const float2 a2 = unpack_bf16x2(pa[i]), u2 = unpack_bf16x2(pu[i]);
+                const float d0 = dh[g8 * 8 + 2 * i], d1 = dh[g8 * 8 + 2 * i + 1];
+                const float s0 = __fdividef(1.0f, 1.0f + __expf(-a2.x)), s1 = __fdividef(1.0f, 1.0f + __expf(-a2.y));
+                pa[i] = pack_bf16x2(d0 * u2.x * s0 * (1.0f + a2.x * (1.0f - s0)), d1 * u2.y * s1 * (1.0f + a2.y * (1.0f - s1)));
+                pu[i] = pack_bf16x2(d0 * a2.x * s0, d1 * a2.y * s1);
+              }
+              sts128(sa + o, wa);   // da over a, du over u: every lane rewrites exactly the bytes it read
+              sts128(su + o, wu);
             }
-            stg_put_row(out_a, lane, a);
-            stg_put_row(out_u, lane, u);
             __syncwarp();
-            stg_to_global(out_a, p.out0 + base + n, p.ld, lane, rows_valid);
-            stg_to_global(out_u, p.out1 + base + n, p.ld, lane, rows_valid);
-            __syncwarp();
+            stg_to_global(sa, p.out0 + base + n, p.ld, lane, rows_valid);
+            stg_to_global(su, p.out1 + base + n, p.ld, lane, rows_valid);
           }
+          __syncwarp();
+          issue(slot);                                        // refill the slot just stored from
           if (++slot == kDhDepth) slot = 0;
         }
         tc_fence_before();
@@ -422,6 +442,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
       }
       cp_async_wait<0>();
     } else {
+    const uint32_t stg1 = stg0 + kStgTile, stg2 = stg1 + kStgTile;  // FWD1 only
     int as = 0;
     uint32_t aphase = 0;
     for (long id = cluster_id; id < sched.total; id += n_clusters) {
@@ -434,7 +455,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
         const int rows_valid = !t.live ? 0 : min(32, p.M - row0);
         bf16* obase = p.out0 + ((size_t)t.group * p.M + row0) * p.N;
 #pragma unroll 1
-        for (int cc = 0; cc < BN / 32 && rows_valid > 0; ++cc) {
+        for (int cc = half; cc < BN / 32 && rows_valid > 0; cc += 2) {
           const int n = t.n_tile * BN + cc * 32;
           if (n >= p.N) break;
           float v[32];
@@ -461,7 +482,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
         if (MODE == FWD1) {
           const size_t base = (size_t)row0 * p.ld + (size_t)t.part * p.F;
 #pragma unroll 1
-          for (int cc = 0; cc < (BN / 2) / 32 && rows_valid > 0; ++cc) {
+          for (int cc = half; cc < (BN / 2) / 32 && rows_valid > 0; cc += 2) {
             const int n = t.n_tile * (BN / 2) + cc * 32;
             if (n >= p.F) break;
             float a[32], u[32];
@@ -481,7 +502,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
           }
         } else {  // FWD2, DX: plain store of a [rows, d] tile
 #pragma unroll 1
-          for (int cc = 0; cc < BN / 32 && rows_valid > 0; ++cc) {
+          for (int cc = half; cc < BN / 32 && rows_valid > 0; cc += 2) {
             const int n = t.n_tile * BN + cc * 32;
             if (n >= p.d) break;
             float v[32];

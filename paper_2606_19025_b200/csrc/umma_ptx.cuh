@@ -67,6 +67,13 @@ __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.
 
 // ---- CTA-pair (cta_group::2) variants: two CTAs of a cluster on one TPC issue ONE MMA over M = 256 rows; each CTA stages
 // its own 128 rows of A and half of the N columns of B, which halves shared-memory and L2 operand traffic per flop ----
+// true in exactly one (the lowest active) lane of a converged warp; lets ptxas issue the single-thread tcgen05 / TMA
+// instructions without a per-lane broadcast loop
+__device__ __forceinline__ bool elect_one_sync() {
+  uint32_t pred;
+  asm volatile("{\n.reg .pred p;\nelect.sync _|p, 0xffffffff;\nselp.u32 %0, 1, 0, p;\n}" : "=r"(pred));
+  return pred != 0;
+}
 __device__ __forceinline__ uint32_t cluster_ctarank() {
   uint32_t r;
   asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
@@ -92,6 +99,13 @@ __device__ __forceinline__ void tma_load_2d_2sm(uint32_t dst, const CUtensorMap*
 __device__ __forceinline__ void umma_bf16_2sm(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
   asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n}"
                ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// same, descriptors passed as (lo, hi) 32-bit halves so that a K step is one 32-bit add
+__device__ __forceinline__ void umma_bf16_2sm_lohi(uint32_t tmem_d, uint32_t alo, uint32_t ahi, uint32_t blo, uint32_t bhi, uint32_t idesc,
+                                                   uint32_t accumulate) {
+  asm volatile("{\n.reg .pred p;\n.reg .b64 da, db;\nsetp.ne.b32 p, %6, 0;\nmov.b64 da, {%1, %2};\nmov.b64 db, {%3, %4};\n"
+               "tcgen05.mma.cta_group::2.kind::f16 [%0], da, db, %5, p;\n}"
+               ::"r"(tmem_d), "r"(alo), "r"(ahi), "r"(blo), "r"(bhi), "r"(idesc), "r"(accumulate) : "memory");
 }
 // arrives (once all prior MMAs of this thread retire) on the barrier at the same offset in every CTA of `mask`
 __device__ __forceinline__ void umma_commit_2sm(uint32_t bar, uint16_t mask) {
