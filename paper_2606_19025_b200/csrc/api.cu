@@ -1,5 +1,6 @@
 // extern "C" entry points of libfomoe (include/fomoe.h): argument checks, workspace carving, kernel sequencing.
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <vector>
@@ -52,6 +53,11 @@ static int check_cfg(const fomoe_config* c, int n_res) {
 }
 
 bool force_simt() { return g_force_simt != 0; }
+// FOMOE_PDL=0 in the environment turns programmatic dependent launch off (A/B measurements, debugging)
+bool pdl_enabled() {
+  static const bool on = [] { const char* e = getenv("FOMOE_PDL"); return !(e && e[0] == '0'); }();
+  return on;
+}
 static bool use_umma(const fomoe_config& c) { return !g_force_simt && umma_supported(c); }
 
 }  // namespace fomoe

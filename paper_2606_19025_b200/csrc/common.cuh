@@ -29,6 +29,30 @@ int set_cuda_error(cudaError_t e, const char* where);
     if (e__ != cudaSuccess) return fomoe::set_cuda_error(e__, name);  \
   } while (0)
 
+// ---- programmatic dependent launch (PDL) ----
+// Every kernel of the bf16 path is launched with cudaLaunchAttributeProgrammaticStreamSerialization: its CTAs may become
+// resident (and run their prologue: barrier init, TMEM allocation, descriptor prefetch) while the previous kernel on the
+// stream is still draining.  The contract that keeps this safe: such a kernel calls pdl_launch_dependents() at its top
+// and pdl_wait() BEFORE its first access to global memory; pdl_wait() returns once every earlier grid has completed and
+// its writes are visible (so dependencies are transitive along the stream).
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+bool pdl_enabled();
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = pdl_enabled() ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 inline __host__ __device__ int ceil_div(int a, int b) { return (a + b - 1) / b; }
 inline __host__ __device__ size_t align_up(size_t a, size_t b) { return (a + b - 1) / b * b; }
 

@@ -169,20 +169,31 @@ __global__ void perm_hist_kernel(const int32_t* __restrict__ topk_idx, const int
 }
 
 // One block.  Per slot: exclusive scan of the per-block counts (in place) -> counts; then offsets, tile-padded
-// offsets, the row-tile -> slot map and the number of tiles in use.
+// offsets, the row-tile -> slot map and the number of tiles in use.  One warp per slot, 32 blocks per shuffle scan.
 __global__ void perm_scan_kernel(int32_t* __restrict__ blk_hist, int n_blk, int n_res, int32_t* __restrict__ counts,
                                  int32_t* __restrict__ offsets, int32_t* __restrict__ pad_offsets,
                                  int32_t* __restrict__ n_mtiles, int32_t* __restrict__ tile_slot, int32_t* __restrict__ pair_info) {
   __shared__ int32_t s_pad[kMaxE + 1];
   __shared__ int32_t s_pair[kMaxE + 1];  // first tile pair of slot s (a pair = two row tiles of ONE slot, the last may be single)
-  for (int s = threadIdx.x; s < n_res; s += blockDim.x) {
+  __shared__ int32_t s_cnt[kMaxE];
+  pdl_launch_dependents();
+  pdl_wait();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, n_warps = blockDim.x >> 5;
+  for (int s = warp; s < n_res; s += n_warps) {
     int run = 0;
-    for (int b = 0; b < n_blk; ++b) {
-      int c = blk_hist[(size_t)b * n_res + s];
-      blk_hist[(size_t)b * n_res + s] = run;
-      run += c;
+    for (int b0 = 0; b0 < n_blk; b0 += 32) {
+      const int b = b0 + lane;
+      const int c = b < n_blk ? blk_hist[(size_t)b * n_res + s] : 0;
+      int inc = c;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += v;
+      }
+      if (b < n_blk) blk_hist[(size_t)b * n_res + s] = run + inc - c;
+      run += __shfl_sync(0xffffffffu, inc, 31);
     }
-    counts[s] = run;
+    if (lane == 0) { counts[s] = run; s_cnt[s] = run; }
   }
   __syncthreads();
   if (threadIdx.x == 0) {
@@ -192,8 +203,8 @@ __global__ void perm_scan_kernel(int32_t* __restrict__ blk_hist, int n_blk, int 
       pad_offsets[s] = pad;
       s_pad[s] = pad;
       s_pair[s] = pairs;
-      off += counts[s];
-      const int tiles = (counts[s] + kTileM - 1) / kTileM;
+      off += s_cnt[s];
+      const int tiles = (s_cnt[s] + kTileM - 1) / kTileM;
       pad += tiles * kTileM;
       pairs += (tiles + 1) / 2;
     }
@@ -222,6 +233,8 @@ perm_scatter_kernel(const int32_t* __restrict__ topk_idx, const float* __restric
                     int32_t* __restrict__ row_token, int32_t* __restrict__ pair_row, int32_t* __restrict__ prow_token,
                     float* __restrict__ prow_gate, int32_t* __restrict__ prow_pair, int32_t* __restrict__ pair_prow) {
   extern __shared__ int32_t sm[];
+  pdl_launch_dependents();
+  pdl_wait();
   int32_t* running = sm;                 // [n_res] kept pairs of this block seen so far, per slot
   int32_t* warp_cnt = sm + n_res;        // [8][n_res]
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -297,8 +310,11 @@ int launch_route(const fomoe_config& c, const void* x, const float* w_router, co
   const long n_pairs = (long)c.T * c.top_k;
   const int pairs_per_blk = kPermTokens * c.top_k;
   const int nr = n_res > 0 ? n_res : 1;
-  FOMOE_CUDA_OK(cudaMemsetAsync(out.row_token, 0xFF, sizeof(int32_t) * (size_t)n_pairs, st));
-  FOMOE_CUDA_OK(cudaMemsetAsync(ws.prow_token, 0xFF, sizeof(int32_t) * (size_t)ws.R_cap, st));
+  const bool tc = c.T > 0 && !force_simt() && route_umma_supported(c);
+  if (!tc) {  // (the tensor-core path fills these in its preparation kernel)
+    FOMOE_CUDA_OK(cudaMemsetAsync(out.row_token, 0xFF, sizeof(int32_t) * (size_t)n_pairs, st));
+    FOMOE_CUDA_OK(cudaMemsetAsync(ws.prow_token, 0xFF, sizeof(int32_t) * (size_t)ws.R_cap, st));
+  }
   if (c.T == 0) {  // empty batch: all counts and offsets are zero, no tile in use
     if (n_res > 0) FOMOE_CUDA_OK(cudaMemsetAsync(out.counts, 0, sizeof(int32_t) * (size_t)n_res, st));
     FOMOE_CUDA_OK(cudaMemsetAsync(out.offsets, 0, sizeof(int32_t) * (size_t)(n_res + 1), st));
@@ -306,7 +322,7 @@ int launch_route(const fomoe_config& c, const void* x, const float* w_router, co
     FOMOE_CUDA_OK(cudaMemsetAsync(ws.n_mtiles, 0, sizeof(int32_t) * 4, st));
     return FOMOE_OK;
   }
-  if (!force_simt() && route_umma_supported(c)) {
+  if (tc) {
     // tensor-core router: logits + gate + top-k + mask + per-block histogram in one kernel
     int rc = launch_route_umma(c, x, w_router, bias, resident_ids, n_res, out, ws, st);
     if (rc != FOMOE_OK) return rc;
@@ -319,12 +335,12 @@ int launch_route(const fomoe_config& c, const void* x, const float* w_router, co
     perm_hist_kernel<<<ws.n_blk, 256, sizeof(int32_t) * nr, st>>>(out.topk_idx, ws.slot_of, n_pairs, pairs_per_blk, n_res, ws.blk_hist);
     FOMOE_LAUNCH_OK("perm_hist_kernel");
   }
-  perm_scan_kernel<<<1, 256, 0, st>>>(ws.blk_hist, ws.n_blk, n_res, out.counts, out.offsets, ws.pad_offsets, ws.n_mtiles,
-                                      ws.tile_slot, ws.pair_info);
+  FOMOE_CUDA_OK(launch_pdl(perm_scan_kernel, 1, 1024, 0, st, ws.blk_hist, ws.n_blk, n_res, out.counts, out.offsets, ws.pad_offsets,
+                           ws.n_mtiles, ws.tile_slot, ws.pair_info));
   FOMOE_LAUNCH_OK("perm_scan_kernel");
-  perm_scatter_kernel<<<ws.n_blk, kPermThreads, sizeof(int32_t) * 9 * nr, st>>>(
-      out.topk_idx, out.gate, ws.slot_of, ws.blk_hist, out.offsets, ws.pad_offsets, n_pairs, pairs_per_blk, c.top_k, n_res,
-      out.row_token, out.pair_row, ws.prow_token, ws.prow_gate, ws.prow_pair, ws.pair_prow);
+  FOMOE_CUDA_OK(launch_pdl(perm_scatter_kernel, ws.n_blk, kPermThreads, sizeof(int32_t) * 9 * nr, st, out.topk_idx, out.gate, ws.slot_of,
+                           ws.blk_hist, out.offsets, ws.pad_offsets, n_pairs, pairs_per_blk, c.top_k, n_res, out.row_token, out.pair_row,
+                           ws.prow_token, ws.prow_gate, ws.prow_pair, ws.pair_prow));
   FOMOE_LAUNCH_OK("perm_scatter_kernel");
   return FOMOE_OK;
 }

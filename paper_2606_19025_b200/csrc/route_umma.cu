@@ -37,10 +37,16 @@ struct RouteUmmaParams {
   int32_t* blk_hist;  // [gridDim.x, n_res]
 };
 
-// slot_of[e] and the bf16 split of W_r: wr_split[i, piece*Epad + e], zero elsewhere (row stride NP).
+// slot_of[e] and the bf16 split of W_r: wr_split[i, piece*Epad + e], zero elsewhere (row stride NP); also presets
+// row_token / prow_token to -1 (rows that no kept pair claims).
 __global__ void route_prep_kernel(const int32_t* __restrict__ resident_ids, int n_res, int E, int32_t* __restrict__ slot_of,
-                                  const float* __restrict__ w_r, int d, int Epad, int pieces, int NP, bf16* __restrict__ wr_split) {
+                                  const float* __restrict__ w_r, int d, int Epad, int pieces, int NP, bf16* __restrict__ wr_split,
+                                  int32_t* __restrict__ row_token, long n_row_token, int32_t* __restrict__ prow_token, long n_prow_token) {
+  pdl_launch_dependents();
+  pdl_wait();
   const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  for (long i = idx; i < n_row_token; i += (long)gridDim.x * blockDim.x) row_token[i] = -1;
+  for (long i = idx; i < n_prow_token; i += (long)gridDim.x * blockDim.x) prow_token[i] = -1;
   if (idx < E) {
     int s = -1;
     for (int i = 0; i < n_res; ++i)
@@ -79,7 +85,7 @@ route_umma_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_consta
   const int num_kb = p.d / 64;
   const uint32_t tmem_cols = p.NP <= 64 ? 64u : p.NP <= 128 ? 128u : 256u;
 
-  for (int i = threadIdx.x; i < p.E; i += kRThreads) s_slot[i] = p.slot_of[i];
+  pdl_launch_dependents();
   for (int i = threadIdx.x; i < p.n_res; i += kRThreads) s_hist[i] = 0;
   if (warp == 0 && lane == 0) { prefetch_tmap(&map_x); prefetch_tmap(&map_w); }
   if (warp == 1 && lane == 0) {
@@ -91,6 +97,8 @@ route_umma_kernel(const __grid_constant__ CUtensorMap map_x, const __grid_consta
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(tmem_cols) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
+  pdl_wait();   // everything above touches only shared / tensor memory
+  for (int i = threadIdx.x; i < p.E; i += kRThreads) s_slot[i] = p.slot_of[i];
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -272,8 +280,8 @@ int launch_route_umma(const fomoe_config& c, const void* x, const float* w_route
   const int NP = (pieces * Epad + 63) / 64 * 64;
   {
     const long n = (long)d * NP > E ? (long)d * NP : E;
-    route_prep_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(resident_ids, n_res, E, ws.slot_of, w_router, d, Epad, pieces, NP,
-                                                                  (bf16*)ws.wr_split);
+    FOMOE_CUDA_OK(launch_pdl(route_prep_kernel, (unsigned)((n + 255) / 256), 256, 0, st, resident_ids, n_res, E, ws.slot_of, w_router, d,
+                             Epad, pieces, NP, (bf16*)ws.wr_split, out.row_token, (long)c.T * c.top_k, ws.prow_token, (long)ws.R_cap));
     FOMOE_LAUNCH_OK("route_prep_kernel");
   }
   CUtensorMap mx, mw;
@@ -286,7 +294,7 @@ int launch_route_umma(const fomoe_config& c, const void* x, const float* w_route
 #define ROUTE_UMMA_CASE(KM)                                                                                        \
   {                                                                                                                \
     FOMOE_CUDA_OK(cudaFuncSetAttribute(route_umma_kernel<KM>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); \
-    route_umma_kernel<KM><<<grid, kRThreads, smem, st>>>(mx, mw, p);                                               \
+    FOMOE_CUDA_OK(launch_pdl(route_umma_kernel<KM>, grid, kRThreads, smem, st, mx, mw, p));                        \
   }
   if (c.top_k <= 2) ROUTE_UMMA_CASE(2)
   else if (c.top_k <= 4) ROUTE_UMMA_CASE(4)

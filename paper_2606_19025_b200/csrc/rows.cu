@@ -48,6 +48,8 @@ template <typename T, int V>
 __global__ void __launch_bounds__(kRowThreads)
 gather_rows_kernel(const T* __restrict__ x, const int32_t* __restrict__ prow_token, const int32_t* __restrict__ n_mtiles, int d,
                    T* __restrict__ xp) {
+  pdl_launch_dependents();
+  pdl_wait();
   const int rows = n_mtiles[1];
   for (int r = blockIdx.x; r < rows; r += gridDim.x) {
     const int t = prow_token[r];
@@ -64,6 +66,8 @@ template <typename T, int V>
 __global__ void __launch_bounds__(kRowThreads)
 combine_kernel(const T* __restrict__ o, const T* __restrict__ y_sh, const float* __restrict__ gate,
                const int32_t* __restrict__ pair_prow, int T_, int d, int k, T* __restrict__ y) {
+  pdl_launch_dependents();
+  pdl_wait();
   for (int t = blockIdx.x; t < T_; t += gridDim.x) {
     for (int c = threadIdx.x * V; c < d; c += kRowThreads * V) {
       Vec<T, V> acc;
@@ -88,6 +92,8 @@ __global__ void __launch_bounds__(kRowThreads)
 combine_bwd_kernel(const T* __restrict__ dy, const T* __restrict__ o, const int32_t* __restrict__ prow_token,
                    const float* __restrict__ prow_gate, const int32_t* __restrict__ prow_pair,
                    const int32_t* __restrict__ n_mtiles, int d, T* __restrict__ dop, float* __restrict__ dgate) {
+  pdl_launch_dependents();
+  pdl_wait();
   __shared__ float red[kRowThreads / 32];
   const int rows = n_mtiles[1];
   for (int r = blockIdx.x; r < rows; r += gridDim.x) {
@@ -128,6 +134,8 @@ __global__ void gate_bwd_kernel(const float* __restrict__ probs, const int32_t* 
                                 const float* __restrict__ gate, const int32_t* __restrict__ pair_prow,
                                 const float* __restrict__ dgate, int T_, int E, int k, int gate_fn, int gate_rule,
                                 float inv_tau, DZ* __restrict__ dz, int ldz) {
+  pdl_launch_dependents();
+  pdl_wait();
   const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (warp >= T_) return;
   const int t = warp;
@@ -175,6 +183,8 @@ template <typename T, int V>
 __global__ void __launch_bounds__(kRowThreads)
 dx_sum_kernel(const T* __restrict__ dxp, const T* __restrict__ dx_sh, const float* __restrict__ dx_r, const T* __restrict__ dx_r_t,
               const int32_t* __restrict__ pair_prow, int T_, int d, int k, T* __restrict__ dx) {
+  pdl_launch_dependents();
+  pdl_wait();
   for (int t = blockIdx.x; t < T_; t += gridDim.x) {
     for (int c = threadIdx.x * V; c < d; c += kRowThreads * V) {
       Vec<T, V> acc;
@@ -215,8 +225,8 @@ dx_sum_kernel(const T* __restrict__ dxp, const T* __restrict__ dx_sh, const floa
   } while (0)
 
 int launch_gather_rows(const fomoe_config& c, const void* x, const RouteWs& ws, void* xp, cudaStream_t st) {
-  ROWS_DISPATCH(c, (gather_rows_kernel<T, V><<<row_grid(ws.R_cap), kRowThreads, 0, st>>>((const T*)x, ws.prow_token, ws.n_mtiles,
-                                                                                         c.d_model, (T*)xp)));
+  ROWS_DISPATCH(c, FOMOE_CUDA_OK(launch_pdl(gather_rows_kernel<T, V>, row_grid(ws.R_cap), kRowThreads, 0, st, (const T*)x, ws.prow_token,
+                                            ws.n_mtiles, c.d_model, (T*)xp)));
   FOMOE_LAUNCH_OK("gather_rows_kernel");
   return FOMOE_OK;
 }
@@ -224,17 +234,17 @@ int launch_gather_rows(const fomoe_config& c, const void* x, const RouteWs& ws, 
 int launch_combine(const fomoe_config& c, const fomoe_route_state& r, const RouteWs& ws, const void* o, const void* y_sh,
                    void* y, cudaStream_t st) {
   if (c.T == 0) return FOMOE_OK;
-  ROWS_DISPATCH(c, (combine_kernel<T, V><<<row_grid(c.T), kRowThreads, 0, st>>>((const T*)o, (const T*)y_sh, r.gate, ws.pair_prow,
-                                                                                c.T, c.d_model, c.top_k, (T*)y)));
+  ROWS_DISPATCH(c, FOMOE_CUDA_OK(launch_pdl(combine_kernel<T, V>, row_grid(c.T), kRowThreads, 0, st, (const T*)o, (const T*)y_sh, r.gate,
+                                            ws.pair_prow, c.T, c.d_model, c.top_k, (T*)y)));
   FOMOE_LAUNCH_OK("combine_kernel");
   return FOMOE_OK;
 }
 
 int launch_combine_bwd(const fomoe_config& c, const void* dy, const void* o, const RouteWs& ws, void* dop, float* dgate,
                        cudaStream_t st) {
-  FOMOE_CUDA_OK(cudaMemsetAsync(dgate, 0, sizeof(float) * (size_t)c.T * c.top_k, st));
-  ROWS_DISPATCH(c, (combine_bwd_kernel<T, V><<<row_grid(ws.R_cap), kRowThreads, 0, st>>>(
-                       (const T*)dy, (const T*)o, ws.prow_token, ws.prow_gate, ws.prow_pair, ws.n_mtiles, c.d_model, (T*)dop, dgate)));
+  // dgate is written for every kept pair and read (gate_bwd_kernel) for kept pairs only: no clearing needed
+  ROWS_DISPATCH(c, FOMOE_CUDA_OK(launch_pdl(combine_bwd_kernel<T, V>, row_grid(ws.R_cap), kRowThreads, 0, st, (const T*)dy, (const T*)o,
+                                            ws.prow_token, ws.prow_gate, ws.prow_pair, ws.n_mtiles, c.d_model, (T*)dop, dgate)));
   FOMOE_LAUNCH_OK("combine_bwd_kernel");
   return FOMOE_OK;
 }
@@ -243,11 +253,11 @@ int launch_gate_bwd(const fomoe_config& c, const fomoe_route_state& r, const Rou
                     void* dz_bf, int ldz_bf, cudaStream_t st) {
   if (c.T == 0) return FOMOE_OK;
   if (dz_bf)
-    gate_bwd_kernel<__nv_bfloat16><<<ceil_div(c.T, 8), 256, 0, st>>>(r.probs, r.topk_idx, r.gate, ws.pair_prow, dgate, c.T, c.E, c.top_k,
-                                                                     c.gate_fn, c.gate_rule, 1.0f / c.temperature, (__nv_bfloat16*)dz_bf, ldz_bf);
+    FOMOE_CUDA_OK(launch_pdl(gate_bwd_kernel<__nv_bfloat16>, ceil_div(c.T, 8), 256, 0, st, r.probs, r.topk_idx, r.gate, ws.pair_prow, dgate,
+                             c.T, c.E, c.top_k, c.gate_fn, c.gate_rule, 1.0f / c.temperature, (__nv_bfloat16*)dz_bf, ldz_bf));
   else
-    gate_bwd_kernel<float><<<ceil_div(c.T, 8), 256, 0, st>>>(r.probs, r.topk_idx, r.gate, ws.pair_prow, dgate, c.T, c.E, c.top_k,
-                                                             c.gate_fn, c.gate_rule, 1.0f / c.temperature, dz, c.E);
+    FOMOE_CUDA_OK(launch_pdl(gate_bwd_kernel<float>, ceil_div(c.T, 8), 256, 0, st, r.probs, r.topk_idx, r.gate, ws.pair_prow, dgate, c.T,
+                             c.E, c.top_k, c.gate_fn, c.gate_rule, 1.0f / c.temperature, dz, c.E));
   FOMOE_LAUNCH_OK("gate_bwd_kernel");
   return FOMOE_OK;
 }
@@ -255,8 +265,8 @@ int launch_gate_bwd(const fomoe_config& c, const fomoe_route_state& r, const Rou
 int launch_dx_sum(const fomoe_config& c, const RouteWs& ws, const void* dxp, const void* dx_sh, const float* dx_r, const void* dx_r_t,
                   void* dx, cudaStream_t st) {
   if (c.T == 0) return FOMOE_OK;
-  ROWS_DISPATCH(c, (dx_sum_kernel<T, V><<<row_grid(c.T), kRowThreads, 0, st>>>((const T*)dxp, (const T*)dx_sh, dx_r, (const T*)dx_r_t,
-                                                                               ws.pair_prow, c.T, c.d_model, c.top_k, (T*)dx)));
+  ROWS_DISPATCH(c, FOMOE_CUDA_OK(launch_pdl(dx_sum_kernel<T, V>, row_grid(c.T), kRowThreads, 0, st, (const T*)dxp, (const T*)dx_sh, dx_r,
+                                            (const T*)dx_r_t, ws.pair_prow, c.T, c.d_model, c.top_k, (T*)dx)));
   FOMOE_LAUNCH_OK("dx_sum_kernel");
   return FOMOE_OK;
 }

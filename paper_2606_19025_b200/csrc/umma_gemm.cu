@@ -232,6 +232,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
   const int cluster_id = blockIdx.x >> 1, n_clusters = gridDim.x >> 1;
   constexpr bool kAMn = (MODE == WGRAD), kBMn = (MODE == DH || MODE == DX || MODE == WGRAD);
 
+  pdl_launch_dependents();
   if (warp == 0 && lane == 0) {
 #pragma unroll
     for (int i = 0; i < 4; ++i) prefetch_tmap(&maps.m[i]);
@@ -249,6 +250,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
   cluster_sync_all();   // barriers of both CTAs initialised, tensor memory allocated in both
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  pdl_wait();   // the prologue above touched only shared / tensor memory; everything below reads the previous kernels' output
 
   const Sched<MODE> sched(p, rank);
   const bool dense = p.n_mtiles == nullptr;
@@ -543,7 +545,7 @@ int launch(const TmaMaps& maps, const UmmaParams& p, cudaStream_t st, const char
     FOMOE_CUDA_OK(cudaFuncSetAttribute(umma_grouped_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes_of(MODE)));
     attr_set = true;
   }
-  umma_grouped_kernel<MODE><<<num_sms() & ~1, kThreads, smem_bytes_of(MODE), st>>>(maps, p);
+  FOMOE_CUDA_OK(launch_pdl(umma_grouped_kernel<MODE>, num_sms() & ~1, kThreads, smem_bytes_of(MODE), st, maps, p));
   FOMOE_LAUNCH_OK(name);
   return FOMOE_OK;
 }
@@ -713,12 +715,16 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
 
 namespace {
 __global__ void wr_to_bf16_kernel(const float* __restrict__ w_r, int d, int E, int Ez, bf16* __restrict__ out) {
+  pdl_launch_dependents();
+  pdl_wait();
   const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= (long)d * Ez) return;
   const int i = (int)(idx / Ez), e = (int)(idx % Ez);
   out[idx] = __float2bfloat16_rn(e < E ? w_r[(size_t)i * E + e] : 0.f);
 }
 __global__ void reduce_wr_parts_kernel(const float* __restrict__ part, int n_parts, int d, int E, int Ez, float* __restrict__ out) {
+  pdl_launch_dependents();
+  pdl_wait();
   const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= (long)d * E) return;
   const int i = (int)(idx / E), e = (int)(idx % E);
@@ -732,7 +738,7 @@ int umma_router_bwd(const fomoe_config& c, const void* x, const float* w_router,
   const int d = c.d_model, E = c.E, Ez = sws.Ez, T = c.T;
   {
     const long n = (long)d * Ez;
-    wr_to_bf16_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(w_router, d, E, Ez, (bf16*)sws.wr_bf);
+    FOMOE_CUDA_OK(launch_pdl(wr_to_bf16_kernel, (unsigned)((n + 255) / 256), 256, 0, st, w_router, d, E, Ez, (bf16*)sws.wr_bf));
     FOMOE_LAUNCH_OK("wr_to_bf16_kernel");
   }
   {  // dx_r [T,d] = dz [T,Ez] W_r^T : FWD2 shape on dense rows (A = dz, K = Ez; B = W_r [d,Ez] K-major)
@@ -767,7 +773,7 @@ int umma_router_bwd(const fomoe_config& c, const void* x, const float* w_router,
   }
   {
     const long n = (long)d * E;
-    reduce_wr_parts_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(sws.dwr_part, G, d, E, Ez, dw_router);
+    FOMOE_CUDA_OK(launch_pdl(reduce_wr_parts_kernel, (unsigned)((n + 255) / 256), 256, 0, st, sws.dwr_part, G, d, E, Ez, dw_router));
     FOMOE_LAUNCH_OK("reduce_wr_parts_kernel");
   }
   return FOMOE_OK;
