@@ -179,12 +179,30 @@ def run_reference(args, w, n_res):
 # ------------------------------------------------------------------------------------------------------------------
 def gemm_flops(mode: str, P: int, T: int, w: W.MoEWorkload) -> float:
     """Algorithmic flops of one launch: 2*rows*d*F per GEMM; FWD1 and DX are two GEMMs."""
+    if "ROUTE" in mode:    # logits x W_r (the bf16 split of W_r multiplies the tensor work, not the algorithmic flops)
+        return 2.0 * T * w.d * w.E
     if "router" in mode:   # dz W_r^T and x^T dz: 2*T*d*E each
         return 2.0 * T * w.d * w.E
     shared = "shared" in mode
     rows, F = (T * w.n_sh, w.F_sh) if shared else (P, w.F)
     mult = 4 if ("FWD1" in mode or "DX" in mode) else 2
     return float(mult) * rows * w.d * F
+
+
+def hbm_bytes(name: str, P: int, T: int, w: W.MoEWorkload):
+    """Algorithmic bytes of one launch of the bandwidth-bound kernels; None for the others."""
+    s = 2 if w.dtype == "bf16" else 4
+    if "ROUTE" in name or name.startswith("route_kernel"):
+        return T * w.d * s + T * w.E * 4 + T * w.k * 8
+    if name.startswith("gather_rows"):
+        return 2 * P * w.d * s
+    if name.startswith("combine_kernel"):
+        return (P + T * (2 if w.n_sh else 1)) * w.d * s
+    if name.startswith("combine_bwd"):
+        return 3 * P * w.d * s
+    if name.startswith("dx_sum"):
+        return (P + T * (2 + (1 if w.n_sh else 0))) * w.d * s
+    return None
 
 
 def run_gpu(args, w, n_res):
@@ -293,7 +311,12 @@ def run_gpu(args, w, n_res):
         kernels = []
         for name, (tt, n) in sorted(agg.items(), key=lambda kv: -kv[1][0]):
             k = {"name": name, "launches_per_step": n / args.steps, "ms_per_launch": tt / n, "share": tt / total}
-            if name.startswith("umma_grouped_kernel"):
+            hb = hbm_bytes(name, P, w.T, w)
+            if hb is not None:
+                k.update(bound="hbm", achieved=hb / (tt / n / 1e3) / 1e9, unit="GB/s")
+                k["frac"] = k["achieved"] / peaks["hbm_gbs"]
+                k["frac_of_nominal_8000"] = k["achieved"] / 8000.0
+            elif name.startswith("umma_grouped_kernel"):
                 fl = gemm_flops(name, P, w.T, w)
                 k.update(bound="tensor", achieved=fl / (tt / n / 1e3) / 1e12, unit="TFLOP/s")
                 k["frac"] = k["achieved"] / tc_peak

@@ -181,7 +181,9 @@ int fomoe_moe_bwd(const fomoe_config* cfg, const void* dy, const void* x, const 
   const bool tc_router = use_umma(*cfg) && cfg->T > 0;
   rc = launch_gate_bwd(*cfg, *route, rws, sws.dgate, sws.dz, tc_router ? sws.dz_bf : nullptr, sws.Ez, st);
   if (rc != FOMOE_OK) return rc;
-  rc = tc_router ? umma_router_bwd(*cfg, x, w_router, sws, dw_router, st) : simt_router_bwd(*cfg, x, w_router, sws, dw_router, st);
+  // (the tensor-core router of fomoe_route left W_r in bf16 in the route workspace)
+  rc = tc_router ? umma_router_bwd(*cfg, x, w_router, route_umma_supported(*cfg) ? rws.wr_bf : nullptr, sws, dw_router, st)
+                 : simt_router_bwd(*cfg, x, w_router, sws, dw_router, st);
   if (rc != FOMOE_OK) return rc;
   // B5
   return launch_dx_sum(*cfg, rws, sws.dxp, cfg->n_shared > 0 ? sws.dx_sh : nullptr, tc_router ? nullptr : sws.dx_r,

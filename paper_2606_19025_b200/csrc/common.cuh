@@ -71,6 +71,7 @@ struct RouteWs {
   int32_t* slot_of;     // [E]            resident slot of expert e or -1 (ghost)
   int32_t* blk_hist;    // [n_blk, n_res] kept pairs per (permutation block, slot); then exclusive over blocks
   int32_t* pad_offsets; // [n_res+1]      first padded row of slot s (multiples of kTileM)
+  int32_t* pad_end64;   // [n_res]        pad_offsets[s] + count[s] rounded up to 64: end of the K range of the slot's wgrad
   int32_t* n_mtiles;    // [4]            [0] = number of kTileM-row tiles in use, [1] = padded rows in use, [2] = tile pairs
   int32_t* tile_slot;   // [max_mtiles]   slot of row tile i
   int32_t* pair_info;   // [max_mtiles]   CTA-pair work items: 2 * first row tile + (second tile belongs to the same slot)
@@ -79,6 +80,7 @@ struct RouteWs {
   int32_t* prow_pair;   // [R_cap]        t*k+j of padded row r
   int32_t* pair_prow;   // [T*k]          padded row of pair, -1 if skipped
   void* wr_split;       // [d, 256] bf16  W_r split into bf16 pieces for the tensor-core router
+  void* wr_bf;          // [d, Ez] bf16   W_r rounded to bf16, Ez = E rounded up to 64 (tensor-core router backward)
   int n_blk, max_mtiles, R_cap;
   size_t bytes;
 };
@@ -97,6 +99,7 @@ inline RouteWs carve_route_ws(const fomoe_config& c, int n_res, void* base) {
   w.slot_of = (int32_t*)take(sizeof(int32_t) * (size_t)c.E);
   w.blk_hist = (int32_t*)take(sizeof(int32_t) * (size_t)w.n_blk * (size_t)(n_res > 0 ? n_res : 1));
   w.pad_offsets = (int32_t*)take(sizeof(int32_t) * (size_t)(n_res + 1));
+  w.pad_end64 = (int32_t*)take(sizeof(int32_t) * (size_t)(n_res > 0 ? n_res : 1));
   w.n_mtiles = (int32_t*)take(sizeof(int32_t) * 4);
   w.tile_slot = (int32_t*)take(sizeof(int32_t) * (size_t)w.max_mtiles);
   w.pair_info = (int32_t*)take(sizeof(int32_t) * (size_t)w.max_mtiles);
@@ -105,6 +108,7 @@ inline RouteWs carve_route_ws(const fomoe_config& c, int n_res, void* base) {
   w.prow_pair = (int32_t*)take(sizeof(int32_t) * (size_t)w.R_cap);
   w.pair_prow = (int32_t*)take(sizeof(int32_t) * (size_t)(pairs > 0 ? pairs : 1));
   w.wr_split = take(sizeof(__nv_bfloat16) * (size_t)c.d_model * 256);
+  w.wr_bf = take(sizeof(__nv_bfloat16) * (size_t)c.d_model * (size_t)((c.E + 63) / 64 * 64));
   w.bytes = off;
   return w;
 }
@@ -227,8 +231,14 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
                  const ScratchWs& sws, const FfnPtrs& w, void* dw_gate, void* dw_up, void* dw_down, void* d_sh_gate,
                  void* d_sh_up, void* d_sh_down, cudaStream_t st);
 
+// F1-F4 on tensor cores (ROUTE mode of the grouped kernel); called by launch_route_umma after the preparation kernel
+int umma_route(const fomoe_config& c, const void* x, const void* wr_split, int NP, int Epad, int pieces, const float* bias, int n_res,
+               const fomoe_route_state& out, const RouteWs& ws, cudaStream_t st);
+
 // B7 on tensor cores: dx_r (bf16, into sws.dx_r reinterpreted) = dz W_r^T and dW_r = x^T dz (split-K, fp32 partials)
-int umma_router_bwd(const fomoe_config& c, const void* x, const float* w_router, const ScratchWs& sws, float* dw_router, cudaStream_t st);
+// wr_bf: W_r already rounded to bf16 [d, Ez] by the tensor-core router's preparation kernel, or nullptr (converted here)
+int umma_router_bwd(const fomoe_config& c, const void* x, const float* w_router, const void* wr_bf, const ScratchWs& sws,
+                    float* dw_router, cudaStream_t st);
 
 int launch_pack(const float* const w_now[3], const float* const w_start[3], int n_res, int64_t eg, int64_t eu, int64_t ed,
                 const int32_t* pack_slots, int n_pack, float* payload, cudaStream_t st);

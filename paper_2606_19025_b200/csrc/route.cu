@@ -171,7 +171,7 @@ __global__ void perm_hist_kernel(const int32_t* __restrict__ topk_idx, const int
 // One block.  Per slot: exclusive scan of the per-block counts (in place) -> counts; then offsets, tile-padded
 // offsets, the row-tile -> slot map and the number of tiles in use.  One warp per slot, 32 blocks per shuffle scan.
 __global__ void perm_scan_kernel(int32_t* __restrict__ blk_hist, int n_blk, int n_res, int32_t* __restrict__ counts,
-                                 int32_t* __restrict__ offsets, int32_t* __restrict__ pad_offsets,
+                                 int32_t* __restrict__ offsets, int32_t* __restrict__ pad_offsets, int32_t* __restrict__ pad_end64,
                                  int32_t* __restrict__ n_mtiles, int32_t* __restrict__ tile_slot, int32_t* __restrict__ pair_info) {
   __shared__ int32_t s_pad[kMaxE + 1];
   __shared__ int32_t s_pair[kMaxE + 1];  // first tile pair of slot s (a pair = two row tiles of ONE slot, the last may be single)
@@ -201,6 +201,7 @@ __global__ void perm_scan_kernel(int32_t* __restrict__ blk_hist, int n_blk, int 
     for (int s = 0; s < n_res; ++s) {
       offsets[s] = off;
       pad_offsets[s] = pad;
+      pad_end64[s] = pad + (s_cnt[s] + 63) / 64 * 64;
       s_pad[s] = pad;
       s_pair[s] = pairs;
       off += s_cnt[s];
@@ -320,6 +321,7 @@ int launch_route(const fomoe_config& c, const void* x, const float* w_router, co
     FOMOE_CUDA_OK(cudaMemsetAsync(out.offsets, 0, sizeof(int32_t) * (size_t)(n_res + 1), st));
     FOMOE_CUDA_OK(cudaMemsetAsync(ws.pad_offsets, 0, sizeof(int32_t) * (size_t)(n_res + 1), st));
     FOMOE_CUDA_OK(cudaMemsetAsync(ws.n_mtiles, 0, sizeof(int32_t) * 4, st));
+    FOMOE_CUDA_OK(cudaMemsetAsync(ws.pad_end64, 0, sizeof(int32_t) * (size_t)nr, st));
     return FOMOE_OK;
   }
   if (tc) {
@@ -336,7 +338,7 @@ int launch_route(const fomoe_config& c, const void* x, const float* w_router, co
     FOMOE_LAUNCH_OK("perm_hist_kernel");
   }
   FOMOE_CUDA_OK(launch_pdl(perm_scan_kernel, 1, 1024, 0, st, ws.blk_hist, ws.n_blk, n_res, out.counts, out.offsets, ws.pad_offsets,
-                           ws.n_mtiles, ws.tile_slot, ws.pair_info));
+                           ws.pad_end64, ws.n_mtiles, ws.tile_slot, ws.pair_info));
   FOMOE_LAUNCH_OK("perm_scan_kernel");
   FOMOE_CUDA_OK(launch_pdl(perm_scatter_kernel, ws.n_blk, kPermThreads, sizeof(int32_t) * 9 * nr, st, out.topk_idx, out.gate, ws.slot_of,
                            ws.blk_hist, out.offsets, ws.pad_offsets, n_pairs, pairs_per_blk, c.top_k, n_res, out.row_token, out.pair_row,

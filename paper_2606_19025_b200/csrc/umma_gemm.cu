@@ -40,11 +40,12 @@ constexpr int kEpiWarps = 8;    // two warps per TMEM lane quarter; they take al
 // row-per-thread TMEM layout into coalesced 16-byte global accesses
 constexpr int kStgTile = 2048;
 constexpr int kDhDepth = 3;  // DH epilogue: chunks of (a, u) kept in flight per warp with cp.async
-enum Mode { FWD1 = 0, FWD2 = 1, DH = 2, DX = 3, WGRAD = 4 };
+enum Mode { FWD1 = 0, FWD2 = 1, DH = 2, DX = 3, WGRAD = 4, ROUTE = 5 };
+constexpr int kRouteStg = 16384;  // ROUTE epilogue scratch: slot map, per-stage histograms, top-k merge lists
 // DH and FWD1 trade TMA stages for epilogue staging: DH streams a and u back in through a cp.async ring
 __host__ __device__ constexpr int stages_of(int mode) { return mode == DH ? 4 : mode == FWD1 ? 5 : 6; }
 __host__ __device__ constexpr int stg_tiles_per_warp(int mode) { return mode == DH ? 2 * kDhDepth : mode == FWD1 ? 3 : 1; }
-__host__ __device__ constexpr int stg_bytes_of(int mode) { return kEpiWarps * stg_tiles_per_warp(mode) * kStgTile; }
+__host__ __device__ constexpr int stg_bytes_of(int mode) { return mode == ROUTE ? kRouteStg : kEpiWarps * stg_tiles_per_warp(mode) * kStgTile; }
 __host__ __device__ constexpr int smem_bytes_of(int mode) {
   return stages_of(mode) * kStageBytes + stg_bytes_of(mode) + 1024 /*align*/ + 256 /*barriers*/;
 }
@@ -54,11 +55,24 @@ struct TmaMaps {
   CUtensorMap m[4];
 };
 
+// ROUTE mode (rows F1-F4 + the per-block histogram of F5): everything the router epilogue needs
+struct RouteEpi {
+  int E, Epad, pieces, k, gate_fn, gate_rule, n_res;
+  float inv_tau;
+  const float* bias;
+  const int32_t* slot_of;
+  float* probs;
+  int32_t* topk_idx;
+  float* gate;
+  int32_t* blk_hist;  // [ceil(T / 128), n_res]
+};
+
 struct UmmaParams {
   const int32_t* n_mtiles;     // routed: device, [2] = tile pairs in use; nullptr = dense rows
   const int32_t* tile_slot;    // routed: slot of row tile
   const int32_t* pair_info;    // routed: 2 * first row tile + (second tile in the same slot)
-  const int32_t* pad_offsets;  // routed WGRAD: padded row range of group g
+  const int32_t* pad_offsets;  // routed WGRAD: first padded row of group g
+  const int32_t* pad_end64;    // routed WGRAD: end of group g's K range (count rounded up to BK; the rows up to it are zero padding)
   int dense_rows;              // dense: number of rows (T)
   int parts;                   // dense: number of shared experts (1 for routed)
   int n_groups;                // WGRAD: number of groups (n_res or n_shared)
@@ -70,6 +84,7 @@ struct UmmaParams {
   float* out_f32;              // WGRAD: if set, fp32 output [n_groups, M, N] instead of out0
   bf16 *out0, *out1, *out2;    // FWD1: a,u,h | FWD2/DX: out | DH: da,du | WGRAD: dW
   const bf16 *in0, *in1;       // DH: a,u
+  RouteEpi r;                  // ROUTE
 };
 
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, bool valid) {
@@ -134,6 +149,7 @@ __host__ __device__ constexpr uint32_t make_idesc(int a_mn, int b_mn, int n) {
 struct Tile {
   int row0;        // first of THIS CTA's 128 rows (row modes) / output rows (WGRAD)
   bool live;       // this CTA's rows exist (false: second half of a single-tile pair, or beyond the row count)
+  bool peer_live;  // row modes: CTA 1's rows exist
   int n_tile;      // column tile
   int n_mma;       // N of the MMA: 256, or 128 when at most 128 columns of the tile exist
   int slot, part, group;  // group: WGRAD only
@@ -158,7 +174,7 @@ struct Sched {
       m_pairs = dense ? (p.dense_rows + 2 * BM - 1) / (2 * BM) : p.n_mtiles[2];
       const int n_extent = (MODE == FWD1 || MODE == DH) ? p.F : p.d;
       const int bn = MODE == FWD1 ? BN / 2 : BN;
-      n_tiles_n = (n_extent + bn - 1) / bn;
+      n_tiles_n = MODE == ROUTE ? 1 : (n_extent + bn - 1) / bn;
       ntn_total = n_tiles_n * ((dense && (MODE == FWD1 || MODE == DH)) ? p.parts : 1);
       total = (long)m_pairs * ntn_total;
     }
@@ -171,11 +187,12 @@ struct Sched {
       int rem = (int)(id % ((long)m_pairs * n_tiles_n));
       t.row0 = (rem / n_tiles_n) * 2 * BM + rank * BM;
       t.live = t.row0 < p.M;
+      t.peer_live = true;
       t.n_tile = rem % n_tiles_n;
       t.n_mma = (p.N - t.n_tile * BN <= BN / 2) ? BN / 2 : BN;
       t.slot = t.part = t.group;
       int r0, r1;
-      if (p.pad_offsets) { r0 = p.pad_offsets[t.group]; r1 = p.pad_offsets[t.group + 1]; }
+      if (p.pad_offsets) { r0 = p.pad_offsets[t.group]; r1 = p.pad_end64[t.group]; }
       else if (p.k_chunk > 0) { r0 = min(t.group * p.k_chunk, p.dense_rows); r1 = min(r0 + p.k_chunk, p.dense_rows); }
       else { r0 = 0; r1 = p.dense_rows; }
       t.k_row0 = r0;
@@ -188,20 +205,22 @@ struct Sched {
       if (dense) {
         t.row0 = pair * 2 * BM + rank * BM;
         t.live = t.row0 < p.dense_rows;
+        t.peer_live = pair * 2 * BM + BM < p.dense_rows;
         t.slot = t.part;
       } else {
         const int info = p.pair_info[pair];
         const int first = info >> 1;
         t.row0 = (first + rank) * BM;
         t.live = rank == 0 || (info & 1);
+        t.peer_live = (info & 1) != 0;
         t.slot = p.tile_slot[first];
       }
       t.group = 0;
       t.k_row0 = 0;
       const int kparts = dense ? p.parts : 1;
       const int n_extent = (MODE == DH) ? p.F : p.d;
-      t.n_mma = (MODE != FWD1 && n_extent - t.n_tile * BN <= BN / 2) ? BN / 2 : BN;
-      if (MODE == FWD1 || MODE == DH) t.num_kb = p.d / BK;
+      t.n_mma = MODE == ROUTE ? p.N : (MODE != FWD1 && n_extent - t.n_tile * BN <= BN / 2) ? BN / 2 : BN;
+      if (MODE == FWD1 || MODE == DH || MODE == ROUTE) t.num_kb = p.d / BK;
       else if (MODE == FWD2) t.num_kb = kparts * (p.F / BK);
       else t.num_kb = 2 * kparts * (p.F / BK);  // DX
     }
@@ -210,11 +229,198 @@ struct Sched {
 };
 
 // ---------------------------------------------------------------------------------------------------------
+// ROUTE epilogue: gate + top-k + residency mask + per-block histogram straight from tensor memory.
+// Accumulator columns are [hi | mid | lo] pieces of the logits (Epad columns each, see route_umma.cu); a token row is one
+// TMEM lane.  Two warps share a lane quarter: warp `half` takes the 16-expert chunks half, half + 2, ...; they exchange
+// their partial max / top-k list / softmax sum through shared memory (named barrier 1 + q, 64 threads) and the
+// half-0 thread finishes the token.  Selection is on the logits z (ties -> lower expert id), Eq. 14;
+// mask and gate rule PAPER.md:157-159, 593.
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16]) {
+  uint32_t* r = reinterpret_cast<uint32_t*>(v);
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+                 "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+               : "r"(taddr));
+}
+__device__ __forceinline__ void bar_sync_named(int id, int threads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory"); }
+
+struct RouteSmem {            // lives in the kernel's staging area (kRouteStg bytes)
+  int32_t slot[128];          // resident slot of expert e, -1 = ghost
+  int32_t hist[kAccStages][128];
+  float lv[8][128];           // half 1 -> half 0: top-k values / ids of row r
+  int32_t li[8][128];
+  float mx[2][128];           // partial max of each half
+  float sum[2][128];          // partial softmax denominators
+};
+static_assert(sizeof(RouteSmem) <= kRouteStg, "route epilogue scratch");
+
+template <int KMAX>
+__device__ __forceinline__ void route_tile_epilogue(const UmmaParams& p, RouteSmem* rs, uint32_t taddr, int q, int half, int lane, int as,
+                                                    int row0, bool live) {
+  const RouteEpi& r = p.r;
+  const int E = r.E, Epad = r.Epad;
+  const bool three = r.pieces == 3, softmax = r.gate_fn == FOMOE_GATE_SOFTMAX;
+  const int rl = q * 32 + lane;        // row within the CTA's 128
+  const int t = row0 + rl;
+  const bool row_ok = live && t < p.dense_rows;
+  if (live) {
+    auto load_z = [&](int c0, float (&z)[16]) {   // logits of 16 experts from c0: identical arithmetic in every pass
+      float md[16], lo[16];
+      tmem_ld16(taddr + c0, z);
+      tmem_ld16(taddr + Epad + c0, md);
+      if (three) tmem_ld16(taddr + 2 * Epad + c0, lo);
+      tmem_ld_wait();
+#pragma unroll
+      for (int i = 0; i < 16; ++i) {
+        float s = z[i] + md[i];
+        if (three) s += lo[i];
+        z[i] = s * r.inv_tau + (r.bias && c0 + i < E ? r.bias[c0 + i] : 0.f);
+      }
+    };
+    // pass 1: partial max and partial top-KMAX (descending, ties -> lower id: ascending scan + strict '>')
+    float tv[KMAX];
+    int ti[KMAX];
+#pragma unroll
+    for (int j = 0; j < KMAX; ++j) { tv[j] = -INFINITY; ti[j] = kMaxE; }
+    float mx = -INFINITY;
+#pragma unroll 1
+    for (int c0 = 16 * half; c0 < Epad; c0 += 32) {
+      float z[16];
+      load_z(c0, z);
+#pragma unroll
+      for (int i = 0; i < 16; ++i) {
+        if (c0 + i < E) {
+          float cv = z[i];
+          int ci = c0 + i;
+          mx = fmaxf(mx, cv);
+          if (cv > tv[KMAX - 1]) {
+            bool ins = false;
+#pragma unroll
+            for (int j = 0; j < KMAX; ++j) {
+              const bool gt = ins || cv > tv[j];
+              const float ov = tv[j];
+              const int oi = ti[j];
+              tv[j] = gt ? cv : ov;
+              ti[j] = gt ? ci : oi;
+              cv = gt ? ov : cv;
+              ci = gt ? oi : ci;
+              ins = gt;
+            }
+          }
+        }
+      }
+    }
+    rs->mx[half][rl] = mx;
+    if (half == 1) {
+#pragma unroll
+      for (int j = 0; j < KMAX; ++j) { rs->lv[j][rl] = tv[j]; rs->li[j][rl] = ti[j]; }
+    }
+    bar_sync_named(1 + q, 64);
+    mx = fmaxf(rs->mx[0][rl], rs->mx[1][rl]);
+    if (half == 0) {   // merge the partner's list: insert its entries (descending) with the (value, lower id) order
+#pragma unroll 1
+      for (int jj = 0; jj < KMAX; ++jj) {
+        float cv = rs->lv[jj][rl];
+        int ci = rs->li[jj][rl];
+        bool ins = false;
+#pragma unroll
+        for (int j = 0; j < KMAX; ++j) {
+          const bool gt = ins || cv > tv[j] || (cv == tv[j] && ci < ti[j]);
+          const float ov = tv[j];
+          const int oi = ti[j];
+          tv[j] = gt ? cv : ov;
+          ti[j] = gt ? ci : oi;
+          cv = gt ? ov : cv;
+          ci = gt ? oi : ci;
+          ins = gt;
+        }
+      }
+    }
+    // pass 2 (softmax): denominator, summed as (half 0) + (half 1) by both warps
+    float inv_s = 1.f;
+    if (softmax) {
+      float sm = 0.f;
+  #pragma unroll 1
+    for (int c0 = 16 * half; c0 < Epad; c0 += 32) {
+        float z[16];
+        load_z(c0, z);
+#pragma unroll
+        for (int i = 0; i < 16; ++i)
+          if (c0 + i < E) sm += __expf(z[i] - mx);
+      }
+      rs->sum[half][rl] = sm;
+      bar_sync_named(1 + q, 64);
+      inv_s = 1.0f / (rs->sum[0][rl] + rs->sum[1][rl]);
+    }
+    auto prob_of = [&](float z) { return softmax ? __expf(z - mx) * inv_s : __fdividef(1.0f, 1.0f + __expf(-z)); };
+    // pass 3: probabilities of this warp's chunks
+#pragma unroll 1
+    for (int c0 = 16 * half; c0 < Epad; c0 += 32) {
+      float z[16];
+      load_z(c0, z);
+#pragma unroll
+      for (int i = 0; i < 16; ++i) z[i] = prob_of(z[i]);
+      if (row_ok) {
+        float* dst = r.probs + (size_t)t * E + c0;
+        if ((E & 3) == 0) {
+#pragma unroll
+          for (int v = 0; v < 4; ++v)
+            if (c0 + 4 * v < E) *reinterpret_cast<float4*>(dst + 4 * v) = make_float4(z[4 * v], z[4 * v + 1], z[4 * v + 2], z[4 * v + 3]);
+        } else {
+#pragma unroll
+          for (int i = 0; i < 16; ++i)
+            if (c0 + i < E) dst[i] = z[i];
+        }
+      }
+    }
+    // residency mask, gate rule, outputs, per-slot histogram of the block
+    if (half == 0 && row_ok) {
+      float pj[KMAX];
+      int sl[KMAX];
+      float s_all = 0.f, s_kept = 0.f;
+#pragma unroll
+      for (int j = 0; j < KMAX; ++j) {
+        pj[j] = 0.f;
+        sl[j] = -1;
+        if (j < r.k) {
+          pj[j] = prob_of(tv[j]);
+          sl[j] = rs->slot[ti[j]];
+          s_all += pj[j];
+          if (sl[j] >= 0) s_kept += pj[j];
+        }
+      }
+#pragma unroll
+      for (int j = 0; j < KMAX; ++j) {
+        if (j < r.k) {
+          float g = 0.f;
+          if (sl[j] >= 0) {
+            g = r.gate_rule == FOMOE_DROP_ONLY ? pj[j] : r.gate_rule == FOMOE_RENORM_TOPK ? pj[j] / s_all : pj[j] / s_kept;
+            atomicAdd(&rs->hist[as][sl[j]], 1);
+          }
+          r.topk_idx[(size_t)t * r.k + j] = ti[j];
+          r.gate[(size_t)t * r.k + j] = g;
+        }
+      }
+    }
+  }
+  // all 8 epilogue warps: the block's histogram is complete; flush and clear it (next use of hist[as] is two tiles later)
+  bar_sync_named(5, kEpiWarps * 32);
+  if (live) {
+    const int tid = (half * 4 + q) * 32 + lane;
+    for (int i = tid; i < r.n_res; i += kEpiWarps * 32) {
+      r.blk_hist[(size_t)(row0 / BM) * r.n_res + i] = rs->hist[as][i];
+      rs->hist[as][i] = 0;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // the kernel
 // ---------------------------------------------------------------------------------------------------------
-template <int MODE>
+template <int MODE, int KMAX = 0>   // KMAX: ROUTE only, capacity of the top-k list (2, 4 or 8)
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
-umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
+umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant__ UmmaParams p) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   constexpr int kStages = stages_of(MODE);
@@ -230,7 +436,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int rank = (int)cluster_ctarank();
   const int cluster_id = blockIdx.x >> 1, n_clusters = gridDim.x >> 1;
-  constexpr bool kAMn = (MODE == WGRAD), kBMn = (MODE == DH || MODE == DX || MODE == WGRAD);
+  constexpr bool kAMn = (MODE == WGRAD), kBMn = (MODE == DH || MODE == DX || MODE == WGRAD || MODE == ROUTE);
 
   pdl_launch_dependents();
   if (warp == 0 && lane == 0) {
@@ -264,27 +470,34 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
         const Tile t = sched.decode(id);
         const int m0 = t.row0;
         const int nh = t.n_mma / 2;                 // B columns staged by each CTA
+        const bool peer_live = MODE == WGRAD || t.peer_live;
         for (int kb = 0; kb < t.num_kb; ++kb) {
           mbar_wait(smem_u32(&empty_bar[stage]), phase ^ 1);
           const uint32_t sa = smem_u32(smem + stage * kStageBytes), sb = sa + kABytes;
           const uint32_t fb = mapa_u32(smem_u32(&full_bar[stage]), 0);
-          if (rank == 0) mbar_expect_tx(smem_u32(&full_bar[stage]), 2 * kStageBytes);
+          // a pair whose second row tile does not exist (odd tile count of a slot, or the dense tail) skips CTA 1's A load:
+          // the MMA then reads stale shared memory for rows nobody stores.  `peer_live` is what CTA 1 decodes as t.live
+          if (rank == 0) mbar_expect_tx(smem_u32(&full_bar[stage]), 2 * kStageBytes - (peer_live ? 0 : kABytes));
           if (MODE == FWD1) {
-            tma_load_2d_2sm(sa, &maps.m[0], fb, kb * BK, m0);
+            if (t.live) tma_load_2d_2sm(sa, &maps.m[0], fb, kb * BK, m0);
             // N columns [0,128) = a (W_gate rows, staged by CTA 0), [128,256) = u (W_up rows, CTA 1)
             tma_load_2d_2sm(sb, &maps.m[1 + rank], fb, kb * BK, t.slot * p.F + t.n_tile * (BN / 2));
           } else if (MODE == FWD2) {
             const int kpp = p.F / BK, part = kb / kpp, kk = kb % kpp;
-            tma_load_2d_2sm(sa, &maps.m[0], fb, part * p.F + kk * BK, m0);
+            if (t.live) tma_load_2d_2sm(sa, &maps.m[0], fb, part * p.F + kk * BK, m0);
             tma_load_2d_2sm(sb, &maps.m[1], fb, kk * BK, (dense ? part : t.slot) * p.d + t.n_tile * BN + rank * nh);
+          } else if (MODE == ROUTE) {   // A = x rows (K-major), B = split W_r [d, N] (MN-major), CTA r stages columns [r N/2, (r+1) N/2)
+            if (t.live) tma_load_2d_2sm(sa, &maps.m[0], fb, kb * BK, m0);
+#pragma unroll
+            for (int j = 0; j < BN / 128; ++j) tma_load_2d_2sm(sb + j * 8192, &maps.m[1], fb, rank * nh + 64 * j, kb * BK);
           } else if (MODE == DH) {
-            tma_load_2d_2sm(sa, &maps.m[0], fb, kb * BK, m0);
+            if (t.live) tma_load_2d_2sm(sa, &maps.m[0], fb, kb * BK, m0);
 #pragma unroll
             for (int j = 0; j < BN / 128; ++j)
               tma_load_2d_2sm(sb + j * 8192, &maps.m[1], fb, t.n_tile * BN + rank * nh + 64 * j, t.slot * p.d + kb * BK);
           } else if (MODE == DX) {
             const int kseg = (dense ? p.parts : 1) * (p.F / BK), seg = kb / kseg, kk = kb % kseg;
-            tma_load_2d_2sm(sa, &maps.m[seg], fb, kk * BK, m0);
+            if (t.live) tma_load_2d_2sm(sa, &maps.m[seg], fb, kk * BK, m0);
             const int brow = (dense ? 0 : t.slot * p.F) + kk * BK;
 #pragma unroll
             for (int j = 0; j < BN / 128; ++j)
@@ -348,7 +561,28 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
     const int half = (warp >> 2) - 1;     // which of the two warps of the quarter: takes chunks half, half + 2, ...
     const uint32_t stg0 = smem_u32(stg_base) + (uint32_t)((warp - 4) * (kStgTilesPerWarp * kStgTile));
     const uint32_t tempty_leader = mapa_u32(smem_u32(&tempty_bar[0]), 0);  // + 8 * stage
-    if (MODE == DH) {
+    if (MODE == ROUTE) {
+      RouteSmem* rs = reinterpret_cast<RouteSmem*>(stg_base);
+      {  // slot map and cleared histograms, visible to all epilogue warps before the first tile
+        const int tid = threadIdx.x - 128;
+        for (int i = tid; i < p.r.E; i += kEpiWarps * 32) rs->slot[i] = p.r.slot_of[i];
+        for (int i = tid; i < kAccStages * 128; i += kEpiWarps * 32) (&rs->hist[0][0])[i] = 0;
+        bar_sync_named(5, kEpiWarps * 32);
+      }
+      int as = 0;
+      uint32_t aphase = 0;
+      for (long id = cluster_id; id < sched.total; id += n_clusters) {
+        const Tile t = sched.decode(id);
+        const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * BN;
+        mbar_wait(smem_u32(&tfull_bar[as]), aphase);
+        tc_fence_after();
+        route_tile_epilogue<(KMAX > 0 ? KMAX : 2)>(p, rs, taddr, q, half, lane, as, t.row0, t.live);
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(tempty_leader + 8 * as);
+        if (++as == kAccStages) { as = 0; aphase ^= 1; }
+      }
+    } else if (MODE == DH) {
       // SwiGLU backward needs a and u for every output element.  They are streamed global -> shared with cp.async,
       // kDhDepth 32-column chunks ahead of the consumer and across tile boundaries (the schedule is static), so the
       // loads never sit on the critical path of the accumulator drain.  A ring slot (a tile | u tile) is overwritten in
@@ -538,14 +772,14 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const UmmaParams p) {
 // ---------------------------------------------------------------------------------------------------------
 // host side: tensor maps and launches
 // ---------------------------------------------------------------------------------------------------------
-template <int MODE>
+template <int MODE, int KMAX = 0>
 int launch(const TmaMaps& maps, const UmmaParams& p, cudaStream_t st, const char* name) {
   static bool attr_set = false;
   if (!attr_set) {
-    FOMOE_CUDA_OK(cudaFuncSetAttribute(umma_grouped_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes_of(MODE)));
+    FOMOE_CUDA_OK(cudaFuncSetAttribute(umma_grouped_kernel<MODE, KMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes_of(MODE)));
     attr_set = true;
   }
-  FOMOE_CUDA_OK(launch_pdl(umma_grouped_kernel<MODE>, num_sms() & ~1, kThreads, smem_bytes_of(MODE), st, maps, p));
+  FOMOE_CUDA_OK(launch_pdl(umma_grouped_kernel<MODE, KMAX>, num_sms() & ~1, kThreads, smem_bytes_of(MODE), st, maps, p));
   FOMOE_LAUNCH_OK(name);
   return FOMOE_OK;
 }
@@ -557,6 +791,22 @@ bool umma_supported(const fomoe_config& c) {
   if (c.d_model % 64 || c.d_ff % 64) return false;
   if (c.n_shared > 0 && c.d_ff_shared % 64) return false;
   return true;
+}
+
+// Router logits + gate + top-k + mask + per-block histogram (ROUTE mode).  wr_split: [d, NP] bf16 pieces of W_r, NP = 128 or 256.
+int umma_route(const fomoe_config& c, const void* x, const void* wr_split, int NP, int Epad, int pieces, const float* bias, int n_res,
+               const fomoe_route_state& out, const RouteWs& ws, cudaStream_t st) {
+  UmmaParams p{};
+  p.dense_rows = c.T; p.parts = 1; p.d = c.d_model; p.F = NP; p.ld = NP; p.N = NP;
+  p.r = RouteEpi{c.E, Epad, pieces, c.top_k, c.gate_fn, c.gate_rule, n_res, 1.0f / c.temperature, bias, ws.slot_of,
+                 out.probs, out.topk_idx, out.gate, ws.blk_hist};
+  TmaMaps m{};
+  MAP_OK(make_map(&m.m[0], x, c.d_model, c.T, c.d_model, 128));
+  MAP_OK(make_map(&m.m[1], wr_split, NP, c.d_model, NP, 64));
+  m.m[2] = m.m[3] = m.m[0];
+  if (c.top_k <= 2) return launch<ROUTE, 2>(m, p, st, "umma_grouped_kernel<ROUTE>");
+  if (c.top_k <= 4) return launch<ROUTE, 4>(m, p, st, "umma_grouped_kernel<ROUTE>");
+  return launch<ROUTE, 8>(m, p, st, "umma_grouped_kernel<ROUTE>");
 }
 
 int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs& rws, const ActWs& aws, const ScratchWs& sws,
@@ -624,7 +874,7 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
   if (n_res > 0) {
     const uint64_t R = (uint64_t)rws.R_cap;
     UmmaParams p{};
-    p.n_mtiles = rws.n_mtiles; p.tile_slot = rws.tile_slot; p.pair_info = rws.pair_info; p.pad_offsets = rws.pad_offsets; p.parts = 1; p.d = d; p.F = F; p.ld = F;
+    p.n_mtiles = rws.n_mtiles; p.tile_slot = rws.tile_slot; p.pair_info = rws.pair_info; p.pad_offsets = rws.pad_offsets; p.pad_end64 = rws.pad_end64; p.parts = 1; p.d = d; p.F = F; p.ld = F;
     if (c.T > 0) {
       {  // dh = dO W_down, fused SwiGLU backward
         TmaMaps m{};
@@ -734,9 +984,11 @@ __global__ void reduce_wr_parts_kernel(const float* __restrict__ part, int n_par
 }
 }  // namespace
 
-int umma_router_bwd(const fomoe_config& c, const void* x, const float* w_router, const ScratchWs& sws, float* dw_router, cudaStream_t st) {
+int umma_router_bwd(const fomoe_config& c, const void* x, const float* w_router, const void* wr_bf, const ScratchWs& sws,
+                    float* dw_router, cudaStream_t st) {
   const int d = c.d_model, E = c.E, Ez = sws.Ez, T = c.T;
-  {
+  if (!wr_bf) {
+    wr_bf = sws.wr_bf;
     const long n = (long)d * Ez;
     FOMOE_CUDA_OK(launch_pdl(wr_to_bf16_kernel, (unsigned)((n + 255) / 256), 256, 0, st, w_router, d, E, Ez, (bf16*)sws.wr_bf));
     FOMOE_LAUNCH_OK("wr_to_bf16_kernel");
@@ -746,7 +998,7 @@ int umma_router_bwd(const fomoe_config& c, const void* x, const float* w_router,
     p.dense_rows = T; p.parts = 1; p.d = d; p.F = Ez; p.ld = Ez;
     TmaMaps m{};
     MAP_OK(make_map(&m.m[0], sws.dz_bf, Ez, T, Ez, 128));
-    MAP_OK(make_map(&m.m[1], sws.wr_bf, Ez, d, Ez, 128));
+    MAP_OK(make_map(&m.m[1], wr_bf, Ez, d, Ez, 128));
     m.m[2] = m.m[3] = m.m[0];
     p.out0 = (bf16*)sws.dx_r;
     int rc = launch<FWD2>(m, p, st, "umma_grouped_kernel<FWD2,router dx>");
