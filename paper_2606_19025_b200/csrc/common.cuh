@@ -116,8 +116,8 @@ inline RouteWs carve_route_ws(const fomoe_config& c, int n_res, void* base) {
 // ---- saved activations (fwd -> bwd) and scratch ----
 struct ActWs {
   void* xp;   // [R_cap, d]   gathered token rows (zero for padding rows)
-  void* a;    // [R_cap, F]   W_gate x
-  void* u;    // [R_cap, F]   W_up x
+  void* a;    // [R_cap, F]   W_gate x          (tcgen05 path: silu'(a) * u, what the backward multiplies dh with for da)
+  void* u;    // [R_cap, F]   W_up x            (tcgen05 path: silu(a), the factor for du)
   void* h;    // [R_cap, F]   silu(a) * u
   void* o;    // [R_cap, d]   W_down h
   void* sa;   // [T, n_sh*F_sh] shared experts: a

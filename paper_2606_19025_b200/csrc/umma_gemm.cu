@@ -15,9 +15,10 @@
 // workspace): the host never learns P.
 //
 // Modes (pair tile 256 x 256, K staged 64 at a time):
-//   FWD1  [a|u] = X W_gate^T | X W_up^T   (A, B K-major; CTA0 stages W_gate, CTA1 W_up; epilogue: a, u, h = silu(a)*u)
+//   FWD1  [a|u] = X W_gate^T | X W_up^T   (A, B K-major; CTA0 stages W_gate, CTA1 W_up; epilogue: h = silu(a)*u, and
+//                                           for the backward silu'(a)*u and silu(a) in place of a and u)
 //   FWD2  o = H W_down^T                  (A, B K-major)
-//   DH    dh = dO W_down                  (A K-major, B MN-major; epilogue: SwiGLU backward -> da, du)
+//   DH    dh = dO W_down                  (A K-major, B MN-major; epilogue: da = dh * silu'(a)u, du = dh * silu(a))
 //   DX    dxp = dA W_gate + dU W_up       (A K-major, B MN-major; two K segments into one accumulator)
 //   WGRAD dW[g] = A[rows(g)]^T B[rows(g)] (A, B MN-major; K = the group's (padded) rows)
 // Row space is either the tile-padded routed rows (pairs of 128-row tiles of ONE slot; the last pair of a slot may hold a
@@ -583,7 +584,8 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
         if (++as == kAccStages) { as = 0; aphase ^= 1; }
       }
     } else if (MODE == DH) {
-      // SwiGLU backward needs a and u for every output element.  They are streamed global -> shared with cp.async,
+      // SwiGLU backward needs two saved factors (silu'(a) u and silu(a), "a" and "u" below) for every output element.
+      // They are streamed global -> shared with cp.async,
       // kDhDepth 32-column chunks ahead of the consumer and across tile boundaries (the schedule is static), so the
       // loads never sit on the critical path of the accumulator drain.  A ring slot (a tile | u tile) is overwritten in
       // place with (da | du) and stored from there.
@@ -653,12 +655,11 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
               uint32_t* pa = reinterpret_cast<uint32_t*>(&wa);
               uint32_t* pu = reinterpret_cast<uint32_t*>(&wu);
 #pragma unroll
-              for (int i = 0; i < 4; ++i) {
+              for (int i = 0; i < 4; ++i) {   // in0 = silu'(a) u, in1 = silu(a) (FWD1 epilogue): da = dh in0, du = dh in1
                 const float2 a2 = unpack_bf16x2(pa[i]), u2 = unpack_bf16x2(pu[i]);
                 const float d0 = dh[g8 * 8 + 2 * i], d1 = dh[g8 * 8 + 2 * i + 1];
-                const float s0 = __fdividef(1.0f, 1.0f + __expf(-a2.x)), s1 = __fdividef(1.0f, 1.0f + __expf(-a2.y));
-                pa[i] = pack_bf16x2(d0 * u2.x * s0 * (1.0f + a2.x * (1.0f - s0)), d1 * u2.y * s1 * (1.0f + a2.y * (1.0f - s1)));
-                pu[i] = pack_bf16x2(d0 * a2.x * s0, d1 * a2.y * s1);
+                pa[i] = pack_bf16x2(d0 * a2.x, d1 * a2.y);
+                pu[i] = pack_bf16x2(d0 * u2.x, d1 * u2.y);
               }
               sts128(sa + o, wa);   // da over a, du over u: every lane rewrites exactly the bytes it read
               sts128(su + o, wu);
@@ -721,15 +722,24 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
           for (int cc = half; cc < (BN / 2) / 32 && rows_valid > 0; cc += 2) {
             const int n = t.n_tile * (BN / 2) + cc * 32;
             if (n >= p.F) break;
-            float a[32], u[32];
+            float a[32], u[32], sa_h[32];
             tmem_ld32(taddr + cc * 32, a);
             tmem_ld32(taddr + BN / 2 + cc * 32, u);
             tmem_ld_wait();
+            // what the backward needs of (a, u) is only silu(a) and d silu(a)/da * u: save those (same bytes as a, u), so
+            // the DH epilogue is two multiplies per element instead of a sigmoid (it is epilogue-bound at small d)
+#pragma unroll
+            for (int i = 0; i < 32; ++i) {
+              const float sg = __fdividef(1.0f, 1.0f + __expf(-a[i]));
+              const float sa = a[i] * sg;                                   // silu(a)
+              a[i] = fmaf(sa, 1.0f - sg, sg) * u[i];                         // silu'(a) * u = s (1 + a (1 - s)) u
+              const float h = sa * u[i];
+              u[i] = sa;
+              sa_h[i] = h;
+            }
             stg_put_row(stg0, lane, a);
             stg_put_row(stg1, lane, u);
-#pragma unroll
-            for (int i = 0; i < 32; ++i) a[i] = __fdividef(a[i], 1.0f + __expf(-a[i])) * u[i];
-            stg_put_row(stg2, lane, a);
+            stg_put_row(stg2, lane, sa_h);
             __syncwarp();
             stg_to_global(stg0, p.out0 + base + n, p.ld, lane, rows_valid);
             stg_to_global(stg1, p.out1 + base + n, p.ld, lane, rows_valid);
