@@ -24,8 +24,9 @@
  *     "ignored by the local computational graph" ....... PAPER.md:157-159, 147 (Fig. 3)
  *   no renormalisation over the surviving experts ...... PAPER.md:593 (§B.3.2)
  *   y = sum_{i in T(x) ∩ S} s_i(x) E_i(x) .............. PAPER.md:515 (Eq. 13)
- *   expert = projection -> SiLU -> projection; BASELINE.json fixes the SwiGLU form
- *     E(x) = W_down (silu(W_gate x) ⊙ W_up x) ........... PAPER.md:589 (§B.3.1), 253
+ *   expert = projection -> SiLU -> projection, E(x) = W_down silu(W_up x) (EXPERT_SILU);
+ *     BASELINE.json's configs fix the SwiGLU form
+ *     E(x) = W_down (silu(W_gate x) ⊙ W_up x) (EXPERT_SWIGLU) PAPER.md:589 (§B.3.1), 253
  *   shared experts: fully replicated dense components .. PAPER.md:86 (§3.2)
  *   delta payload per resident expert (up+down, router
  *     column excluded in skip-token mode) .............. PAPER.md:253, 824 (Alg. 2 l.19)
@@ -49,6 +50,11 @@
 
 enum { GATE_SOFTMAX = 0, GATE_SIGMOID = 1 };
 enum { RULE_DROP_ONLY = 0, RULE_RENORM_TOPK = 1, RULE_RENORM_RESIDENT = 2 };
+/* expert form: SwiGLU (BASELINE.json's five configs) or the paper's own sigma-MoE expert
+ * E(x) = W_down SiLU(W_up x): "After each expert projection from d_model to d_expert, the Silu nonlinearity is applied"
+ * (§B.3.1); the expert payload "includes up and down projection".  In the SiLU form W_gate does
+ * not exist (pointers may be NULL, dw_gate is not written). */
+enum { EXPERT_SWIGLU = 0, EXPERT_SILU = 1 };
 
 int oracle_real_bytes(void) { return (int)sizeof(REAL); }
 
@@ -161,12 +167,19 @@ int oracle_route(int T, int d, int E, int k, int gate_fn, int gate_rule, double 
   return 0;
 }
 
-/* One SwiGLU expert on one token: a = W_g x, u = W_u x, h = a*sigmoid(a) ⊙ u, o = W_d h. */
-static void expert_fwd_(const REAL* xt, int d, int F, const REAL* wg, const REAL* wu, const REAL* wd,
+/* One expert on one token.
+ * SwiGLU: a = W_g x, u = W_u x, h = a*sigmoid(a) ⊙ u, o = W_d h.
+ * SiLU: a = W_u x, h = a*sigmoid(a), o = W_d h   (u is set to 1 so the shared backward formulas hold). */
+static void expert_fwd_(int expert_fn, const REAL* xt, int d, int F, const REAL* wg, const REAL* wu, const REAL* wd,
                         REAL* a, REAL* u, REAL* h, REAL* o) {
   for (int f = 0; f < F; ++f) {
-    a[f] = dot_(wg + (size_t)f * d, xt, d);
-    u[f] = dot_(wu + (size_t)f * d, xt, d);
+    if (expert_fn == EXPERT_SILU) {
+      a[f] = dot_(wu + (size_t)f * d, xt, d);
+      u[f] = (REAL)1;
+    } else {
+      a[f] = dot_(wg + (size_t)f * d, xt, d);
+      u[f] = dot_(wu + (size_t)f * d, xt, d);
+    }
     h[f] = a[f] * sigmoid_(a[f]) * u[f];
   }
   if (o)
@@ -177,7 +190,7 @@ static void expert_fwd_(const REAL* xt, int d, int F, const REAL* wg, const REAL
  * Steps 7-8: y_t = sum_{j kept, ascending j} g_tj * E_{e_tj}(x_t) + sum_s FFN_s(x_t)   (86)
  * Tokens with no kept pair and no shared expert give y_t = 0 exactly.
  * ---------------------------------------------------------------------------------------------- */
-int oracle_moe_fwd(int T, int d, int E, int k, int F, int n_sh, int F_sh,
+int oracle_moe_fwd(int T, int d, int E, int k, int F, int n_sh, int F_sh, int expert_fn,
                    const REAL* x, const int32_t* topk_idx, const REAL* gate,
                    const int32_t* resident_ids, int n_res,
                    const REAL* w_gate, const REAL* w_up, const REAL* w_down,
@@ -197,11 +210,11 @@ int oracle_moe_fwd(int T, int d, int E, int k, int F, int n_sh, int F_sh,
       for (int j = 0; j < k; ++j) {
         int s = slot_of[topk_idx[(size_t)t * k + j]];
         if (s < 0) continue; /* ghost expert: skipped */
-        expert_fwd_(xt, d, F, w_gate + (size_t)s * F * d, w_up + (size_t)s * F * d, w_down + (size_t)s * d * F, a, u, h, o);
+        expert_fwd_(expert_fn, xt, d, F, w_gate ? w_gate + (size_t)s * F * d : NULL, w_up + (size_t)s * F * d, w_down + (size_t)s * d * F, a, u, h, o);
         axpy_(gate[(size_t)t * k + j], o, yt, d);
       }
       for (int s = 0; s < n_sh; ++s) {
-        expert_fwd_(xt, d, F_sh, sh_gate + (size_t)s * F_sh * d, sh_up + (size_t)s * F_sh * d, sh_down + (size_t)s * d * F_sh, a, u, h, o);
+        expert_fwd_(expert_fn, xt, d, F_sh, sh_gate ? sh_gate + (size_t)s * F_sh * d : NULL, sh_up + (size_t)s * F_sh * d, sh_down + (size_t)s * d * F_sh, a, u, h, o);
         axpy_((REAL)1, o, yt, d);
       }
     }
@@ -214,11 +227,11 @@ int oracle_moe_fwd(int T, int d, int E, int k, int F, int n_sh, int F_sh,
 /* Backward of one expert on one token given do = dL/do.  Adds W_g^T da + W_u^T du into dx_acc (if
  * non-NULL) and the rank-1 weight-gradient terms into dwg/dwu/dwd (if non-NULL). Returns via a,u,h the
  * recomputed forward. */
-static void expert_bwd_(const REAL* xt, const REAL* dov, int d, int F,
+static void expert_bwd_(int expert_fn, const REAL* xt, const REAL* dov, int d, int F,
                         const REAL* wg, const REAL* wu, const REAL* wd,
                         REAL* a, REAL* u, REAL* h, REAL* dh, REAL* dx_acc,
                         REAL* dwg, REAL* dwu, REAL* dwd) {
-  expert_fwd_(xt, d, F, wg, wu, wd, a, u, h, NULL);
+  expert_fwd_(expert_fn, xt, d, F, wg, wu, wd, a, u, h, NULL);
   for (int f = 0; f < F; ++f) dh[f] = 0;
   for (int i = 0; i < d; ++i) axpy_(dov[i], wd + (size_t)i * F, dh, F); /* dh = W_d^T do */
   if (dwd)
@@ -227,6 +240,11 @@ static void expert_bwd_(const REAL* xt, const REAL* dov, int d, int F,
     REAL sg = sigmoid_(a[f]);
     REAL da = dh[f] * u[f] * sg * ((REAL)1 + a[f] * ((REAL)1 - sg)); /* d silu(a)/da = sg (1 + a (1 - sg)) */
     REAL du = dh[f] * a[f] * sg;
+    if (expert_fn == EXPERT_SILU) { /* a = W_u x is the only projection: da flows into W_up, there is no u path */
+      if (dx_acc) axpy_(da, wu + (size_t)f * d, dx_acc, d);
+      if (dwu) axpy_(da, xt, dwu + (size_t)f * d, d);
+      continue;
+    }
     if (dx_acc) {
       axpy_(da, wg + (size_t)f * d, dx_acc, d);
       axpy_(du, wu + (size_t)f * d, dx_acc, d);
@@ -243,7 +261,7 @@ static void expert_bwd_(const REAL* xt, const REAL* dov, int d, int F,
  * Outputs (all overwritten): dx [T,d]; dw_router [d,E]; dw_gate, dw_up [n_res,F,d]; dw_down [n_res,d,F];
  * d_sh_* like their weights; dgate [T,k] (dL/dg_tj, 0 for skipped pairs); dlogits [T,E].
  * ---------------------------------------------------------------------------------------------- */
-int oracle_moe_bwd(int T, int d, int E, int k, int F, int n_sh, int F_sh,
+int oracle_moe_bwd(int T, int d, int E, int k, int F, int n_sh, int F_sh, int expert_fn,
                    int gate_fn, int gate_rule, double tau,
                    const REAL* x, const REAL* dy, const REAL* w_r,
                    const REAL* probs, const int32_t* topk_idx, const REAL* gate,
@@ -278,14 +296,14 @@ int oracle_moe_bwd(int T, int d, int E, int k, int F, int n_sh, int F_sh,
         *dg = 0;
         int s = slot_of[idx[j]];
         if (s < 0) continue; /* ghost path does not exist in the graph */
-        const REAL *wg = w_gate + (size_t)s * F * d, *wu = w_up + (size_t)s * F * d, *wd = w_down + (size_t)s * d * F;
-        expert_fwd_(xt, d, F, wg, wu, wd, a, u, h, o);
+        const REAL *wg = w_gate ? w_gate + (size_t)s * F * d : NULL, *wu = w_up + (size_t)s * F * d, *wd = w_down + (size_t)s * d * F;
+        expert_fwd_(expert_fn, xt, d, F, wg, wu, wd, a, u, h, o);
         *dg = dot_(dyt, o, d);                      /* y += g o  =>  dg = <dy, o> */
         for (int i = 0; i < d; ++i) dov[i] = g[j] * dyt[i]; /*            do = g dy */
-        expert_bwd_(xt, dov, d, F, wg, wu, wd, a, u, h, dh, dxt, NULL, NULL, NULL);
+        expert_bwd_(expert_fn, xt, dov, d, F, wg, wu, wd, a, u, h, dh, dxt, NULL, NULL, NULL);
       }
       for (int s = 0; s < n_sh; ++s)
-        expert_bwd_(xt, dyt, d, F_sh, sh_gate + (size_t)s * F_sh * d, sh_up + (size_t)s * F_sh * d,
+        expert_bwd_(expert_fn, xt, dyt, d, F_sh, sh_gate ? sh_gate + (size_t)s * F_sh * d : NULL, sh_up + (size_t)s * F_sh * d,
                     sh_down + (size_t)s * d * F_sh, a, u, h, dh, dxt, NULL, NULL, NULL);
       /* gate rule backward: dp from dg */
       if (gate_rule == RULE_DROP_ONLY) {
@@ -340,9 +358,9 @@ int oracle_moe_bwd(int T, int d, int E, int k, int F, int n_sh, int F_sh,
     REAL *u = a + Fm, *h = u + Fm, *dh = h + Fm, *dov = dh + Fm;
 #pragma omp for schedule(dynamic, 1)
     for (int s = 0; s < n_res; ++s) {
-      const REAL *wg = w_gate + (size_t)s * F * d, *wu = w_up + (size_t)s * F * d, *wd = w_down + (size_t)s * d * F;
-      REAL *dwg = dw_gate + (size_t)s * F * d, *dwu = dw_up + (size_t)s * F * d, *dwd = dw_down + (size_t)s * d * F;
-      memset(dwg, 0, sizeof(REAL) * (size_t)F * d);
+      const REAL *wg = w_gate ? w_gate + (size_t)s * F * d : NULL, *wu = w_up + (size_t)s * F * d, *wd = w_down + (size_t)s * d * F;
+      REAL *dwg = dw_gate ? dw_gate + (size_t)s * F * d : NULL, *dwu = dw_up + (size_t)s * F * d, *dwd = dw_down + (size_t)s * d * F;
+      if (dwg) memset(dwg, 0, sizeof(REAL) * (size_t)F * d);
       memset(dwu, 0, sizeof(REAL) * (size_t)F * d);
       memset(dwd, 0, sizeof(REAL) * (size_t)F * d);
       for (int r = offsets[s]; r < offsets[s + 1]; ++r) {
@@ -351,17 +369,17 @@ int oracle_moe_bwd(int T, int d, int E, int k, int F, int n_sh, int F_sh,
           if (topk_idx[(size_t)t * k + jj] == resident_ids[s]) j = jj;
         REAL gj = gate[(size_t)t * k + j];
         for (int i = 0; i < d; ++i) dov[i] = gj * dy[(size_t)t * d + i];
-        expert_bwd_(x + (size_t)t * d, dov, d, F, wg, wu, wd, a, u, h, dh, NULL, dwg, dwu, dwd);
+        expert_bwd_(expert_fn, x + (size_t)t * d, dov, d, F, wg, wu, wd, a, u, h, dh, NULL, dwg, dwu, dwd);
       }
     }
     free(a);
   }
   /* shared experts: every token, gate 1 */
   for (int s = 0; s < n_sh; ++s) {
-    const REAL *wg = sh_gate + (size_t)s * F_sh * d, *wu = sh_up + (size_t)s * F_sh * d, *wd = sh_down + (size_t)s * d * F_sh;
-    REAL *dwg = d_sh_gate + (size_t)s * F_sh * d, *dwu = d_sh_up + (size_t)s * F_sh * d, *dwd = d_sh_down + (size_t)s * d * F_sh;
+    const REAL *wg = sh_gate ? sh_gate + (size_t)s * F_sh * d : NULL, *wu = sh_up + (size_t)s * F_sh * d, *wd = sh_down + (size_t)s * d * F_sh;
+    REAL *dwg = d_sh_gate ? d_sh_gate + (size_t)s * F_sh * d : NULL, *dwu = d_sh_up + (size_t)s * F_sh * d, *dwd = d_sh_down + (size_t)s * d * F_sh;
     size_t n = (size_t)F_sh * d;
-    memset(dwg, 0, sizeof(REAL) * n);
+    if (dwg) memset(dwg, 0, sizeof(REAL) * n);
     memset(dwu, 0, sizeof(REAL) * n);
     memset(dwd, 0, sizeof(REAL) * n);
 #pragma omp parallel
@@ -371,10 +389,10 @@ int oracle_moe_bwd(int T, int d, int E, int k, int F, int n_sh, int F_sh,
       REAL* loc = (REAL*)calloc(3 * n, sizeof(REAL));
 #pragma omp for schedule(static)
       for (int t = 0; t < T; ++t)
-        expert_bwd_(x + (size_t)t * d, dy + (size_t)t * d, d, F_sh, wg, wu, wd, a, u, h, dh, NULL, loc, loc + n, loc + 2 * n);
+        expert_bwd_(expert_fn, x + (size_t)t * d, dy + (size_t)t * d, d, F_sh, wg, wu, wd, a, u, h, dh, NULL, loc, loc + n, loc + 2 * n);
 #pragma omp critical
       {
-        axpy_((REAL)1, loc, dwg, (int)n);
+        if (dwg) axpy_((REAL)1, loc, dwg, (int)n);
         axpy_((REAL)1, loc + n, dwu, (int)n);
         axpy_((REAL)1, loc + 2 * n, dwd, (int)n);
       }
@@ -394,7 +412,7 @@ int oracle_moe_bwd(int T, int d, int E, int k, int F, int n_sh, int F_sh,
  * h_rf = silu(a_rf) u_rf, da = dh u s (1 + a (1 - s)), du = dh a s   (same formulas as expert_bwd_, one f at a time).
  * Outputs [n_f, d] each.  Pinned against oracle_moe_bwd in tests/test_oracle_pins.py.
  * ---------------------------------------------------------------------------------------------- */
-int oracle_dw_sample(int d, int k, int F, const REAL* x, const REAL* dy, const int32_t* topk_idx, const REAL* gate,
+int oracle_dw_sample(int d, int k, int F, int expert_fn, const REAL* x, const REAL* dy, const int32_t* topk_idx, const REAL* gate,
                      int resident_id, int row_begin, int row_end, const int32_t* row_token,
                      const REAL* wg, const REAL* wu, const REAL* wd, /* this slot's [F,d], [F,d], [d,F] */
                      const int32_t* f_idx, int n_f, REAL* dwg_rows, REAL* dwu_rows, REAL* dwd_cols) {
@@ -410,12 +428,18 @@ int oracle_dw_sample(int d, int k, int F, const REAL* x, const REAL* dy, const i
         if (topk_idx[(size_t)t * k + jj] == resident_id) j = jj;
       const REAL g = gate[(size_t)t * k + j];
       const REAL *xt = x + (size_t)t * d, *dyt = dy + (size_t)t * d;
-      REAL a = dot_(wg + (size_t)f * d, xt, d), u = dot_(wu + (size_t)f * d, xt, d);
+      const int silu = expert_fn == EXPERT_SILU; /* SiLU form: a = W_up x, u = 1, the gradient of W_up is da x */
+      REAL a = silu ? dot_(wu + (size_t)f * d, xt, d) : dot_(wg + (size_t)f * d, xt, d);
+      REAL u = silu ? (REAL)1 : dot_(wu + (size_t)f * d, xt, d);
       REAL sg = sigmoid_(a), h = a * sg * u, dh = 0;
       for (int i = 0; i < d; ++i) dh += g * dyt[i] * wd[(size_t)i * F + f];
       REAL da = dh * u * sg * ((REAL)1 + a * ((REAL)1 - sg)), du = dh * a * sg;
-      axpy_(da, xt, og, d);
-      axpy_(du, xt, ou, d);
+      if (silu) {
+        axpy_(da, xt, ou, d);
+      } else {
+        axpy_(da, xt, og, d);
+        axpy_(du, xt, ou, d);
+      }
       axpy_(g * h, dyt, od, d);
     }
   }

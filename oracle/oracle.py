@@ -74,22 +74,23 @@ class Oracle:
         return out
 
     # ---- steps 7-8 -------------------------------------------------------------------------------
-    def moe_fwd(self, x, route, resident, w_gate, w_up, w_down, shared=None, E=None):
+    def moe_fwd(self, x, route, resident, w_gate, w_up, w_down, shared=None, E=None, expert_fn=0):
+        """expert_fn 0 = SwiGLU, 1 = the paper's W_down silu(W_up x) (w_gate and shared[0] are None then)."""
         x = self._r(x)
         resident = np.ascontiguousarray(resident, dtype=np.int32)
         T, d = x.shape
         k = route["topk_idx"].shape[1]
         E = route["probs"].shape[1] if E is None else E
         wg, wu, wd = self._r(w_gate), self._r(w_up), self._r(w_down)
-        F = wg.shape[1] if wg.ndim == 3 and wg.shape[0] > 0 else (wd.shape[2] if wd.ndim == 3 else 0)
+        F = wu.shape[1] if wu.ndim == 3 and wu.shape[0] > 0 else (wd.shape[2] if wd.ndim == 3 else 0)
         sg = su = sd = None
         n_sh = F_sh = 0
         if shared is not None:
             sg, su, sd = (self._r(s) for s in shared)
-            n_sh, F_sh = sg.shape[0], sg.shape[1]
+            n_sh, F_sh = su.shape[0], su.shape[1]
         y = np.empty((T, d), self.dt)
         rc = self.lib.oracle_moe_fwd(C.c_int(T), C.c_int(d), C.c_int(E), C.c_int(k), C.c_int(F), C.c_int(n_sh), C.c_int(F_sh),
-                                     _ptr(x), _ptr(route["topk_idx"]), _ptr(self._r(route["gate"])),
+                                     C.c_int(expert_fn), _ptr(x), _ptr(route["topk_idx"]), _ptr(self._r(route["gate"])),
                                      _ptr(resident), C.c_int(len(resident)), _ptr(wg), _ptr(wu), _ptr(wd),
                                      _ptr(sg), _ptr(su), _ptr(sd), _ptr(y))
         if rc != 0:
@@ -98,7 +99,7 @@ class Oracle:
 
     # ---- step 9 ----------------------------------------------------------------------------------
     def moe_bwd(self, x, dy, w_r, route, resident, w_gate, w_up, w_down, shared=None,
-                gate_fn=0, gate_rule=0, tau=1.0):
+                gate_fn=0, gate_rule=0, tau=1.0, expert_fn=0):
         x, dy, w_r = self._r(x), self._r(dy), self._r(w_r)
         resident = np.ascontiguousarray(resident, dtype=np.int32)
         T, d = x.shape
@@ -106,25 +107,28 @@ class Oracle:
         k = route["topk_idx"].shape[1]
         wg, wu, wd = self._r(w_gate), self._r(w_up), self._r(w_down)
         n_res = len(resident)
-        F = wg.shape[1]
+        F = wu.shape[1]
         sg = su = sd = None
         n_sh = F_sh = 0
         if shared is not None:
             sg, su, sd = (self._r(s) for s in shared)
-            n_sh, F_sh = sg.shape[0], sg.shape[1]
+            n_sh, F_sh = su.shape[0], su.shape[1]
         out = dict(dx=np.empty((T, d), self.dt), dw_router=np.empty((d, E), self.dt),
-                   dw_gate=np.empty((n_res, F, d), self.dt), dw_up=np.empty((n_res, F, d), self.dt),
-                   dw_down=np.empty((n_res, d, F), self.dt),
+                   dw_up=np.empty((n_res, F, d), self.dt), dw_down=np.empty((n_res, d, F), self.dt),
                    dgate=np.empty((T, k), self.dt), dlogits=np.empty((T, E), self.dt))
+        if wg is not None:
+            out["dw_gate"] = np.empty((n_res, F, d), self.dt)
         if shared is not None:
-            out.update(d_sh_gate=np.empty_like(sg), d_sh_up=np.empty_like(su), d_sh_down=np.empty_like(sd))
+            out.update(d_sh_up=np.empty_like(su), d_sh_down=np.empty_like(sd))
+            if sg is not None:
+                out["d_sh_gate"] = np.empty_like(sg)
         rc = self.lib.oracle_moe_bwd(
-            C.c_int(T), C.c_int(d), C.c_int(E), C.c_int(k), C.c_int(F), C.c_int(n_sh), C.c_int(F_sh),
+            C.c_int(T), C.c_int(d), C.c_int(E), C.c_int(k), C.c_int(F), C.c_int(n_sh), C.c_int(F_sh), C.c_int(expert_fn),
             C.c_int(gate_fn), C.c_int(gate_rule), C.c_double(tau),
             _ptr(x), _ptr(dy), _ptr(w_r), _ptr(self._r(route["probs"])), _ptr(route["topk_idx"]), _ptr(self._r(route["gate"])),
             _ptr(resident), C.c_int(n_res), _ptr(route["offsets"]), _ptr(route["row_token"]),
             _ptr(wg), _ptr(wu), _ptr(wd), _ptr(sg), _ptr(su), _ptr(sd),
-            _ptr(out["dx"]), _ptr(out["dw_router"]), _ptr(out["dw_gate"]), _ptr(out["dw_up"]), _ptr(out["dw_down"]),
+            _ptr(out["dx"]), _ptr(out["dw_router"]), _ptr(out.get("dw_gate")), _ptr(out["dw_up"]), _ptr(out["dw_down"]),
             _ptr(out.get("d_sh_gate")), _ptr(out.get("d_sh_up")), _ptr(out.get("d_sh_down")),
             _ptr(out["dgate"]), _ptr(out["dlogits"]))
         if rc != 0:
@@ -132,15 +136,15 @@ class Oracle:
         return out
 
     # ---- sampled weight gradients (full-size parity) -----------------------------------------------
-    def dw_sample(self, x, dy, route, resident, slot, f_idx, w_gate_s, w_up_s, w_down_s):
+    def dw_sample(self, x, dy, route, resident, slot, f_idx, w_gate_s, w_up_s, w_down_s, expert_fn=0):
         """dW_gate[slot, f, :], dW_up[slot, f, :], dW_down[slot, :, f] for f in f_idx; weights are that slot's matrices."""
         x, dy = self._r(x), self._r(dy)
         wg, wu, wd = self._r(w_gate_s), self._r(w_up_s), self._r(w_down_s)
-        F, d = wg.shape
+        F, d = wu.shape
         k = route["topk_idx"].shape[1]
         f_idx = np.ascontiguousarray(f_idx, dtype=np.int32)
         outs = [np.empty((len(f_idx), d), self.dt) for _ in range(3)]
-        rc = self.lib.oracle_dw_sample(C.c_int(d), C.c_int(k), C.c_int(F), _ptr(x), _ptr(dy), _ptr(route["topk_idx"]),
+        rc = self.lib.oracle_dw_sample(C.c_int(d), C.c_int(k), C.c_int(F), C.c_int(expert_fn), _ptr(x), _ptr(dy), _ptr(route["topk_idx"]),
                                        _ptr(self._r(route["gate"])), C.c_int(int(resident[slot])),
                                        C.c_int(int(route["offsets"][slot])), C.c_int(int(route["offsets"][slot + 1])),
                                        _ptr(route["row_token"]), _ptr(wg), _ptr(wu), _ptr(wd), _ptr(f_idx), C.c_int(len(f_idx)),

@@ -17,6 +17,7 @@ import torch
 
 GATE_SOFTMAX, GATE_SIGMOID = 0, 1
 RULE_DROP_ONLY, RULE_RENORM_TOPK, RULE_RENORM_RESIDENT = 0, 1, 2
+EXPERT_SWIGLU, EXPERT_SILU = 0, 1   # SILU: the paper's expert W_down silu(W_up x); W_gate is ignored
 
 
 def tiny_problem(seed, T=6, d=5, E=4, k=2, F=3, n_res=2, n_sh=0, F_sh=0, wscale=0.5):
@@ -56,7 +57,7 @@ def _gate_probs(z, gate_fn):
     return [v / s for v in ex]
 
 
-def brute_force_fwd(prob, gate_fn=GATE_SOFTMAX, gate_rule=RULE_DROP_ONLY, tau=1.0, bias=None):
+def brute_force_fwd(prob, gate_fn=GATE_SOFTMAX, gate_rule=RULE_DROP_ONLY, tau=1.0, bias=None, expert_fn=EXPERT_SWIGLU):
     """All-experts-times-indicator evaluation with Python loops."""
     x, w_r, S, full, k, E = prob["x"], prob["w_r"], set(int(s) for s in prob["resident"]), prob["full"], prob["k"], prob["E"]
     T, d = x.shape
@@ -70,9 +71,13 @@ def brute_force_fwd(prob, gate_fn=GATE_SOFTMAX, gate_rule=RULE_DROP_ONLY, tau=1.
         s_kept = sum(p[e] for e in sel if e in S)
         for e in range(E):  # every expert is evaluated; the indicator zeroes the rest
             ind = 1.0 if (e in sel and e in S) else 0.0
-            a = full["w_gate"][e] @ x[t]
-            u = full["w_up"][e] @ x[t]
-            h = a / (1.0 + np.exp(-a)) * u
+            if expert_fn == EXPERT_SILU:
+                v = full["w_up"][e] @ x[t]
+                h = v / (1.0 + np.exp(-v))
+            else:
+                a = full["w_gate"][e] @ x[t]
+                u = full["w_up"][e] @ x[t]
+                h = a / (1.0 + np.exp(-a)) * u
             o = full["w_down"][e] @ h
             if gate_rule == RULE_DROP_ONLY:
                 g = p[e]
@@ -83,14 +88,18 @@ def brute_force_fwd(prob, gate_fn=GATE_SOFTMAX, gate_rule=RULE_DROP_ONLY, tau=1.
             y[t] += ind * g * o
         if prob["shared"] is not None:
             sg, su, sd = prob["shared"]
-            for s in range(sg.shape[0]):
+            for s in range(su.shape[0]):
+                if expert_fn == EXPERT_SILU:
+                    v = su[s] @ x[t]
+                    y[t] += sd[s] @ (v / (1.0 + np.exp(-v)))
+                    continue
                 a = sg[s] @ x[t]
                 u = su[s] @ x[t]
                 y[t] += sd[s] @ (a / (1.0 + np.exp(-a)) * u)
     return y
 
 
-def torch_dense_moe(prob, gate_fn=GATE_SOFTMAX, gate_rule=RULE_DROP_ONLY, tau=1.0, bias=None):
+def torch_dense_moe(prob, gate_fn=GATE_SOFTMAX, gate_rule=RULE_DROP_ONLY, tau=1.0, bias=None, expert_fn=EXPERT_SWIGLU):
     """Returns (y, grads dict) for L = sum(dy * y).  grads: dx, dw_router, dw_gate/up/down (resident slots), d_sh_*."""
     f64 = torch.float64
     x = torch.tensor(prob["x"], dtype=f64, requires_grad=True)
@@ -117,26 +126,37 @@ def torch_dense_moe(prob, gate_fn=GATE_SOFTMAX, gate_rule=RULE_DROP_ONLY, tau=1.
         kept = sel * res_mask
         den = (p * kept).sum(-1, keepdim=True)
         g = torch.where(den > 0, p * kept / torch.where(den > 0, den, torch.ones_like(den)), torch.zeros_like(p))
-    a = torch.einsum("td,efd->tef", x, wg)
     u = torch.einsum("td,efd->tef", x, wu)
-    h = torch.nn.functional.silu(a) * u
+    if expert_fn == EXPERT_SILU:
+        h = torch.nn.functional.silu(u)
+    else:
+        a = torch.einsum("td,efd->tef", x, wg)
+        h = torch.nn.functional.silu(a) * u
     o = torch.einsum("tef,edf->ted", h, wd)
     y = (g[:, :, None] * o).sum(1)
     sh = None
     if prob["shared"] is not None:
         sh = [torch.tensor(s, dtype=f64, requires_grad=True) for s in prob["shared"]]
-        a2 = torch.einsum("td,sfd->tsf", x, sh[0])
         u2 = torch.einsum("td,sfd->tsf", x, sh[1])
-        y = y + torch.einsum("tsf,sdf->td", torch.nn.functional.silu(a2) * u2, sh[2])
+        if expert_fn == EXPERT_SILU:
+            h2 = torch.nn.functional.silu(u2)
+        else:
+            h2 = torch.nn.functional.silu(torch.einsum("td,sfd->tsf", x, sh[0])) * u2
+        y = y + torch.einsum("tsf,sdf->td", h2, sh[2])
     L = (y * torch.tensor(prob["dy"], dtype=f64)).sum()
     L.backward()
     Sn = prob["resident"]
-    grads = dict(dx=x.grad.numpy(), dw_router=w_r.grad.numpy(), dw_gate=wg.grad.numpy()[Sn], dw_up=wu.grad.numpy()[Sn],
-                 dw_down=wd_full.grad.numpy()[Sn])
+    silu_form = expert_fn == EXPERT_SILU
+    wg_grad = np.zeros_like(prob["full"]["w_gate"]) if silu_form else wg.grad.numpy()
+    grads = dict(dx=x.grad.numpy(), dw_router=w_r.grad.numpy(), dw_up=wu.grad.numpy()[Sn], dw_down=wd_full.grad.numpy()[Sn])
+    if not silu_form:
+        grads["dw_gate"] = wg_grad[Sn]
     ghost = np.setdiff1d(np.arange(E), Sn)
-    grads["ghost_grad_max"] = max([float(np.abs(wg.grad.numpy()[ghost]).max(initial=0.0)),
+    grads["ghost_grad_max"] = max([float(np.abs(wg_grad[ghost]).max(initial=0.0)),
                                    float(np.abs(wu.grad.numpy()[ghost]).max(initial=0.0)),
                                    float(np.abs(wd_full.grad.numpy()[ghost]).max(initial=0.0))])
     if sh is not None:
-        grads.update(d_sh_gate=sh[0].grad.numpy(), d_sh_up=sh[1].grad.numpy(), d_sh_down=sh[2].grad.numpy())
+        grads.update(d_sh_up=sh[1].grad.numpy(), d_sh_down=sh[2].grad.numpy())
+        if not silu_form:
+            grads["d_sh_gate"] = sh[0].grad.numpy()
     return y.detach().numpy(), grads
