@@ -323,12 +323,17 @@ def run_gpu(args, w, n_res):
             kernels.append(k)
         out["kernels"] = kernels
         traffic = None
-        tf = ROOT / "profiles" / "traffic.json"
+        tf = ROOT / "profiles" / "r1d_traffic.csv"   # DRAM bytes per launch from the committed ncu --set full captures
+        traffic_rows = {}
+        if tf.exists():
+            for line in tf.read_text().splitlines()[1:]:
+                wl, rest = line.split(",", 1)          # kernel names contain commas: workload,kernel,bytes,launches
+                kname, nbytes, _ = rest.rsplit(",", 2)
+                traffic_rows[(wl, kname)] = float(nbytes)
         gemms = [k for k in kernels if k.get("bound") == "tensor" and "router" not in k["name"]]
         if gemms:
             dom = gemms[0]
-            if tf.exists():
-                traffic = json.loads(tf.read_text()).get(w.name, {}).get(dom["name"])
+            traffic = traffic_rows.get((w.name, dom["name"]))
             out["roofline"] = {"kernel": dom["name"], "bound": "tensor", "achieved": dom["achieved"],
                                "peak": tc_peak, "unit": "TFLOP/s", "frac": dom["frac"], "traffic": traffic,
                                "peak_source": peak_src + ", " + tc_peak_name,
