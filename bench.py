@@ -35,7 +35,9 @@ FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustain
 
 def workload_desc(w: W.MoEWorkload, n_res: int) -> str:
     sh = f" + {w.n_sh} shared (d_ff {w.F_sh})" if w.n_sh else ""
-    return (f"{w.name}: T={w.T}, d_model={w.d}, E={w.E}{sh}, top-{w.k}, SwiGLU d_ff={w.F}, {n_res} of {w.E} resident, "
+    ex = "SwiGLU d_ff" if w.expert_fn == W.EXPERT_SWIGLU else "two-matrix SiLU expert (PAPER.md:589) d_expert"
+    gf = "softmax" if w.gate_fn == W.GATE_SOFTMAX else "sigmoid"
+    return (f"{w.name}: T={w.T}, d_model={w.d}, E={w.E}{sh}, top-{w.k}, {gf} gate, {ex}={w.F}, {n_res} of {w.E} resident, "
             f"{w.dtype}, fp32 router, x~N(0,1), weights~N(0,0.02), seed {w.seed}"
             + (f", Zipf(alpha={w.zipf_alpha}) router bias" if w.zipf_alpha else ""))
 
@@ -150,8 +152,8 @@ def oracle_sample_time(w: W.MoEWorkload, n_res: int, sample_tokens: int, reps: i
     for _ in range(reps):
         t0 = time.perf_counter()
         r = o.route(x, w_r, S, ws.k, ws.gate_fn, ws.gate_rule, ws.temperature, bias)
-        o.moe_fwd(x, r, S, wg, wu, wd, shared)
-        o.moe_bwd(x, dy, w_r, r, S, wg, wu, wd, shared, ws.gate_fn, ws.gate_rule, ws.temperature)
+        o.moe_fwd(x, r, S, wg, wu, wd, shared, expert_fn=ws.expert_fn)
+        o.moe_bwd(x, dy, w_r, r, S, wg, wu, wd, shared, ws.gate_fn, ws.gate_rule, ws.temperature, expert_fn=ws.expert_fn)
         times.append(time.perf_counter() - t0)
     return times, o.threads()
 
@@ -185,7 +187,7 @@ def gemm_flops(mode: str, P: int, T: int, w: W.MoEWorkload) -> float:
         return 2.0 * T * w.d * w.E
     shared = "shared" in mode
     rows, F = (T * w.n_sh, w.F_sh) if shared else (P, w.F)
-    mult = 4 if ("FWD1" in mode or "DX" in mode) else 2
+    mult = 4 if (("FWD1" in mode and "FWD1S" not in mode) or ("DX" in mode and w.expert_fn == W.EXPERT_SWIGLU)) else 2
     return float(mult) * rows * w.d * F
 
 
@@ -285,7 +287,8 @@ def run_gpu(args, w, n_res):
         "clocks": clocks, "gpu_launches": launches[0] * args.steps,
         "kept_pairs": P, "kept_fraction": P / max(1, w.T * w.k), "ms_min": min(ms_list),
     }
-    flops_step = 18.0 * P * w.d * w.F + 18.0 * w.T * w.n_sh * w.d * w.F_sh
+    fl_pair = 18.0 if w.expert_fn == W.EXPERT_SWIGLU else 12.0   # flops per (row, d, F): 3 (2) GEMMs forward, twice that backward
+    flops_step = fl_pair * P * w.d * w.F + fl_pair * w.T * w.n_sh * w.d * w.F_sh
     out["tflops"] = flops_step / (ms / 1e3) / 1e12
 
     if rank == 0:
@@ -359,6 +362,8 @@ def run_gpu(args, w, n_res):
         # ---- resident-delta pack (row S1), HBM bound: 12 B per parameter ----
         S = W.resident_set(w, n_res)
         now = [torch.from_numpy(np.stack(t)).cuda() for t in zip(*(W.make_expert_master(w, int(e)) for e in S))]
+        if w.expert_fn == W.EXPERT_SILU:   # the paper's expert payload is up + down: no gate block
+            now[0] = now[0][:, :0].contiguous()
         start = [t + 1e-3 * torch.randn_like(t) for t in now]
         payload = torch.empty((n_res, sum(int(t[0].numel()) for t in now)), dtype=torch.float32, device="cuda")
         pk = timed_steps(lambda: pack_resident_deltas(now, start, None, payload), max(args.steps, 10), 3)
@@ -377,7 +382,7 @@ def run_gpu(args, w, n_res):
             ms_full = timed_steps(lambda: full.step(x, dy), args.steps, args.warmup)
             mf = sum(ms_full) / len(ms_full)
             out["skip_token"] = {"ms_all_resident": mf, "speedup_vs_all_resident": mf / ms,
-                                 "ideal_flop_ratio": (w.k * 18.0 * w.d * w.F * w.T + 18.0 * w.T * w.n_sh * w.d * w.F_sh) / flops_step}
+                                 "ideal_flop_ratio": (w.k * fl_pair * w.d * w.F * w.T + fl_pair * w.T * w.n_sh * w.d * w.F_sh) / flops_step}
             del full
 
         # ---- the oracle, as it stands, on the host cores (reported baseline, not the target) ----

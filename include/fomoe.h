@@ -34,7 +34,7 @@
 extern "C" {
 #endif
 
-#define FOMOE_ABI_VERSION 1
+#define FOMOE_ABI_VERSION 2
 
 #if defined(__GNUC__)
 #define FOMOE_API __attribute__((visibility("default")))
@@ -61,18 +61,25 @@ extern "C" {
 #define FOMOE_RENORM_TOPK 1     /* g = p / sum over all k selected (resident or not) */
 #define FOMOE_RENORM_RESIDENT 2 /* g = p / sum over the kept (resident) selected experts */
 
+/* fomoe_config.expert_fn: form of an expert (routed and shared alike) */
+#define FOMOE_EXPERT_SWIGLU 0 /* BASELINE.json: E(x) = W_down (silu(W_gate x) * W_up x), three matrices */
+#define FOMOE_EXPERT_SILU 1   /* paper: E(x) = W_down silu(W_up x), "after each expert projection from d_model to d_expert,
+                                 the Silu nonlinearity is applied" (§B.3.1); the expert's payload "includes up and
+                                 down projection".  W_gate / dW_gate arguments are ignored and may be NULL. */
+
 typedef struct fomoe_config {
   int32_t T;           /* tokens (batch x sequence, flattened) */
   int32_t d_model;     /* d */
   int32_t E;           /* routed experts N_e (router width), 1..512 */
   int32_t top_k;       /* k, 1..min(E,32) */
-  int32_t d_ff;        /* F: hidden size of a routed SwiGLU expert */
+  int32_t d_ff;        /* F: hidden size of a routed expert (d_expert in the paper) */
   int32_t n_shared;    /* always-resident shared experts, 0 if none */
   int32_t d_ff_shared; /* hidden size of a shared expert, 0 if none */
   int32_t dtype;       /* FOMOE_F32 | FOMOE_BF16 */
   int32_t gate_fn;     /* FOMOE_GATE_* */
   int32_t gate_rule;   /* FOMOE_DROP_ONLY | FOMOE_RENORM_* */
   float temperature;   /* tau: logits = x W_r / tau + bias (PAPER.md:175 names it, gives no formula); 1 by default */
+  int32_t expert_fn;   /* FOMOE_EXPERT_SWIGLU | FOMOE_EXPERT_SILU */
 } fomoe_config;
 
 /*
@@ -121,6 +128,7 @@ FOMOE_API int fomoe_route(const fomoe_config* cfg, const void* x, const float* w
  * Forward (rows F6-F8): y_t = sum_{j kept} g_tj W_down,e (silu(W_gate,e x_t) ⊙ W_up,e x_t) + sum_s FFN_s(x_t)
  *   (Eq. 13 over T(x) ∩ S; expert PAPER.md:589 in BASELINE.json's SwiGLU form; shared PAPER.md:86).
  *   Tokens with no kept pair and no shared expert get y_t = 0 exactly.
+ *   With cfg->expert_fn == FOMOE_EXPERT_SILU every expert is W_down silu(W_up x) and the *_gate arguments are ignored.
  * w_gate, w_up [n_res,F,d]; w_down [n_res,d,F]  (cfg->dtype; may be NULL iff n_res == 0)
  * sh_gate, sh_up [n_shared,F_sh,d]; sh_down [n_shared,d,F_sh]  (NULL iff n_shared == 0)
  * y [T,d] cfg->dtype, overwritten.   saved_acts, scratch: see fomoe_workspace_bytes.
@@ -154,6 +162,7 @@ FOMOE_API int fomoe_moe_bwd(const fomoe_config* cfg, const void* dy, const void*
  * in skip-token mode.  All fp32; each word is one IEEE subtraction (bit-exact vs the oracle).
  * w_now / w_start: host arrays of 3 device pointers (gate, up, down), each [n_res, elems_*] fp32.
  * pack_slots: [n_pack] int32 device or NULL (= all slots, n_pack must equal n_res).  elems_* must be multiples of 4.
+ * A tensor with elems_* == 0 may be NULL: the paper's two-matrix expert packs up | down only (elems_gate = 0).
  */
 FOMOE_API int fomoe_pack_resident_deltas(const float* const w_now[3], const float* const w_start[3], int32_t n_res,
                                int64_t elems_gate, int64_t elems_up, int64_t elems_down,

@@ -47,6 +47,7 @@ static int check_cfg(const fomoe_config* c, int n_res) {
   if (c->gate_fn != FOMOE_GATE_SOFTMAX && c->gate_fn != FOMOE_GATE_SIGMOID) return FOMOE_ERR_BADARG;
   if (c->gate_rule < FOMOE_DROP_ONLY || c->gate_rule > FOMOE_RENORM_RESIDENT) return FOMOE_ERR_BADARG;
   if (!(c->temperature > 0.f)) return FOMOE_ERR_BADARG;
+  if (c->expert_fn != FOMOE_EXPERT_SWIGLU && c->expert_fn != FOMOE_EXPERT_SILU) return FOMOE_ERR_BADARG;
   if (c->E > kMaxE || c->top_k > kMaxK) return FOMOE_ERR_UNSUPPORTED;
   if ((long)c->T * c->top_k + (long)kTileM * (n_res + 1) > 0x7fffffffL / 2) return FOMOE_ERR_UNSUPPORTED;  // int32 row ids
   return FOMOE_OK;
@@ -124,8 +125,9 @@ int fomoe_moe_fwd(const fomoe_config* cfg, const void* x, const fomoe_route_stat
   int rc = check_cfg(cfg, n_res);
   if (rc != FOMOE_OK) return rc;
   if (!route || !route->internal || !saved_acts || !scratch || ((!x || !y) && cfg->T > 0)) return FOMOE_ERR_BADARG;
-  if (n_res > 0 && (!w_gate || !w_up || !w_down)) return FOMOE_ERR_BADARG;
-  if (cfg->n_shared > 0 && (!sh_gate || !sh_up || !sh_down)) return FOMOE_ERR_BADARG;
+  const bool swiglu = cfg->expert_fn == FOMOE_EXPERT_SWIGLU;   // the paper's two-matrix expert has no W_gate
+  if (n_res > 0 && ((swiglu && !w_gate) || !w_up || !w_down)) return FOMOE_ERR_BADARG;
+  if (cfg->n_shared > 0 && ((swiglu && !sh_gate) || !sh_up || !sh_down)) return FOMOE_ERR_BADARG;
   if (!aligned16(x) || !aligned16(y) || !aligned16(saved_acts) || !aligned16(scratch) || !aligned16(w_gate) || !aligned16(w_up) ||
       !aligned16(w_down) || !aligned16(sh_gate) || !aligned16(sh_up) || !aligned16(sh_down))
     return FOMOE_ERR_BADARG;
@@ -154,8 +156,9 @@ int fomoe_moe_bwd(const fomoe_config* cfg, const void* dy, const void* x, const 
   if (rc != FOMOE_OK) return rc;
   if (!route || !route->internal || !saved_acts || !scratch || !w_router || !dw_router) return FOMOE_ERR_BADARG;
   if (cfg->T > 0 && (!dy || !x || !dx)) return FOMOE_ERR_BADARG;
-  if (n_res > 0 && (!w_gate || !w_up || !w_down || !dw_gate || !dw_up || !dw_down)) return FOMOE_ERR_BADARG;
-  if (cfg->n_shared > 0 && (!sh_gate || !sh_up || !sh_down || !d_sh_gate || !d_sh_up || !d_sh_down)) return FOMOE_ERR_BADARG;
+  const bool swiglu = cfg->expert_fn == FOMOE_EXPERT_SWIGLU;
+  if (n_res > 0 && ((swiglu && (!w_gate || !dw_gate)) || !w_up || !w_down || !dw_up || !dw_down)) return FOMOE_ERR_BADARG;
+  if (cfg->n_shared > 0 && ((swiglu && (!sh_gate || !d_sh_gate)) || !sh_up || !sh_down || !d_sh_up || !d_sh_down)) return FOMOE_ERR_BADARG;
   if (!aligned16(dy) || !aligned16(x) || !aligned16(dx) || !aligned16(dw_router) || !aligned16(dw_gate) || !aligned16(dw_up) ||
       !aligned16(dw_down) || !aligned16(d_sh_gate) || !aligned16(d_sh_up) || !aligned16(d_sh_down) || !aligned16(scratch) ||
       !aligned16(saved_acts))
@@ -198,8 +201,11 @@ int fomoe_pack_resident_deltas(const float* const w_now[3], const float* const w
   if (!pack_slots && n_pack != n_res) return FOMOE_ERR_BADARG;
   if (n_pack == 0) return FOMOE_OK;
   if (!payload || !aligned16(payload)) return FOMOE_ERR_BADARG;
-  for (int i = 0; i < 3; ++i)
-    if (!w_now[i] || !w_start[i] || !aligned16(w_now[i]) || !aligned16(w_start[i])) return FOMOE_ERR_BADARG;
+  const int64_t elems[3] = {elems_gate, elems_up, elems_down};
+  for (int i = 0; i < 3; ++i) {   // a tensor of zero elements may be NULL (two-matrix expert: no gate block)
+    if (elems[i] > 0 && (!w_now[i] || !w_start[i])) return FOMOE_ERR_BADARG;
+    if (!aligned16(w_now[i]) || !aligned16(w_start[i])) return FOMOE_ERR_BADARG;
+  }
   if (elems_gate % 4 || elems_up % 4 || elems_down % 4) return FOMOE_ERR_UNSUPPORTED;
   note_api_entry("@fomoe_pack_resident_deltas", (cudaStream_t)stream);
   return launch_pack(w_now, w_start, n_res, elems_gate, elems_up, elems_down, pack_slots, n_pack, payload, (cudaStream_t)stream);

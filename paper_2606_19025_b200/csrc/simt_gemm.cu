@@ -82,6 +82,7 @@ __device__ __forceinline__ bool row_tile(const RowSpace& rs, int& row0, int& m_v
 }
 
 // F6 / F6s: a = X W_g^T, u = X W_u^T, h = silu(a) * u.   X [rows, d]; W [slots, F, d]; outputs [rows, ld] at col part*F.
+// Wg == nullptr: the paper's two-matrix expert, a = X W_u^T, h = silu(a); u is not written.
 template <typename T>
 __global__ void __launch_bounds__(kGemmThreads)
 simt_ffn1_kernel(RowSpace rs, const T* __restrict__ X, int d, int F, const T* __restrict__ Wg, const T* __restrict__ Wu, int ld,
@@ -94,8 +95,9 @@ simt_ffn1_kernel(RowSpace rs, const T* __restrict__ X, int d, int F, const T* __
   zero_acc(ag);
   zero_acc(au);
   const T* A = X + (size_t)row0 * d;
-  tile_acc(ag, A, d, 1, m_valid, Wg + ((size_t)slot * F + n0) * d, d, 1, n_valid, d, sm);
-  tile_acc(au, A, d, 1, m_valid, Wu + ((size_t)slot * F + n0) * d, d, 1, n_valid, d, sm);
+  const bool silu_only = Wg == nullptr;
+  tile_acc(ag, A, d, 1, m_valid, (silu_only ? Wu : Wg) + ((size_t)slot * F + n0) * d, d, 1, n_valid, d, sm);
+  if (!silu_only) tile_acc(au, A, d, 1, m_valid, Wu + ((size_t)slot * F + n0) * d, d, 1, n_valid, d, sm);
   const int ty = threadIdx.x >> 4, tx = threadIdx.x & 15;
 #pragma unroll
   for (int i = 0; i < 4; ++i)
@@ -104,9 +106,9 @@ simt_ffn1_kernel(RowSpace rs, const T* __restrict__ X, int d, int F, const T* __
       int m = ty * 4 + i, n = tx * 4 + j;
       if (m < m_valid && n < n_valid) {
         size_t off = (size_t)(row0 + m) * ld + (size_t)part * F + n0 + n;
-        float av = ag[i][j], uv = au[i][j];
+        float av = ag[i][j], uv = silu_only ? 1.0f : au[i][j];
         a_out[off] = from_f32<T>(av);
-        u_out[off] = from_f32<T>(uv);
+        if (!silu_only) u_out[off] = from_f32<T>(uv);
         h_out[off] = from_f32<T>(av / (1.0f + expf(-av)) * uv);
       }
     }
@@ -158,10 +160,10 @@ simt_dh_kernel(RowSpace rs, const T* __restrict__ dO, int d, int F, const T* __r
       int m = ty * 4 + i, n = tx * 4 + j;
       if (m < m_valid && n < n_valid) {
         size_t off = (size_t)(row0 + m) * ld + (size_t)part * F + n0 + n;
-        float av = to_f32(a_in[off]), uv = to_f32(u_in[off]), dh = acc[i][j];
+        float av = to_f32(a_in[off]), uv = u_in ? to_f32(u_in[off]) : 1.0f, dh = acc[i][j];   // u_in == nullptr: h = silu(a)
         float s = 1.0f / (1.0f + expf(-av));
         da_out[off] = from_f32<T>(dh * uv * s * (1.0f + av * (1.0f - s)));
-        du_out[off] = from_f32<T>(dh * av * s);
+        if (u_in) du_out[off] = from_f32<T>(dh * av * s);
       }
     }
 }
@@ -180,8 +182,12 @@ simt_dx_kernel(RowSpace rs, const T* __restrict__ dA, const T* __restrict__ dU, 
   for (int p = 0; p < parts; ++p) {
     int s = rs.tile_slot ? slot : p;
     // B(n = i, k = f) = W[s][f][i]
-    tile_acc(acc, dA + (size_t)row0 * ld + (size_t)p * F, ld, 1, m_valid, Wg + (size_t)s * F * d + n0, 1, d, n_valid, F, sm);
-    tile_acc(acc, dU + (size_t)row0 * ld + (size_t)p * F, ld, 1, m_valid, Wu + (size_t)s * F * d + n0, 1, d, n_valid, F, sm);
+    if (Wg) {
+      tile_acc(acc, dA + (size_t)row0 * ld + (size_t)p * F, ld, 1, m_valid, Wg + (size_t)s * F * d + n0, 1, d, n_valid, F, sm);
+      tile_acc(acc, dU + (size_t)row0 * ld + (size_t)p * F, ld, 1, m_valid, Wu + (size_t)s * F * d + n0, 1, d, n_valid, F, sm);
+    } else {  // two-matrix expert: dxp = dA W_up
+      tile_acc(acc, dA + (size_t)row0 * ld + (size_t)p * F, ld, 1, m_valid, Wu + (size_t)s * F * d + n0, 1, d, n_valid, F, sm);
+    }
   }
   const int ty = threadIdx.x >> 4, tx = threadIdx.x & 15;
 #pragma unroll
@@ -253,8 +259,10 @@ __global__ void reduce_parts_kernel(const float* __restrict__ part, int n_parts,
 // ---------------------------------------------------------------------------------------------------------
 template <typename T>
 static int ffn_fwd_t(const fomoe_config& c, int n_res, const T* x, const RouteWs& rws, const ActWs& aws, const ScratchWs& sws,
-                     const FfnPtrs& w, cudaStream_t st) {
+                     const FfnPtrs& w_in, cudaStream_t st) {
   const int d = c.d_model, F = c.d_ff;
+  FfnPtrs w = w_in;
+  if (c.expert_fn == FOMOE_EXPERT_SILU) w.w_gate = w.sh_gate = nullptr;   // whatever was passed is ignored (fomoe.h)
   if (n_res > 0 && c.T > 0) {
     RowSpace rs{rws.n_mtiles, rws.tile_slot, 0};
     dim3 g1(rws.R_cap / kBM, ceil_div(F, kBN));
@@ -287,15 +295,18 @@ int simt_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs&
 
 template <typename T>
 static int ffn_bwd_t(const fomoe_config& c, int n_res, const T* x, const T* dy, const RouteWs& rws, const ActWs& aws,
-                     const ScratchWs& sws, const FfnPtrs& w, T* dw_gate, T* dw_up, T* dw_down, T* d_sh_gate, T* d_sh_up,
+                     const ScratchWs& sws, const FfnPtrs& w_in, T* dw_gate, T* dw_up, T* dw_down, T* d_sh_gate, T* d_sh_up,
                      T* d_sh_down, cudaStream_t st) {
   const int d = c.d_model, F = c.d_ff;
+  const bool silu = c.expert_fn == FOMOE_EXPERT_SILU;   // two-matrix expert: no gate path, dW_up = dA^T x
+  FfnPtrs w = w_in;
+  if (silu) w.w_gate = w.sh_gate = nullptr;
   if (n_res > 0) {
     RowSpace rs{rws.n_mtiles, rws.tile_slot, 0};
     if (c.T > 0) {
       dim3 g1(rws.R_cap / kBM, ceil_div(F, kBN));
       simt_dh_kernel<T><<<g1, kGemmThreads, 0, st>>>(rs, (const T*)sws.dop, d, F, (const T*)w.w_down, F, (const T*)aws.a,
-                                                     (const T*)aws.u, (T*)sws.da, (T*)sws.du);
+                                                     silu ? nullptr : (const T*)aws.u, (T*)sws.da, (T*)sws.du);
       FOMOE_LAUNCH_OK("simt_dh_kernel");
       dim3 g2(rws.R_cap / kBM, ceil_div(d, kBN));
       simt_dx_kernel<T><<<g2, kGemmThreads, 0, st>>>(rs, (const T*)sws.da, (const T*)sws.du, F, d, F, 1, (const T*)w.w_gate,
@@ -308,10 +319,12 @@ static int ffn_bwd_t(const fomoe_config& c, int n_res, const T* x, const T* dy, 
                                                             dw_down);
     FOMOE_LAUNCH_OK("simt_wgrad_kernel(down)");
     dim3 gg(ceil_div(F, kBM), ceil_div(d, kBN), n_res);
-    simt_wgrad_kernel<T, T, T><<<gg, kGemmThreads, 0, st>>>(rws.pad_offsets, 0, 0, (const T*)sws.da, F, 0, (const T*)aws.xp, d, 0, F, d,
-                                                            dw_gate);
-    FOMOE_LAUNCH_OK("simt_wgrad_kernel(gate)");
-    simt_wgrad_kernel<T, T, T><<<gg, kGemmThreads, 0, st>>>(rws.pad_offsets, 0, 0, (const T*)sws.du, F, 0, (const T*)aws.xp, d, 0, F, d,
+    if (!silu) {
+      simt_wgrad_kernel<T, T, T><<<gg, kGemmThreads, 0, st>>>(rws.pad_offsets, 0, 0, (const T*)sws.da, F, 0, (const T*)aws.xp, d, 0, F, d,
+                                                              dw_gate);
+      FOMOE_LAUNCH_OK("simt_wgrad_kernel(gate)");
+    }
+    simt_wgrad_kernel<T, T, T><<<gg, kGemmThreads, 0, st>>>(rws.pad_offsets, 0, 0, (const T*)(silu ? sws.da : sws.du), F, 0, (const T*)aws.xp, d, 0, F, d,
                                                             dw_up);
     FOMOE_LAUNCH_OK("simt_wgrad_kernel(up)");
   }
@@ -320,7 +333,7 @@ static int ffn_bwd_t(const fomoe_config& c, int n_res, const T* x, const T* dy, 
     RowSpace rs{nullptr, nullptr, c.T};
     if (c.T > 0) {
       dim3 g1(ceil_div(c.T, kBM), ceil_div(Fs, kBN), c.n_shared);
-      simt_dh_kernel<T><<<g1, kGemmThreads, 0, st>>>(rs, dy, d, Fs, (const T*)w.sh_down, ld, (const T*)aws.sa, (const T*)aws.su,
+      simt_dh_kernel<T><<<g1, kGemmThreads, 0, st>>>(rs, dy, d, Fs, (const T*)w.sh_down, ld, (const T*)aws.sa, silu ? nullptr : (const T*)aws.su,
                                                      (T*)sws.dsa, (T*)sws.dsu);
       FOMOE_LAUNCH_OK("simt_dh_kernel(shared)");
       dim3 g2(ceil_div(c.T, kBM), ceil_div(d, kBN), 1);
@@ -333,9 +346,11 @@ static int ffn_bwd_t(const fomoe_config& c, int n_res, const T* x, const T* dy, 
     simt_wgrad_kernel<T, T, T><<<gd, kGemmThreads, 0, st>>>(nullptr, c.T, 0, dy, d, 0, (const T*)aws.sh, ld, Fs, d, Fs, d_sh_down);
     FOMOE_LAUNCH_OK("simt_wgrad_kernel(sh_down)");
     dim3 gg(ceil_div(Fs, kBM), ceil_div(d, kBN), c.n_shared);
-    simt_wgrad_kernel<T, T, T><<<gg, kGemmThreads, 0, st>>>(nullptr, c.T, 0, (const T*)sws.dsa, ld, Fs, x, d, 0, Fs, d, d_sh_gate);
-    FOMOE_LAUNCH_OK("simt_wgrad_kernel(sh_gate)");
-    simt_wgrad_kernel<T, T, T><<<gg, kGemmThreads, 0, st>>>(nullptr, c.T, 0, (const T*)sws.dsu, ld, Fs, x, d, 0, Fs, d, d_sh_up);
+    if (!silu) {
+      simt_wgrad_kernel<T, T, T><<<gg, kGemmThreads, 0, st>>>(nullptr, c.T, 0, (const T*)sws.dsa, ld, Fs, x, d, 0, Fs, d, d_sh_gate);
+      FOMOE_LAUNCH_OK("simt_wgrad_kernel(sh_gate)");
+    }
+    simt_wgrad_kernel<T, T, T><<<gg, kGemmThreads, 0, st>>>(nullptr, c.T, 0, (const T*)(silu ? sws.dsa : sws.dsu), ld, Fs, x, d, 0, Fs, d, d_sh_up);
     FOMOE_LAUNCH_OK("simt_wgrad_kernel(sh_up)");
   }
   return FOMOE_OK;

@@ -18,6 +18,8 @@
 //   FWD1  [a|u] = X W_gate^T | X W_up^T   (A, B K-major; CTA0 stages W_gate, CTA1 W_up; epilogue: h = silu(a)*u, and
 //                                           for the backward silu'(a)*u and silu(a) in place of a and u)
 //   FWD2  o = H W_down^T                  (A, B K-major)
+//   FWD1S a = X W_up^T                    (the paper's two-matrix expert: epilogue h = silu(a), and silu'(a) for
+//                                           the backward; loads like FWD2 with K = d)
 //   DH    dh = dO W_down                  (A K-major, B MN-major; epilogue: da = dh * silu'(a)u, du = dh * silu(a))
 //   DX    dxp = dA W_gate + dU W_up       (A K-major, B MN-major; two K segments into one accumulator)
 //   WGRAD dW[g] = A[rows(g)]^T B[rows(g)] (A, B MN-major; K = the group's (padded) rows)
@@ -41,11 +43,11 @@ constexpr int kEpiWarps = 8;    // two warps per TMEM lane quarter; they take al
 // row-per-thread TMEM layout into coalesced 16-byte global accesses
 constexpr int kStgTile = 2048;
 constexpr int kDhDepth = 3;  // DH epilogue: chunks of (a, u) kept in flight per warp with cp.async
-enum Mode { FWD1 = 0, FWD2 = 1, DH = 2, DX = 3, WGRAD = 4, ROUTE = 5 };
+enum Mode { FWD1 = 0, FWD2 = 1, DH = 2, DX = 3, WGRAD = 4, ROUTE = 5, FWD1S = 6 };
 constexpr int kRouteStg = 16384;  // ROUTE epilogue scratch: slot map, per-stage histograms, top-k merge lists
 // DH and FWD1 trade TMA stages for epilogue staging: DH streams a and u back in through a cp.async ring
-__host__ __device__ constexpr int stages_of(int mode) { return mode == DH ? 4 : mode == FWD1 ? 5 : 6; }
-__host__ __device__ constexpr int stg_tiles_per_warp(int mode) { return mode == DH ? 2 * kDhDepth : mode == FWD1 ? 3 : 1; }
+__host__ __device__ constexpr int stages_of(int mode) { return mode == DH ? 4 : (mode == FWD1 || mode == FWD1S) ? 5 : 6; }
+__host__ __device__ constexpr int stg_tiles_per_warp(int mode) { return mode == DH ? 2 * kDhDepth : mode == FWD1 ? 3 : mode == FWD1S ? 2 : 1; }
 __host__ __device__ constexpr int stg_bytes_of(int mode) { return mode == ROUTE ? kRouteStg : kEpiWarps * stg_tiles_per_warp(mode) * kStgTile; }
 __host__ __device__ constexpr int smem_bytes_of(int mode) {
   return stages_of(mode) * kStageBytes + stg_bytes_of(mode) + 1024 /*align*/ + 256 /*barriers*/;
@@ -81,6 +83,7 @@ struct UmmaParams {
   int ld;                      // leading dimension of the [rows, hidden] activations (F, or parts*F for dense)
   int M, N;                    // WGRAD: output rows / cols per group
   int a_gcol, b_gcol;          // WGRAD dense: per-group column offset into A / B
+  int ksegs;                   // DX: K segments (2: dA W_gate + dU W_up; 1: dA W_up, two-matrix expert)
   int k_chunk;                 // WGRAD dense: > 0 = split-K, group g reduces rows [g*k_chunk, (g+1)*k_chunk)
   float* out_f32;              // WGRAD: if set, fp32 output [n_groups, M, N] instead of out0
   bf16 *out0, *out1, *out2;    // FWD1: a,u,h | FWD2/DX: out | DH: da,du | WGRAD: dW
@@ -173,10 +176,10 @@ struct Sched {
       total = (long)p.n_groups * m_pairs * n_tiles_n;
     } else {
       m_pairs = dense ? (p.dense_rows + 2 * BM - 1) / (2 * BM) : p.n_mtiles[2];
-      const int n_extent = (MODE == FWD1 || MODE == DH) ? p.F : p.d;
+      const int n_extent = (MODE == FWD1 || MODE == FWD1S || MODE == DH) ? p.F : p.d;
       const int bn = MODE == FWD1 ? BN / 2 : BN;
       n_tiles_n = MODE == ROUTE ? 1 : (n_extent + bn - 1) / bn;
-      ntn_total = n_tiles_n * ((dense && (MODE == FWD1 || MODE == DH)) ? p.parts : 1);
+      ntn_total = n_tiles_n * ((dense && (MODE == FWD1 || MODE == FWD1S || MODE == DH)) ? p.parts : 1);
       total = (long)m_pairs * ntn_total;
     }
   }
@@ -219,11 +222,11 @@ struct Sched {
       t.group = 0;
       t.k_row0 = 0;
       const int kparts = dense ? p.parts : 1;
-      const int n_extent = (MODE == DH) ? p.F : p.d;
+      const int n_extent = (MODE == DH || MODE == FWD1S) ? p.F : p.d;
       t.n_mma = MODE == ROUTE ? p.N : (MODE != FWD1 && n_extent - t.n_tile * BN <= BN / 2) ? BN / 2 : BN;
-      if (MODE == FWD1 || MODE == DH || MODE == ROUTE) t.num_kb = p.d / BK;
+      if (MODE == FWD1 || MODE == FWD1S || MODE == DH || MODE == ROUTE) t.num_kb = p.d / BK;
       else if (MODE == FWD2) t.num_kb = kparts * (p.F / BK);
-      else t.num_kb = 2 * kparts * (p.F / BK);  // DX
+      else t.num_kb = p.ksegs * kparts * (p.F / BK);  // DX
     }
     return t;
   }
@@ -483,6 +486,9 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
             if (t.live) tma_load_2d_2sm(sa, &maps.m[0], fb, kb * BK, m0);
             // N columns [0,128) = a (W_gate rows, staged by CTA 0), [128,256) = u (W_up rows, CTA 1)
             tma_load_2d_2sm(sb, &maps.m[1 + rank], fb, kb * BK, t.slot * p.F + t.n_tile * (BN / 2));
+          } else if (MODE == FWD1S) {   // B = W_up rows [slot F + n_tile BN + rank nh, ..), K-major
+            if (t.live) tma_load_2d_2sm(sa, &maps.m[0], fb, kb * BK, m0);
+            tma_load_2d_2sm(sb, &maps.m[1], fb, kb * BK, t.slot * p.F + t.n_tile * BN + rank * nh);
           } else if (MODE == FWD2) {
             const int kpp = p.F / BK, part = kb / kpp, kk = kb % kpp;
             if (t.live) tma_load_2d_2sm(sa, &maps.m[0], fb, part * p.F + kk * BK, m0);
@@ -612,7 +618,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
               const bool ok = r < prows;
               const size_t g = off + (size_t)(ok ? r : 0) * p.ld + c * 8;
               cp_async16(sa + stg_off(r, c), p.in0 + g, ok);
-              cp_async16(su + stg_off(r, c), p.in1 + g, ok);
+              if (p.in1) cp_async16(su + stg_off(r, c), p.in1 + g, ok);   // in1 == nullptr: two-matrix expert, da only
             }
           }
           pcc += 2;
@@ -651,7 +657,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
 #pragma unroll
             for (int g8 = 0; g8 < 4; ++g8) {
               const uint32_t o = stg_off(lane, g8);
-              uint4 wa = lds128(sa + o), wu = lds128(su + o);
+              uint4 wa = lds128(sa + o), wu = p.in1 ? lds128(su + o) : make_uint4(0u, 0u, 0u, 0u);
               uint32_t* pa = reinterpret_cast<uint32_t*>(&wa);
               uint32_t* pu = reinterpret_cast<uint32_t*>(&wu);
 #pragma unroll
@@ -662,11 +668,11 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
                 pu[i] = pack_bf16x2(d0 * u2.x, d1 * u2.y);
               }
               sts128(sa + o, wa);   // da over a, du over u: every lane rewrites exactly the bytes it read
-              sts128(su + o, wu);
+              if (p.in1) sts128(su + o, wu);
             }
             __syncwarp();
             stg_to_global(sa, p.out0 + base + n, p.ld, lane, rows_valid);
-            stg_to_global(su, p.out1 + base + n, p.ld, lane, rows_valid);
+            if (p.in1) stg_to_global(su, p.out1 + base + n, p.ld, lane, rows_valid);
           }
           __syncwarp();
           issue(slot);                                        // refill the slot just stored from
@@ -746,6 +752,28 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
             stg_to_global(stg2, p.out2 + base + n, p.ld, lane, rows_valid);
             __syncwarp();
           }
+        } else if (MODE == FWD1S) {   // two-matrix expert: h = silu(a); out0 <- silu'(a) (the backward's factor), out2 <- h
+          const size_t base = (size_t)row0 * p.ld + (size_t)t.part * p.F;
+#pragma unroll 1
+          for (int cc = half; cc < BN / 32 && rows_valid > 0; cc += 2) {
+            const int n = t.n_tile * BN + cc * 32;
+            if (n >= p.F) break;
+            float a[32], h[32];
+            tmem_ld32(taddr + cc * 32, a);
+            tmem_ld_wait();
+#pragma unroll
+            for (int i = 0; i < 32; ++i) {
+              const float sg = __fdividef(1.0f, 1.0f + __expf(-a[i]));
+              h[i] = a[i] * sg;                          // silu(a)
+              a[i] = fmaf(h[i], 1.0f - sg, sg);           // silu'(a) = s (1 + a (1 - s))
+            }
+            stg_put_row(stg0, lane, a);
+            stg_put_row(stg1, lane, h);
+            __syncwarp();
+            stg_to_global(stg0, p.out0 + base + n, p.ld, lane, rows_valid);
+            stg_to_global(stg1, p.out2 + base + n, p.ld, lane, rows_valid);
+            __syncwarp();
+          }
         } else {  // FWD2, DX: plain store of a [rows, d] tile
 #pragma unroll 1
           for (int cc = half; cc < BN / 32 && rows_valid > 0; cc += 2) {
@@ -822,11 +850,21 @@ int umma_route(const fomoe_config& c, const void* x, const void* wr_split, int N
 int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs& rws, const ActWs& aws, const ScratchWs& sws,
                  const FfnPtrs& w, cudaStream_t st) {
   const int d = c.d_model, F = c.d_ff;
+  const bool silu = c.expert_fn == FOMOE_EXPERT_SILU;
   if (n_res > 0 && c.T > 0) {
     const uint64_t R = (uint64_t)rws.R_cap;
     UmmaParams p{};
     p.n_mtiles = rws.n_mtiles; p.tile_slot = rws.tile_slot; p.pair_info = rws.pair_info; p.parts = 1; p.d = d; p.F = F; p.ld = F;
-    {
+    if (silu) {   // two-matrix expert: a = X W_up^T, h = silu(a)
+      TmaMaps m{};
+      MAP_OK(make_map(&m.m[0], aws.xp, d, R, d, 128));
+      MAP_OK(make_map(&m.m[1], w.w_up, d, (uint64_t)n_res * F, d, 128));
+      m.m[2] = m.m[3] = m.m[0];
+      UmmaParams q = p;
+      q.out0 = (bf16*)aws.a; q.out2 = (bf16*)aws.h;
+      int rc = launch<FWD1S>(m, q, st, "umma_grouped_kernel<FWD1S>");
+      if (rc != FOMOE_OK) return rc;
+    } else {
       TmaMaps m{};
       MAP_OK(make_map(&m.m[0], aws.xp, d, R, d, 128));
       MAP_OK(make_map(&m.m[1], w.w_gate, d, (uint64_t)n_res * F, d, 128));
@@ -852,7 +890,16 @@ int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs&
     const int Fs = c.d_ff_shared, ns = c.n_shared, ld = ns * Fs;
     UmmaParams p{};
     p.dense_rows = c.T; p.parts = ns; p.d = d; p.F = Fs; p.ld = ld;
-    {
+    if (silu) {
+      TmaMaps m{};
+      MAP_OK(make_map(&m.m[0], x, d, c.T, d, 128));
+      MAP_OK(make_map(&m.m[1], w.sh_up, d, (uint64_t)ns * Fs, d, 128));
+      m.m[2] = m.m[3] = m.m[0];
+      UmmaParams q = p;
+      q.out0 = (bf16*)aws.sa; q.out2 = (bf16*)aws.sh;
+      int rc = launch<FWD1S>(m, q, st, "umma_grouped_kernel<FWD1S,shared>");
+      if (rc != FOMOE_OK) return rc;
+    } else {
       TmaMaps m{};
       MAP_OK(make_map(&m.m[0], x, d, c.T, d, 128));
       MAP_OK(make_map(&m.m[1], w.sh_gate, d, (uint64_t)ns * Fs, d, 128));
@@ -881,6 +928,7 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
                  const ScratchWs& sws, const FfnPtrs& w, void* dw_gate, void* dw_up, void* dw_down, void* d_sh_gate,
                  void* d_sh_up, void* d_sh_down, cudaStream_t st) {
   const int d = c.d_model, F = c.d_ff;
+  const bool silu = c.expert_fn == FOMOE_EXPERT_SILU;   // two-matrix expert: one saved factor, dxp = dA W_up, dW_up = dA^T x
   if (n_res > 0) {
     const uint64_t R = (uint64_t)rws.R_cap;
     UmmaParams p{};
@@ -892,17 +940,18 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
         MAP_OK(make_map(&m.m[1], w.w_down, F, (uint64_t)n_res * d, F, 64));
         m.m[2] = m.m[3] = m.m[0];
         UmmaParams q = p;
-        q.in0 = (const bf16*)aws.a; q.in1 = (const bf16*)aws.u; q.out0 = (bf16*)sws.da; q.out1 = (bf16*)sws.du;
+        q.in0 = (const bf16*)aws.a; q.in1 = silu ? nullptr : (const bf16*)aws.u; q.out0 = (bf16*)sws.da; q.out1 = (bf16*)sws.du;
         int rc = launch<DH>(m, q, st, "umma_grouped_kernel<DH>");
         if (rc != FOMOE_OK) return rc;
       }
       {  // dxp = dA W_gate + dU W_up
         TmaMaps m{};
         MAP_OK(make_map(&m.m[0], sws.da, F, R, F, 128));
-        MAP_OK(make_map(&m.m[1], sws.du, F, R, F, 128));
-        MAP_OK(make_map(&m.m[2], w.w_gate, d, (uint64_t)n_res * F, d, 64));
+        MAP_OK(make_map(&m.m[1], silu ? sws.da : sws.du, F, R, F, 128));
+        MAP_OK(make_map(&m.m[2], silu ? w.w_up : w.w_gate, d, (uint64_t)n_res * F, d, 64));
         MAP_OK(make_map(&m.m[3], w.w_up, d, (uint64_t)n_res * F, d, 64));
         UmmaParams q = p;
+        q.ksegs = silu ? 1 : 2;
         q.out0 = (bf16*)sws.dxp;
         int rc = launch<DX>(m, q, st, "umma_grouped_kernel<DX>");
         if (rc != FOMOE_OK) return rc;
@@ -910,8 +959,10 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
     }
     // weight gradients, K = the slot's padded rows (padding rows are zero)
     struct WG { const void* A; int lda; const void* B; int ldb; int M, N; void* out; };
-    const WG jobs[3] = {{sws.dop, d, aws.h, F, d, F, dw_down}, {sws.da, F, aws.xp, d, F, d, dw_gate}, {sws.du, F, aws.xp, d, F, d, dw_up}};
-    for (const WG& j : jobs) {
+    const WG jobs[3] = {{sws.dop, d, aws.h, F, d, F, dw_down}, {sws.da, F, aws.xp, d, F, d, silu ? dw_up : dw_gate},
+                        {sws.du, F, aws.xp, d, F, d, dw_up}};
+    for (int ji = 0; ji < (silu ? 2 : 3); ++ji) {
+      const WG& j = jobs[ji];
       TmaMaps m{};
       MAP_OK(make_map(&m.m[0], j.A, j.lda, R, j.lda, 64));
       MAP_OK(make_map(&m.m[1], j.B, j.ldb, R, j.ldb, 64));
@@ -924,7 +975,7 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
   }
   if (c.n_shared > 0 && c.T == 0) {  // empty batch: exact zeros
     const size_t n = sizeof(bf16) * (size_t)c.n_shared * c.d_ff_shared * d;
-    FOMOE_CUDA_OK(cudaMemsetAsync(d_sh_gate, 0, n, st));
+    if (!silu) FOMOE_CUDA_OK(cudaMemsetAsync(d_sh_gate, 0, n, st));
     FOMOE_CUDA_OK(cudaMemsetAsync(d_sh_up, 0, n, st));
     FOMOE_CUDA_OK(cudaMemsetAsync(d_sh_down, 0, n, st));
   } else if (c.n_shared > 0) {
@@ -938,17 +989,18 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
         MAP_OK(make_map(&m.m[1], w.sh_down, Fs, (uint64_t)ns * d, Fs, 64));
         m.m[2] = m.m[3] = m.m[0];
         UmmaParams q = p;
-        q.in0 = (const bf16*)aws.sa; q.in1 = (const bf16*)aws.su; q.out0 = (bf16*)sws.dsa; q.out1 = (bf16*)sws.dsu;
+        q.in0 = (const bf16*)aws.sa; q.in1 = silu ? nullptr : (const bf16*)aws.su; q.out0 = (bf16*)sws.dsa; q.out1 = (bf16*)sws.dsu;
         int rc = launch<DH>(m, q, st, "umma_grouped_kernel<DH,shared>");
         if (rc != FOMOE_OK) return rc;
       }
       {
         TmaMaps m{};
         MAP_OK(make_map(&m.m[0], sws.dsa, ld, c.T, ld, 128));
-        MAP_OK(make_map(&m.m[1], sws.dsu, ld, c.T, ld, 128));
-        MAP_OK(make_map(&m.m[2], w.sh_gate, d, (uint64_t)ns * Fs, d, 64));
+        MAP_OK(make_map(&m.m[1], silu ? sws.dsa : sws.dsu, ld, c.T, ld, 128));
+        MAP_OK(make_map(&m.m[2], silu ? w.sh_up : w.sh_gate, d, (uint64_t)ns * Fs, d, 64));
         MAP_OK(make_map(&m.m[3], w.sh_up, d, (uint64_t)ns * Fs, d, 64));
         UmmaParams q = p;
+        q.ksegs = silu ? 1 : 2;
         q.out0 = (bf16*)sws.dx_sh;
         int rc = launch<DX>(m, q, st, "umma_grouped_kernel<DX,shared>");
         if (rc != FOMOE_OK) return rc;
@@ -956,9 +1008,10 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
     }
     struct WG { const void* A; int lda; int a_gcol; const void* B; int ldb; int b_gcol; int M, N; void* out; };
     const WG jobs[3] = {{dy, d, 0, aws.sh, ld, Fs, d, Fs, d_sh_down},
-                        {sws.dsa, ld, Fs, x, d, 0, Fs, d, d_sh_gate},
+                        {sws.dsa, ld, Fs, x, d, 0, Fs, d, silu ? d_sh_up : d_sh_gate},
                         {sws.dsu, ld, Fs, x, d, 0, Fs, d, d_sh_up}};
-    for (const WG& j : jobs) {
+    for (int ji = 0; ji < (silu ? 2 : 3); ++ji) {
+      const WG& j = jobs[ji];
       TmaMaps m{};
       MAP_OK(make_map(&m.m[0], j.A, j.lda, c.T, j.lda, 64));
       MAP_OK(make_map(&m.m[1], j.B, j.ldb, c.T, j.ldb, 64));

@@ -31,7 +31,7 @@ class SkipTokenMoE:
         self.n_res = int(len(resident))
         self.tdtype = torch.bfloat16 if w.dtype == "bf16" else torch.float32
         self.cfg = B.make_config(w.T, w.d, w.E, w.k, w.F, w.n_sh, w.F_sh, B.FOMOE_BF16 if w.dtype == "bf16" else B.FOMOE_F32,
-                                 w.gate_fn, w.gate_rule, w.temperature)
+                                 w.gate_fn, w.gate_rule, w.temperature, w.expert_fn)
         dv, td = self.device, self.tdtype
         self.resident = _dev(np.asarray(resident, np.int32), torch.int32, dv) if self.n_res else torch.empty(0, dtype=torch.int32, device=dv)
         self.w_router = _dev(w_router, torch.float32, dv)
@@ -45,8 +45,9 @@ class SkipTokenMoE:
         self.y = torch.empty((w.T, w.d), dtype=td, device=dv)
         self.dx = torch.empty((w.T, w.d), dtype=td, device=dv)
         self.dw_router = torch.empty((w.d, w.E), dtype=torch.float32, device=dv)
-        self.dw_gate, self.dw_up, self.dw_down = (torch.empty_like(t) for t in (self.w_gate, self.w_up, self.w_down))
-        self.d_shared = None if self.shared is None else tuple(torch.empty_like(t) for t in self.shared)
+        # (the paper's two-matrix expert has no W_gate: w_gate / shared[0] are None then, and so are their gradients)
+        self.dw_gate, self.dw_up, self.dw_down = (None if t is None else torch.empty_like(t) for t in (self.w_gate, self.w_up, self.w_down))
+        self.d_shared = None if self.shared is None else tuple(None if t is None else torch.empty_like(t) for t in self.shared)
         self.launches = 0
 
     def to_dev(self, a: np.ndarray) -> torch.Tensor:

@@ -49,6 +49,7 @@ class MoEWorkload:
     gate_fn: int = GATE_SOFTMAX       # BASELINE.json: softmax; paper Eq. 17: sigmoid
     gate_rule: int = RULE_DROP_ONLY   # paper: drop-only
     temperature: float = 1.0
+    expert_fn: int = 0                # 0 = SwiGLU (BASELINE.json), 1 = the paper's W_down silu(W_up x)
     seed: int = 0
     fixed_resident: Optional[tuple] = None
 
@@ -65,6 +66,16 @@ CONFIGS = {
     "C5": MoEWorkload("C5", T=32768, d=4096, E=128, k=8, F=1536, n_res=32),
 }
 C4_RESIDENT_SWEEP = (8, 16, 32, 64)
+EXPERT_SWIGLU, EXPERT_SILU = 0, 1
+# The paper's own sigma-MoE layer at its Table 1 shapes: sigmoid gate (Eq. 17), two-matrix SiLU expert of
+# width d_expert = 128 (Eq. 16, §B.3.1), N_active of N_experts, sequence length 2048 x 8 sequences;
+# half of the experts resident (overlap O_e / M = 1/2).  P0 is a small fp32 case for element-wise parity.
+CONFIGS.update({
+    "P0": MoEWorkload("P0", T=256, d=64, E=8, k=2, F=32, n_res=4, dtype="f32", gate_fn=GATE_SIGMOID, expert_fn=EXPERT_SILU),
+    "P1": MoEWorkload("P1", T=16384, d=512, E=16, k=4, F=128, n_res=8, gate_fn=GATE_SIGMOID, expert_fn=EXPERT_SILU),    # Medium (150M)
+    "P2": MoEWorkload("P2", T=16384, d=1024, E=32, k=8, F=128, n_res=16, gate_fn=GATE_SIGMOID, expert_fn=EXPERT_SILU),  # Large (2B)
+    "P3": MoEWorkload("P3", T=16384, d=2048, E=64, k=16, F=128, n_res=32, gate_fn=GATE_SIGMOID, expert_fn=EXPERT_SILU), # XL (13B)
+})
 
 
 def config(name: str) -> MoEWorkload:
@@ -150,11 +161,14 @@ def make_resident_experts(w: MoEWorkload, resident: np.ndarray):
     """Resident-compact stacks W_gate [n_res,F,d], W_up [n_res,F,d], W_down [n_res,d,F]; slot i <-> resident[i]
     (stored only for resident experts: the memory saving is the point)."""
     n = len(resident)
-    wg = np.empty((n, w.F, w.d), dtype=np.float32)
+    silu = w.expert_fn == EXPERT_SILU   # the paper's expert has no W_gate (PAPER.md:589, 253): None in its place
+    wg = None if silu else np.empty((n, w.F, w.d), dtype=np.float32)
     wu = np.empty((n, w.F, w.d), dtype=np.float32)
     wd = np.empty((n, w.d, w.F), dtype=np.float32)
     for i, e in enumerate(resident):
-        wg[i], wu[i], wd[i] = make_expert(w, int(e))
+        g, wu[i], wd[i] = make_expert(w, int(e))
+        if not silu:
+            wg[i] = g
     return wg, wu, wd
 
 
@@ -162,7 +176,7 @@ def make_shared_experts(w: MoEWorkload):
     """Shared (always-resident, dense) experts (PAPER.md:86): [n_sh,F_sh,d], [n_sh,F_sh,d], [n_sh,d,F_sh]; None if n_sh=0."""
     if w.n_sh == 0:
         return None
-    sg = np.stack([_store(w, _normal(_rng(w, "sh_gate", s), (w.F_sh, w.d), 0.02)) for s in range(w.n_sh)])
+    sg = None if w.expert_fn == EXPERT_SILU else np.stack([_store(w, _normal(_rng(w, "sh_gate", s), (w.F_sh, w.d), 0.02)) for s in range(w.n_sh)])
     su = np.stack([_store(w, _normal(_rng(w, "sh_up", s), (w.F_sh, w.d), 0.02)) for s in range(w.n_sh)])
     sd = np.stack([_store(w, _normal(_rng(w, "sh_down", s), (w.d, w.F_sh), 0.02)) for s in range(w.n_sh)])
     return sg, su, sd

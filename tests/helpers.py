@@ -47,10 +47,11 @@ def margin_clean(p: Problem, oracle64, max_attempts=20) -> int:
 def oracle_all(p: Problem, o, bwd=True):
     w = p.w
     r = o.route(p.x, p.w_router, p.resident, w.k, w.gate_fn, w.gate_rule, w.temperature, p.bias)
-    y = o.moe_fwd(p.x, r, p.resident, p.wg, p.wu, p.wd, p.shared)
+    y = o.moe_fwd(p.x, r, p.resident, p.wg, p.wu, p.wd, p.shared, expert_fn=w.expert_fn)
     b = None
     if bwd:
-        b = o.moe_bwd(p.x, p.dy, p.w_router, r, p.resident, p.wg, p.wu, p.wd, p.shared, w.gate_fn, w.gate_rule, w.temperature)
+        b = o.moe_bwd(p.x, p.dy, p.w_router, r, p.resident, p.wg, p.wu, p.wd, p.shared, w.gate_fn, w.gate_rule, w.temperature,
+                      expert_fn=w.expert_fn)
     return r, y, b
 
 
