@@ -385,6 +385,30 @@ def run_gpu(args, w, n_res):
                                  "ideal_flop_ratio": (w.k * fl_pair * w.d * w.F * w.T + fl_pair * w.T * w.n_sh * w.d * w.F_sh) / flops_step}
             del full
 
+        # ---- Fig. 11 analogue: step time against the number of ghost (non-resident) experts ----
+        if args.ghost_sweep:
+            try:
+                del layer
+            except NameError:
+                pass
+            torch.cuda.empty_cache()
+            sweep = []
+            base_ms = None
+            for nr in sorted({w.E, (3 * w.E) // 4, w.E // 2, w.E // 4, w.E // 8}, reverse=True):
+                if nr < 1:
+                    continue
+                lay = build_layer(nr)
+                lay.step(x, dy)
+                st = lay.capture_step(x, dy)
+                t_ms = timed_steps(st, args.steps, args.warmup)
+                m = sum(t_ms) / len(t_ms)
+                base_ms = m if base_ms is None else base_ms
+                sweep.append({"n_res": nr, "ghost_experts": w.E - nr, "ms_per_step": m, "kept_pairs": lay.routing_numpy()["P"],
+                              "speedup_vs_all_resident": base_ms / m})
+                del lay, st
+                torch.cuda.empty_cache()
+            out["ghost_sweep"] = sweep
+
         # ---- the oracle, as it stands, on the host cores (reported baseline, not the target) ----
         if not args.no_cpu_baseline:
             sample = min(w.T, args.ref_tokens)
@@ -409,6 +433,7 @@ def main():
     ap.add_argument("--ref-tokens", type=int, default=1024, help="tokens per step of the CPU oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-all-resident", action="store_true")
+    ap.add_argument("--ghost-sweep", action="store_true", help="also time the step for n_res = E, 3E/4, E/2, E/4, E/8 (Fig. 11 analogue)")
     ap.add_argument("--no-graph", action="store_true", help="launch kernels eagerly instead of replaying a CUDA graph")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

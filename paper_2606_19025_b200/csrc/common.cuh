@@ -194,7 +194,7 @@ inline ScratchWs carve_scratch_ws(const fomoe_config& c, int R_cap, void* base) 
 // ---- launchers implemented in the other translation units (all enqueue on `st`, return FOMOE_* status) ----
 int launch_route(const fomoe_config& c, const void* x, const float* w_router, const float* bias,
                  const int32_t* resident_ids, int n_res, const fomoe_route_state& out, const RouteWs& ws, cudaStream_t st);
-// tensor-core router (route_umma.cu): bf16 tokens, d % 64 == 0, E <= 128, k <= 8
+// tensor-core router (route_umma.cu + ROUTE mode of umma_gemm.cu): bf16 tokens, d % 64 == 0, E <= 128, k <= 32
 bool route_umma_supported(const fomoe_config& c);
 int launch_route_umma(const fomoe_config& c, const void* x, const float* w_router, const float* bias, const int32_t* resident_ids,
                       int n_res, const fomoe_route_state& out, const RouteWs& ws, cudaStream_t st);

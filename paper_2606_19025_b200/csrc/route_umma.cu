@@ -52,7 +52,7 @@ __global__ void route_prep_kernel(const int32_t* __restrict__ resident_ids, int 
 }  // namespace
 
 bool route_umma_supported(const fomoe_config& c) {
-  return c.dtype == FOMOE_BF16 && c.d_model % 64 == 0 && c.E <= 128 && c.top_k <= 8 && c.T > 0;
+  return c.dtype == FOMOE_BF16 && c.d_model % 64 == 0 && c.E <= 128 && c.top_k <= kMaxK && c.T > 0;
 }
 
 // x [T,d] bf16.  Writes slot_of, probs, topk_idx, gate and blk_hist (one row per 128-token block).

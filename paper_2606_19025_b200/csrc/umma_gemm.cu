@@ -44,9 +44,9 @@ constexpr int kEpiWarps = 8;    // two warps per TMEM lane quarter; they take al
 constexpr int kStgTile = 2048;
 constexpr int kDhDepth = 3;  // DH epilogue: chunks of (a, u) kept in flight per warp with cp.async
 enum Mode { FWD1 = 0, FWD2 = 1, DH = 2, DX = 3, WGRAD = 4, ROUTE = 5, FWD1S = 6 };
-constexpr int kRouteStg = 16384;  // ROUTE epilogue scratch: slot map, per-stage histograms, top-k merge lists
+constexpr int kRouteStg = 40960;  // ROUTE epilogue scratch: slot map, per-stage histograms, top-k merge lists (k <= 32)
 // DH and FWD1 trade TMA stages for epilogue staging: DH streams a and u back in through a cp.async ring
-__host__ __device__ constexpr int stages_of(int mode) { return mode == DH ? 4 : (mode == FWD1 || mode == FWD1S) ? 5 : 6; }
+__host__ __device__ constexpr int stages_of(int mode) { return mode == DH ? 4 : (mode == FWD1 || mode == FWD1S || mode == ROUTE) ? 5 : 6; }
 __host__ __device__ constexpr int stg_tiles_per_warp(int mode) { return mode == DH ? 2 * kDhDepth : mode == FWD1 ? 3 : mode == FWD1S ? 2 : 1; }
 __host__ __device__ constexpr int stg_bytes_of(int mode) { return mode == ROUTE ? kRouteStg : kEpiWarps * stg_tiles_per_warp(mode) * kStgTile; }
 __host__ __device__ constexpr int smem_bytes_of(int mode) {
@@ -252,8 +252,8 @@ __device__ __forceinline__ void bar_sync_named(int id, int threads) { asm volati
 struct RouteSmem {            // lives in the kernel's staging area (kRouteStg bytes)
   int32_t slot[128];          // resident slot of expert e, -1 = ghost
   int32_t hist[kAccStages][128];
-  float lv[8][128];           // half 1 -> half 0: top-k values / ids of row r
-  int32_t li[8][128];
+  float lv[kMaxK][128];       // half 1 -> half 0: top-k values / ids of row r
+  int32_t li[kMaxK][128];
   float mx[2][128];           // partial max of each half
   float sum[2][128];          // partial softmax denominators
 };
@@ -422,7 +422,7 @@ __device__ __forceinline__ void route_tile_epilogue(const UmmaParams& p, RouteSm
 // ---------------------------------------------------------------------------------------------------------
 // the kernel
 // ---------------------------------------------------------------------------------------------------------
-template <int MODE, int KMAX = 0>   // KMAX: ROUTE only, capacity of the top-k list (2, 4 or 8)
+template <int MODE, int KMAX = 0>   // KMAX: ROUTE only, capacity of the top-k list (2, 4, 8, 16 or 32)
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant__ UmmaParams p) {
   extern __shared__ uint8_t smem_raw[];
@@ -844,7 +844,9 @@ int umma_route(const fomoe_config& c, const void* x, const void* wr_split, int N
   m.m[2] = m.m[3] = m.m[0];
   if (c.top_k <= 2) return launch<ROUTE, 2>(m, p, st, "umma_grouped_kernel<ROUTE>");
   if (c.top_k <= 4) return launch<ROUTE, 4>(m, p, st, "umma_grouped_kernel<ROUTE>");
-  return launch<ROUTE, 8>(m, p, st, "umma_grouped_kernel<ROUTE>");
+  if (c.top_k <= 8) return launch<ROUTE, 8>(m, p, st, "umma_grouped_kernel<ROUTE>");
+  if (c.top_k <= 16) return launch<ROUTE, 16>(m, p, st, "umma_grouped_kernel<ROUTE>");   // Table 1: N_active up to 32
+  return launch<ROUTE, 32>(m, p, st, "umma_grouped_kernel<ROUTE>");
 }
 
 int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs& rws, const ActWs& aws, const ScratchWs& sws,

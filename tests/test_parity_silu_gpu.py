@@ -35,6 +35,15 @@ def test_small_bf16_wide_expert(oracle64):
     print("silu_wide", errs)
 
 
+@pytest.mark.parametrize("E,k,n_res", [(64, 16, 32), (128, 32, 48), (32, 8, 16)])
+def test_table1_active_counts(oracle64, E, k, n_res):
+    """N_active = 8, 16, 32 of N_experts = 32, 64, 128 (Table 1) on the tensor-core router: ordered top-k
+    lists, counts and the permutation bit-exact; outputs and gradients element by element."""
+    w = W.MoEWorkload("silu_k", T=700, d=192, E=E, k=k, F=128, n_res=n_res, gate_fn=W.GATE_SIGMOID, expert_fn=W.EXPERT_SILU, seed=6)
+    errs, _ = run_and_compare(H.Problem(w), oracle64)
+    print("silu_k", E, k, errs)
+
+
 def test_edge_cases_silu(oracle64):
     for kw in (dict(n_res=0, n_sh=1, F_sh=128), dict(n_res=16), dict(T=1, n_res=8), dict(T=127, n_res=3)):
         base = dict(T=300, d=128, E=16, k=4, F=128, n_res=8, gate_fn=W.GATE_SIGMOID, expert_fn=W.EXPERT_SILU, seed=5)
@@ -42,7 +51,7 @@ def test_edge_cases_silu(oracle64):
         run_and_compare(H.Problem(W.MoEWorkload("silu_edge", **base)), oracle64)
 
 
-@pytest.mark.parametrize("name", ["P1", "P2"])
+@pytest.mark.parametrize("name", ["P1", "P2", "P3"])
 def test_paper_shapes_sampled(oracle64, name):
     import torch
     w = W.config(name)
