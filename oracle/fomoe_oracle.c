@@ -55,6 +55,13 @@ enum { RULE_DROP_ONLY = 0, RULE_RENORM_TOPK = 1, RULE_RENORM_RESIDENT = 2 };
  * (§B.3.1); the expert payload "includes up and down projection".  In the SiLU form W_gate does
  * not exist (pointers may be NULL, dw_gate is not written). */
 enum { EXPERT_SWIGLU = 0, EXPERT_SILU = 1 };
+/* routing mode.  SKIP_TOKEN: the router is not partitioned, top-k over all E, ghost pairs dropped afterwards.
+ * FORCED_LOCAL: the paper's default outside §3.3.3 — the router is partitioned along with the experts "so that individual
+ * tokens are not routed to experts that are unavailable to the local worker", it "scores only N_le experts"
+ * (655-660 Eq. 19) and local routing is bounded by min(k, N_le): the caller passes
+ * k <= n_res.  Written out: the logits of non-resident experts do not exist (-inf here, probability 0), gate and top-k run
+ * over the resident ones, every selected pair is kept. */
+enum { ROUTE_SKIP_TOKEN = 0, ROUTE_FORCED_LOCAL = 1 };
 
 int oracle_real_bytes(void) { return (int)sizeof(REAL); }
 
@@ -85,12 +92,13 @@ static int* make_slot_of(int E, const int32_t* resident_ids, int n_res) {
  * gate g [T,k] (0 for skipped pairs); counts [n_res]; offsets [n_res+1]; row_token [T*k] (first P
  * valid, rest -1); pair_row [T,k] (row of the pair in slot-major order, or -1 if skipped).
  * ---------------------------------------------------------------------------------------------- */
-int oracle_route(int T, int d, int E, int k, int gate_fn, int gate_rule, double tau,
+int oracle_route(int T, int d, int E, int k, int gate_fn, int gate_rule, double tau, int route_mode,
                  const REAL* x, const REAL* w_r, const REAL* bias,
                  const int32_t* resident_ids, int n_res,
                  REAL* logits, REAL* probs, int32_t* topk_idx, REAL* gate,
                  int32_t* counts, int32_t* offsets, int32_t* row_token, int32_t* pair_row) {
   if (T < 0 || d <= 0 || E <= 0 || k <= 0 || k > E || n_res < 0 || n_res > E) return -1;
+  if (route_mode == ROUTE_FORCED_LOCAL && k > n_res) return -1; /* bounded by min(k, N_le) */
   int* slot_of = make_slot_of(E, resident_ids, n_res);
 
 #pragma omp parallel for schedule(static)
@@ -103,13 +111,14 @@ int oracle_route(int T, int d, int E, int k, int gate_fn, int gate_rule, double 
       REAL s = 0;
       for (int i = 0; i < d; ++i) s += xt[i] * w_r[(size_t)i * E + e];
       z[e] = s / (REAL)tau + (bias ? bias[e] : (REAL)0);
+      if (route_mode == ROUTE_FORCED_LOCAL && slot_of[e] < 0) z[e] = (REAL)-INFINITY; /* no router column for it */
     }
     /* 2. gate function (PAPER.md:517 sigmoid; BASELINE.json softmax, max-subtracted) */
     if (gate_fn == GATE_SIGMOID) {
       for (int e = 0; e < E; ++e) p[e] = sigmoid_(z[e]);
     } else {
-      REAL m = z[0], sum = 0;
-      for (int e = 1; e < E; ++e) m = z[e] > m ? z[e] : m;
+      REAL m = (REAL)-INFINITY, sum = 0;
+      for (int e = 0; e < E; ++e) m = z[e] > m ? z[e] : m;
       for (int e = 0; e < E; ++e) { p[e] = (REAL)exp((double)(z[e] - m)); sum += p[e]; }
       for (int e = 0; e < E; ++e) p[e] /= sum;
     }

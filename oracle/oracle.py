@@ -53,7 +53,8 @@ class Oracle:
         return None if a is None else np.ascontiguousarray(a, dtype=self.dt)
 
     # ---- steps 1-6 -------------------------------------------------------------------------------
-    def route(self, x, w_r, resident, k, gate_fn=0, gate_rule=0, tau=1.0, bias=None):
+    def route(self, x, w_r, resident, k, gate_fn=0, gate_rule=0, tau=1.0, bias=None, route_mode=0):
+        """route_mode 0 = skip-token (top-k over all E, ghosts dropped), 1 = forced-local (router over resident experts only)."""
         x, w_r, bias = self._r(x), self._r(w_r), self._r(bias)
         resident = np.ascontiguousarray(resident, dtype=np.int32)
         T, d = x.shape
@@ -65,7 +66,7 @@ class Oracle:
             counts=np.zeros(n_res, np.int32), offsets=np.zeros(n_res + 1, np.int32),
             row_token=np.empty(T * k, np.int32), pair_row=np.empty((T, k), np.int32))
         rc = self.lib.oracle_route(C.c_int(T), C.c_int(d), C.c_int(E), C.c_int(k), C.c_int(gate_fn), C.c_int(gate_rule),
-                                   C.c_double(tau), _ptr(x), _ptr(w_r), _ptr(bias), _ptr(resident), C.c_int(n_res),
+                                   C.c_double(tau), C.c_int(route_mode), _ptr(x), _ptr(w_r), _ptr(bias), _ptr(resident), C.c_int(n_res),
                                    _ptr(out["logits"]), _ptr(out["probs"]), _ptr(out["topk_idx"]), _ptr(out["gate"]),
                                    _ptr(out["counts"]), _ptr(out["offsets"]), _ptr(out["row_token"]), _ptr(out["pair_row"]))
         if rc != 0:

@@ -113,3 +113,58 @@ def test_silu_pack_payload_is_up_then_down(oracle64):
     pay = oracle64.pack(now, start)
     assert pay.shape == (3, 16)
     assert np.array_equal(pay[:, :8], start[1] - now[1]) and np.array_equal(pay[:, 8:], start[2] - now[2])
+
+
+# ----------------------------------------------------------------------------------------------------
+# forced-local routing (the paper's default mode): the partitioned router IS a standard
+# top-k MoE over the resident experts with the router sliced to their columns
+# ----------------------------------------------------------------------------------------------------
+def _sliced(prob, k):
+    S = prob["resident"]
+    full = {key: v[S].copy() for key, v in prob["full"].items()}
+    return dict(x=prob["x"], w_r=prob["w_r"][:, S].copy(), resident=np.arange(len(S), dtype=np.int32), full=full,
+                shared=prob["shared"], dy=prob["dy"], k=k, E=len(S))
+
+
+@pytest.mark.parametrize("seed", range(3))
+@pytest.mark.parametrize("gate_fn", [GATE_SOFTMAX, GATE_SIGMOID])
+@pytest.mark.parametrize("expert_fn", [0, EXPERT_SILU])
+def test_forced_local_is_standard_moe_on_resident_slice(oracle64, seed, gate_fn, expert_fn):
+    prob = refs.tiny_problem(60 + seed, T=31, d=9, E=8, k=2, F=6, n_res=[3, 5, 8][seed], n_sh=[0, 1, 0][seed], F_sh=4)
+    S, k = prob["resident"], prob["k"]
+    wg, wu, wd = refs.resident_stacks(prob)
+    shared = prob["shared"]
+    if expert_fn == EXPERT_SILU:
+        wg = None
+        shared = None if shared is None else (None, shared[1], shared[2])
+    r = oracle64.route(prob["x"], prob["w_r"], S, k, gate_fn, RULE_DROP_ONLY, 1.0, None, route_mode=1)
+    # every selected expert is resident, ghosts have probability 0 and logit -inf
+    assert np.isin(r["topk_idx"], S).all() and (r["pair_row"] >= 0).all() and r["P"] == 31 * k
+    ghost = np.setdiff1d(np.arange(8), S)
+    assert np.all(r["probs"][:, ghost] == 0) and np.all(np.isneginf(r["logits"][:, ghost]))
+    y = oracle64.moe_fwd(prob["x"], r, S, wg, wu, wd, shared, expert_fn=expert_fn)
+    b = oracle64.moe_bwd(prob["x"], prob["dy"], prob["w_r"], r, S, wg, wu, wd, shared, gate_fn, RULE_DROP_ONLY, 1.0, expert_fn=expert_fn)
+    # independent construction: torch autograd of the dense standard MoE over the resident slice
+    y_ref, g = refs.torch_dense_moe(_sliced(prob, k), gate_fn, expert_fn=expert_fn)
+    np.testing.assert_allclose(y, y_ref, rtol=1e-11, atol=1e-12)
+    np.testing.assert_allclose(b["dx"], g["dx"], rtol=1e-9, atol=1e-11)
+    np.testing.assert_allclose(b["dw_router"][:, S], g["dw_router"], rtol=1e-9, atol=1e-11)
+    assert np.all(b["dw_router"][:, ghost] == 0)      # no router column, no gradient
+    for key in ("dw_up", "dw_down") + (() if expert_fn == EXPERT_SILU else ("dw_gate",)):
+        np.testing.assert_allclose(b[key], g[key], rtol=1e-9, atol=1e-11, err_msg=key)
+    # and brute force over the slice
+    np.testing.assert_allclose(y, refs.brute_force_fwd(_sliced(prob, k), gate_fn, expert_fn=expert_fn), rtol=1e-11, atol=1e-13)
+
+
+def test_forced_local_all_resident_equals_skip_token(oracle64):
+    prob = refs.tiny_problem(70, T=20, d=7, E=6, k=3, F=5, n_res=6)
+    a = oracle64.route(prob["x"], prob["w_r"], prob["resident"], 3, GATE_SIGMOID, route_mode=0)
+    b = oracle64.route(prob["x"], prob["w_r"], prob["resident"], 3, GATE_SIGMOID, route_mode=1)
+    for key in ("topk_idx", "gate", "probs", "counts", "offsets", "row_token", "pair_row"):
+        assert np.array_equal(a[key], b[key]), key
+
+
+def test_forced_local_rejects_k_above_resident_count(oracle64):
+    prob = refs.tiny_problem(71, T=5, d=4, E=6, k=3, F=3, n_res=2)
+    with pytest.raises(ValueError):
+        oracle64.route(prob["x"], prob["w_r"], prob["resident"], 3, GATE_SIGMOID, route_mode=1)
