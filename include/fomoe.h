@@ -34,7 +34,7 @@
 extern "C" {
 #endif
 
-#define FOMOE_ABI_VERSION 2
+#define FOMOE_ABI_VERSION 3
 
 #if defined(__GNUC__)
 #define FOMOE_API __attribute__((visibility("default")))
@@ -67,6 +67,15 @@ extern "C" {
                                  the Silu nonlinearity is applied" (§B.3.1); the expert's payload "includes up and
                                  down projection".  W_gate / dW_gate arguments are ignored and may be NULL. */
 
+/* fomoe_config.route_mode */
+#define FOMOE_ROUTE_SKIP_TOKEN 0   /* router over all E experts, top-k, THEN ghost pairs are dropped (§3.3.3) */
+#define FOMOE_ROUTE_FORCED_LOCAL 1 /* the paper's default mode: the router is partitioned with the experts, "so that individual
+                                      tokens are not routed to experts that are unavailable to the local worker"; it
+                                      scores only the N_le resident experts (655-660 Eq. 19) and routing is bounded by
+                                      min(k, N_le): top_k must be <= n_res.  w_router / dw_router keep the full
+                                      [d,E] layout; ghost columns are not read into the decision (their logit is -inf, probability
+                                      0) and get zero gradient.  Every selected pair is kept. */
+
 typedef struct fomoe_config {
   int32_t T;           /* tokens (batch x sequence, flattened) */
   int32_t d_model;     /* d */
@@ -80,6 +89,7 @@ typedef struct fomoe_config {
   int32_t gate_rule;   /* FOMOE_DROP_ONLY | FOMOE_RENORM_* */
   float temperature;   /* tau: logits = x W_r / tau + bias (PAPER.md:175 names it, gives no formula); 1 by default */
   int32_t expert_fn;   /* FOMOE_EXPERT_SWIGLU | FOMOE_EXPERT_SILU */
+  int32_t route_mode;  /* FOMOE_ROUTE_SKIP_TOKEN | FOMOE_ROUTE_FORCED_LOCAL */
 } fomoe_config;
 
 /*

@@ -22,6 +22,7 @@ FOMOE_F32, FOMOE_BF16 = 0, 1
 FOMOE_GATE_SOFTMAX, FOMOE_GATE_SIGMOID = 0, 1
 FOMOE_DROP_ONLY, FOMOE_RENORM_TOPK, FOMOE_RENORM_RESIDENT = 0, 1, 2
 FOMOE_EXPERT_SWIGLU, FOMOE_EXPERT_SILU = 0, 1
+FOMOE_ROUTE_SKIP_TOKEN, FOMOE_ROUTE_FORCED_LOCAL = 0, 1
 
 EXPORTS = ("fomoe_workspace_bytes", "fomoe_route", "fomoe_moe_fwd", "fomoe_moe_bwd", "fomoe_pack_resident_deltas",
            "fomoe_moe_step_host", "fomoe_last_launch_count", "fomoe_last_cuda_error", "fomoe_abi_version",
@@ -31,7 +32,7 @@ EXPORTS = ("fomoe_workspace_bytes", "fomoe_route", "fomoe_moe_fwd", "fomoe_moe_b
 class fomoe_config(C.Structure):
     _fields_ = [("T", C.c_int32), ("d_model", C.c_int32), ("E", C.c_int32), ("top_k", C.c_int32), ("d_ff", C.c_int32),
                 ("n_shared", C.c_int32), ("d_ff_shared", C.c_int32), ("dtype", C.c_int32), ("gate_fn", C.c_int32),
-                ("gate_rule", C.c_int32), ("temperature", C.c_float), ("expert_fn", C.c_int32)]
+                ("gate_rule", C.c_int32), ("temperature", C.c_float), ("expert_fn", C.c_int32), ("route_mode", C.c_int32)]
 
 
 class fomoe_route_state(C.Structure):
@@ -56,7 +57,7 @@ def lib() -> C.CDLL:
         for name in EXPORTS:
             getattr(_lib, name).restype = C.c_int
         _lib.fomoe_last_cuda_error.restype = C.c_char_p
-        if _lib.fomoe_abi_version() != 2:
+        if _lib.fomoe_abi_version() != 3:
             raise FomoeError("libfomoe.so ABI version mismatch")
     return _lib
 
@@ -81,8 +82,9 @@ def _stream(stream=None) -> C.c_void_p:
 
 
 def make_config(T, d_model, E, top_k, d_ff, n_shared=0, d_ff_shared=0, dtype=FOMOE_BF16, gate_fn=FOMOE_GATE_SOFTMAX,
-                gate_rule=FOMOE_DROP_ONLY, temperature=1.0, expert_fn=FOMOE_EXPERT_SWIGLU) -> fomoe_config:
-    return fomoe_config(T, d_model, E, top_k, d_ff, n_shared, d_ff_shared, dtype, gate_fn, gate_rule, temperature, expert_fn)
+                gate_rule=FOMOE_DROP_ONLY, temperature=1.0, expert_fn=FOMOE_EXPERT_SWIGLU,
+                route_mode=FOMOE_ROUTE_SKIP_TOKEN) -> fomoe_config:
+    return fomoe_config(T, d_model, E, top_k, d_ff, n_shared, d_ff_shared, dtype, gate_fn, gate_rule, temperature, expert_fn, route_mode)
 
 
 def fomoe_workspace_bytes(cfg: fomoe_config, n_res: int):

@@ -48,6 +48,8 @@ static int check_cfg(const fomoe_config* c, int n_res) {
   if (c->gate_rule < FOMOE_DROP_ONLY || c->gate_rule > FOMOE_RENORM_RESIDENT) return FOMOE_ERR_BADARG;
   if (!(c->temperature > 0.f)) return FOMOE_ERR_BADARG;
   if (c->expert_fn != FOMOE_EXPERT_SWIGLU && c->expert_fn != FOMOE_EXPERT_SILU) return FOMOE_ERR_BADARG;
+  if (c->route_mode != FOMOE_ROUTE_SKIP_TOKEN && c->route_mode != FOMOE_ROUTE_FORCED_LOCAL) return FOMOE_ERR_BADARG;
+  if (c->route_mode == FOMOE_ROUTE_FORCED_LOCAL && c->top_k > n_res) return FOMOE_ERR_BADARG;   // bounded by min(k, N_le)
   if (c->E > kMaxE || c->top_k > kMaxK) return FOMOE_ERR_UNSUPPORTED;
   if ((long)c->T * c->top_k + (long)kTileM * (n_res + 1) > 0x7fffffffL / 2) return FOMOE_ERR_UNSUPPORTED;  // int32 row ids
   return FOMOE_OK;

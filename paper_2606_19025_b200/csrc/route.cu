@@ -29,7 +29,7 @@ constexpr int kRouteKC = 64;  // K chunk staged in shared memory
 template <typename XT, int EPW>  // EPW = experts per warp = ceil(E / 8)
 __global__ void __launch_bounds__(kRouteThreads)
 route_kernel(const XT* __restrict__ x, const float* __restrict__ w_r, const float* __restrict__ bias,
-             const int32_t* __restrict__ slot_of, int T, int d, int E, int k, int gate_fn, int gate_rule, float inv_tau,
+             const int32_t* __restrict__ slot_of, int T, int d, int E, int k, int gate_fn, int gate_rule, float inv_tau, int forced_local,
              float* __restrict__ probs, int32_t* __restrict__ topk_idx, float* __restrict__ gate) {
   extern __shared__ float smem[];
   float* xs = smem;                            // [kTok][kRouteKC + 1]
@@ -69,7 +69,8 @@ route_kernel(const XT* __restrict__ x, const float* __restrict__ w_r, const floa
 #pragma unroll
   for (int i = 0; i < EPW; ++i) {
     int e = warp + 8 * i;
-    if (e < E) zs[lane * (E + 1) + e] = acc[i] * inv_tau + (bias ? bias[e] : 0.f);
+    // forced-local routing: the partitioned router has no column for a non-resident expert
+    if (e < E) zs[lane * (E + 1) + e] = (forced_local && slot_of[e] < 0) ? -INFINITY : acc[i] * inv_tau + (bias ? bias[e] : 0.f);
   }
   __syncthreads();
 
@@ -292,7 +293,7 @@ static int launch_route_t(const fomoe_config& c, const XT* x, const float* w_rou
     auto kern = route_kernel<XT, N>;                                                                                    \
     FOMOE_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                   \
     kern<<<grid, kRouteThreads, smem, st>>>(x, w_router, bias, ws.slot_of, c.T, c.d_model, E, c.top_k, c.gate_fn,        \
-                                            c.gate_rule, inv_tau, out.probs, out.topk_idx, out.gate);                   \
+                                            c.gate_rule, inv_tau, c.route_mode == FOMOE_ROUTE_FORCED_LOCAL ? 1 : 0, out.probs, out.topk_idx, out.gate);                   \
   }
   if (epw <= 1) ROUTE_CASE(1)
   else if (epw <= 2) ROUTE_CASE(2)

@@ -60,7 +60,7 @@ struct TmaMaps {
 
 // ROUTE mode (rows F1-F4 + the per-block histogram of F5): everything the router epilogue needs
 struct RouteEpi {
-  int E, Epad, pieces, k, gate_fn, gate_rule, n_res;
+  int E, Epad, pieces, k, gate_fn, gate_rule, n_res, forced_local;
   float inv_tau;
   const float* bias;
   const int32_t* slot_of;
@@ -280,6 +280,8 @@ __device__ __forceinline__ void route_tile_epilogue(const UmmaParams& p, RouteSm
         float s = z[i] + md[i];
         if (three) s += lo[i];
         z[i] = s * r.inv_tau + (r.bias && c0 + i < E ? r.bias[c0 + i] : 0.f);
+        // forced-local routing: no router column for a non-resident expert: logit -inf, probability 0
+        if (r.forced_local && c0 + i < E && rs->slot[c0 + i] < 0) z[i] = -INFINITY;
       }
     };
     // pass 1: partial max and partial top-KMAX (descending, ties -> lower id: ascending scan + strict '>')
@@ -836,7 +838,8 @@ int umma_route(const fomoe_config& c, const void* x, const void* wr_split, int N
                const fomoe_route_state& out, const RouteWs& ws, cudaStream_t st) {
   UmmaParams p{};
   p.dense_rows = c.T; p.parts = 1; p.d = c.d_model; p.F = NP; p.ld = NP; p.N = NP;
-  p.r = RouteEpi{c.E, Epad, pieces, c.top_k, c.gate_fn, c.gate_rule, n_res, 1.0f / c.temperature, bias, ws.slot_of,
+  p.r = RouteEpi{c.E, Epad, pieces, c.top_k, c.gate_fn, c.gate_rule, n_res, c.route_mode == FOMOE_ROUTE_FORCED_LOCAL ? 1 : 0,
+                 1.0f / c.temperature, bias, ws.slot_of,
                  out.probs, out.topk_idx, out.gate, ws.blk_hist};
   TmaMaps m{};
   MAP_OK(make_map(&m.m[0], x, c.d_model, c.T, c.d_model, 128));

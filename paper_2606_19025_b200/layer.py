@@ -31,7 +31,7 @@ class SkipTokenMoE:
         self.n_res = int(len(resident))
         self.tdtype = torch.bfloat16 if w.dtype == "bf16" else torch.float32
         self.cfg = B.make_config(w.T, w.d, w.E, w.k, w.F, w.n_sh, w.F_sh, B.FOMOE_BF16 if w.dtype == "bf16" else B.FOMOE_F32,
-                                 w.gate_fn, w.gate_rule, w.temperature, w.expert_fn)
+                                 w.gate_fn, w.gate_rule, w.temperature, w.expert_fn, w.route_mode)
         dv, td = self.device, self.tdtype
         self.resident = _dev(np.asarray(resident, np.int32), torch.int32, dv) if self.n_res else torch.empty(0, dtype=torch.int32, device=dv)
         self.w_router = _dev(w_router, torch.float32, dv)

@@ -49,6 +49,7 @@ class MoEWorkload:
     gate_fn: int = GATE_SOFTMAX       # BASELINE.json: softmax; paper Eq. 17: sigmoid
     gate_rule: int = RULE_DROP_ONLY   # paper: drop-only
     temperature: float = 1.0
+    route_mode: int = 0               # 0 = skip-token, 1 = forced-local (partitioned router)
     expert_fn: int = 0                # 0 = SwiGLU (BASELINE.json), 1 = the paper's W_down silu(W_up x)
     seed: int = 0
     fixed_resident: Optional[tuple] = None
@@ -67,6 +68,7 @@ CONFIGS = {
 }
 C4_RESIDENT_SWEEP = (8, 16, 32, 64)
 EXPERT_SWIGLU, EXPERT_SILU = 0, 1
+ROUTE_SKIP_TOKEN, ROUTE_FORCED_LOCAL = 0, 1
 # The paper's own sigma-MoE layer at its Table 1 shapes: sigmoid gate (Eq. 17), two-matrix SiLU expert of
 # width d_expert = 128 (Eq. 16, §B.3.1), N_active of N_experts, sequence length 2048 x 8 sequences;
 # half of the experts resident (overlap O_e / M = 1/2).  P0 is a small fp32 case for element-wise parity.

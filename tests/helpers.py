@@ -35,7 +35,7 @@ def margin_clean(p: Problem, oracle64, max_attempts=20) -> int:
     w = p.w
     total = 0
     for attempt in range(max_attempts):
-        r = oracle64.route(p.x, p.w_router, p.resident, w.k, w.gate_fn, w.gate_rule, w.temperature, p.bias)
+        r = oracle64.route(p.x, p.w_router, p.resident, w.k, w.gate_fn, w.gate_rule, w.temperature, p.bias, w.route_mode)
         bad = np.nonzero(margins(r["logits"], w.k) < 2 * MARGIN)[0]
         if len(bad) == 0:
             return total
@@ -46,7 +46,7 @@ def margin_clean(p: Problem, oracle64, max_attempts=20) -> int:
 
 def oracle_all(p: Problem, o, bwd=True):
     w = p.w
-    r = o.route(p.x, p.w_router, p.resident, w.k, w.gate_fn, w.gate_rule, w.temperature, p.bias)
+    r = o.route(p.x, p.w_router, p.resident, w.k, w.gate_fn, w.gate_rule, w.temperature, p.bias, w.route_mode)
     y = o.moe_fwd(p.x, r, p.resident, p.wg, p.wu, p.wd, p.shared, expert_fn=w.expert_fn)
     b = None
     if bwd:

@@ -94,3 +94,32 @@ def test_paper_shapes_sampled(oracle64, name):
     print(name, "P", g["P"], {k: f"{v:.1e}" for k, v in errs.items()})
     bad = {k: v for k, v in errs.items() if not v <= TOL}
     assert not bad, bad
+
+
+# ---- forced-local routing: partitioned router, every selected pair is kept ----
+@pytest.mark.parametrize("expert_fn", [W.EXPERT_SWIGLU, W.EXPERT_SILU])
+@pytest.mark.parametrize("gate_fn", [W.GATE_SIGMOID, W.GATE_SOFTMAX])
+def test_forced_local_bf16_full(oracle64, gate_fn, expert_fn):
+    w = W.MoEWorkload("forced_bf16", T=1300, d=256, E=16, k=4, F=192, n_res=6, n_sh=1, F_sh=128, gate_fn=gate_fn,
+                      expert_fn=expert_fn, route_mode=W.ROUTE_FORCED_LOCAL, seed=7)
+    p = H.Problem(w)
+    errs, layer = run_and_compare(p, oracle64)
+    g = layer.routing_numpy()
+    assert g["P"] == w.T * w.k and np.isin(g["topk_idx"], p.resident).all()      # nothing is skipped
+    ghost = np.setdiff1d(np.arange(w.E), p.resident)
+    assert np.all(g["probs"][:, ghost] == 0) and np.all(H.t2n(layer.dw_router)[:, ghost] == 0)
+    print("forced_bf16", errs)
+
+
+def test_forced_local_fp32_full(oracle64):
+    w = W.config("P0").with_(route_mode=W.ROUTE_FORCED_LOCAL, n_res=5)
+    errs, layer = run_and_compare(H.Problem(w), oracle64)
+    assert layer.routing_numpy()["P"] == w.T * w.k
+    print("forced_f32", errs)
+
+
+def test_forced_local_rejects_k_above_n_res():
+    from paper_2606_19025_b200 import binding as B
+    cfg = B.make_config(T=64, d_model=64, E=8, top_k=4, d_ff=64, route_mode=B.FOMOE_ROUTE_FORCED_LOCAL)
+    with pytest.raises(B.FomoeError):
+        B.fomoe_workspace_bytes(cfg, 3)
