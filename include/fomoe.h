@@ -179,6 +179,34 @@ FOMOE_API int fomoe_pack_resident_deltas(const float* const w_now[3], const floa
                                const int32_t* pack_slots, int32_t n_pack, float* payload, void* stream);
 
 /*
+ * Fused local AdamW over the resident experts ("workers execute AdamW locally on their
+ * parameter subsets ... workers maintain history only for their own experts"; Table 7: weight decay 0,
+ * betas (0.9, 0.95), eps 1e-8).  The paper prints no formula; this is Loshchilov & Hutter's (R13), in fp32:
+ *   m = b1 m + (1-b1) g;  v = b2 v + (1-b2) g^2;  w -= lr wd w;  w -= lr (m / (1-b1^step)) / (sqrt(v / (1-b2^step)) + eps)
+ * w_master, m, v: host arrays of 3 device pointers (gate, up, down), each fp32 [n_res, elems_*], updated in place.
+ * grad: same shapes in `dtype` (FOMOE_F32 | FOMOE_BF16: what fomoe_moe_bwd wrote).  w_compute: NULL, or 3 device pointers
+ * (entries may be NULL) receiving w rounded to `dtype` — the copy the GEMMs read.  step counts from 1.
+ * A tensor with elems_* == 0 may be NULL (two-matrix expert).  elems_* must be multiples of 4.
+ */
+FOMOE_API int fomoe_adamw_resident(float* const w_master[3], const void* const grad[3], float* const m[3], float* const v[3],
+                         void* const w_compute[3], int32_t dtype, int32_t n_res, int64_t elems_gate, int64_t elems_up,
+                         int64_t elems_down, int32_t step, float lr, float beta1, float beta2, float eps, float weight_decay,
+                         void* stream);
+
+/*
+ * Outer optimizer step on the receiving side of the round boundary (Alg. 2 l.19-20; "DiLoCo/Nesterov uses
+ * server learning rate 0.7 and momentum 0.9").  payload_avg has the layout fomoe_pack_resident_deltas writes
+ * ([n_pack, elems_gate + elems_up + elems_down], block b <-> slot pack_slots[b]) and holds the replica-group AVERAGE of
+ * delta = w_round_start - w_local (the collective that averages it is out of scope: one GPU).  Per element (fp32):
+ *   buf = mu buf + delta;   w = w_start - lr (delta + mu buf)
+ * and w is written to w_start (the next round's start), w_now (the local master copy) and, if given, w_compute (rounded to
+ * `dtype`).  w_start, w_now, momentum: host arrays of 3 device pointers, fp32 [n_res, elems_*].  Slots not packed are untouched.
+ */
+FOMOE_API int fomoe_outer_nesterov(float* const w_start[3], float* const w_now[3], float* const momentum[3], void* const w_compute[3],
+                         int32_t dtype, const float* payload_avg, int32_t n_res, int64_t elems_gate, int64_t elems_up,
+                         int64_t elems_down, const int32_t* pack_slots, int32_t n_pack, float lr, float mu, void* stream);
+
+/*
  * One whole step from HOST buffers (the end-to-end path bench.py times): copies x_host (and dy_host) to the device,
  * runs fomoe_route + fomoe_moe_fwd + fomoe_moe_bwd, copies y and dx back.  x_host, dy_host, y_host, dx_host:
  * HOST pointers, [T,d] cfg->dtype, ideally pinned.  x_dev, dy_dev, y_dev, dx_dev: device staging buffers [T,d].

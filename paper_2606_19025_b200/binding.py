@@ -25,6 +25,7 @@ FOMOE_EXPERT_SWIGLU, FOMOE_EXPERT_SILU = 0, 1
 FOMOE_ROUTE_SKIP_TOKEN, FOMOE_ROUTE_FORCED_LOCAL = 0, 1
 
 EXPORTS = ("fomoe_workspace_bytes", "fomoe_route", "fomoe_moe_fwd", "fomoe_moe_bwd", "fomoe_pack_resident_deltas",
+           "fomoe_adamw_resident", "fomoe_outer_nesterov",
            "fomoe_moe_step_host", "fomoe_last_launch_count", "fomoe_last_cuda_error", "fomoe_abi_version",
            "fomoe_set_force_simt", "fomoe_profile_enable", "fomoe_profile_collect")
 
@@ -155,6 +156,44 @@ def fomoe_pack_resident_deltas(w_now, w_start, pack_slots, payload, stream=None)
     _check(lib().fomoe_pack_resident_deltas(now, start, C.c_int32(n_res), C.c_int64(elems[0]), C.c_int64(elems[1]),
                                             C.c_int64(elems[2]), _p(pack_slots), C.c_int32(n_pack), _p(payload), _stream(stream)),
            "fomoe_pack_resident_deltas")
+
+
+def _arr3(ts):
+    """Host array of 3 device pointers; None entries (zero-element tensors, two-matrix expert) become NULL."""
+    return (C.c_void_p * 3)(*(0 if t is None or t.numel() == 0 else t.data_ptr() for t in ts))
+
+
+def _elems3(ts):
+    return [0 if t is None or t.shape[0] == 0 else int(t[0].numel()) for t in ts]
+
+
+def fomoe_adamw_resident(w_master, grad, m, v, w_compute, step, lr, beta1=0.9, beta2=0.95, eps=1e-8, weight_decay=0.0,
+                         stream=None) -> None:
+    """3-tuples (gate, up, down) of device tensors [n_res, ...]: fp32 master / moments, grads in f32 or bf16."""
+    n_res = next(t.shape[0] for t in w_master if t is not None)
+    e = _elems3(w_master)
+    gd = next(t for t in grad if t is not None).dtype
+    dtype = FOMOE_BF16 if gd == torch.bfloat16 else FOMOE_F32
+    wc = _arr3(w_compute) if w_compute is not None else None
+    assert w_compute is None or all(t is None or t.dtype == gd for t in w_compute), "w_compute must have the gradients' dtype"
+    _check(lib().fomoe_adamw_resident(_arr3(w_master), _arr3(grad), _arr3(m), _arr3(v), wc, C.c_int32(dtype), C.c_int32(n_res),
+                                      C.c_int64(e[0]), C.c_int64(e[1]), C.c_int64(e[2]), C.c_int32(step), C.c_float(lr),
+                                      C.c_float(beta1), C.c_float(beta2), C.c_float(eps), C.c_float(weight_decay), _stream(stream)),
+           "fomoe_adamw_resident")
+
+
+def fomoe_outer_nesterov(w_start, w_now, momentum, w_compute, payload_avg, pack_slots=None, lr=0.7, mu=0.9, stream=None) -> None:
+    n_res = next(t.shape[0] for t in w_start if t is not None)
+    e = _elems3(w_start)
+    dtype = FOMOE_F32
+    wc = None
+    if w_compute is not None:
+        wc = _arr3(w_compute)
+        dtype = FOMOE_BF16 if next(t for t in w_compute if t is not None).dtype == torch.bfloat16 else FOMOE_F32
+    n_pack = n_res if pack_slots is None else int(pack_slots.numel())
+    _check(lib().fomoe_outer_nesterov(_arr3(w_start), _arr3(w_now), _arr3(momentum), wc, C.c_int32(dtype), _p(payload_avg),
+                                      C.c_int32(n_res), C.c_int64(e[0]), C.c_int64(e[1]), C.c_int64(e[2]), _p(pack_slots),
+                                      C.c_int32(n_pack), C.c_float(lr), C.c_float(mu), _stream(stream)), "fomoe_outer_nesterov")
 
 
 def fomoe_moe_step_host(cfg, x_host, dy_host, y_host, dx_host, x_dev, dy_dev, y_dev, dx_dev, w_router, router_bias, resident_ids,

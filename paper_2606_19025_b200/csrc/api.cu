@@ -213,6 +213,46 @@ int fomoe_pack_resident_deltas(const float* const w_now[3], const float* const w
   return launch_pack(w_now, w_start, n_res, elems_gate, elems_up, elems_down, pack_slots, n_pack, payload, (cudaStream_t)stream);
 }
 
+int fomoe_adamw_resident(float* const w_master[3], const void* const grad[3], float* const m[3], float* const v[3],
+                         void* const w_compute[3], int32_t dtype, int32_t n_res, int64_t elems_gate, int64_t elems_up,
+                         int64_t elems_down, int32_t step, float lr, float beta1, float beta2, float eps, float weight_decay,
+                         void* stream) {
+  g_launches = 0;
+  if (!w_master || !grad || !m || !v || n_res < 0 || step < 1 || elems_gate < 0 || elems_up < 0 || elems_down < 0) return FOMOE_ERR_BADARG;
+  if (dtype != FOMOE_F32 && dtype != FOMOE_BF16) return FOMOE_ERR_BADARG;
+  if (!(beta1 >= 0.f && beta1 < 1.f && beta2 >= 0.f && beta2 < 1.f) || !(eps >= 0.f)) return FOMOE_ERR_BADARG;
+  const int64_t elems[3] = {elems_gate, elems_up, elems_down};
+  for (int i = 0; i < 3; ++i) {
+    if (elems[i] % 4) return FOMOE_ERR_UNSUPPORTED;
+    if (elems[i] > 0 && n_res > 0 && (!w_master[i] || !grad[i] || !m[i] || !v[i])) return FOMOE_ERR_BADARG;
+    if (!aligned16(w_master[i]) || !aligned16(grad[i]) || !aligned16(m[i]) || !aligned16(v[i]) || (w_compute && !aligned16(w_compute[i])))
+      return FOMOE_ERR_BADARG;
+  }
+  note_api_entry("@fomoe_adamw_resident", (cudaStream_t)stream);
+  return launch_adamw(w_master, grad, m, v, w_compute, dtype, n_res, elems, step, lr, beta1, beta2, eps, weight_decay, (cudaStream_t)stream);
+}
+
+int fomoe_outer_nesterov(float* const w_start[3], float* const w_now[3], float* const momentum[3], void* const w_compute[3],
+                         int32_t dtype, const float* payload_avg, int32_t n_res, int64_t elems_gate, int64_t elems_up,
+                         int64_t elems_down, const int32_t* pack_slots, int32_t n_pack, float lr, float mu, void* stream) {
+  g_launches = 0;
+  if (!w_start || !w_now || !momentum || n_res < 0 || n_pack < 0 || elems_gate < 0 || elems_up < 0 || elems_down < 0) return FOMOE_ERR_BADARG;
+  if (dtype != FOMOE_F32 && dtype != FOMOE_BF16) return FOMOE_ERR_BADARG;
+  if (!pack_slots && n_pack != n_res) return FOMOE_ERR_BADARG;
+  if (n_pack == 0) return FOMOE_OK;
+  if (!payload_avg || !aligned16(payload_avg)) return FOMOE_ERR_BADARG;
+  const int64_t elems[3] = {elems_gate, elems_up, elems_down};
+  for (int i = 0; i < 3; ++i) {
+    if (elems[i] % 4) return FOMOE_ERR_UNSUPPORTED;
+    if (elems[i] > 0 && (!w_start[i] || !w_now[i] || !momentum[i])) return FOMOE_ERR_BADARG;
+    if (!aligned16(w_start[i]) || !aligned16(w_now[i]) || !aligned16(momentum[i]) || (w_compute && !aligned16(w_compute[i])))
+      return FOMOE_ERR_BADARG;
+  }
+  note_api_entry("@fomoe_outer_nesterov", (cudaStream_t)stream);
+  return launch_outer_nesterov(w_start, w_now, momentum, w_compute, dtype, payload_avg, elems, pack_slots, n_pack, lr, mu,
+                               (cudaStream_t)stream);
+}
+
 int fomoe_moe_step_host(const fomoe_config* cfg, const void* x_host, const void* dy_host, void* y_host, void* dx_host, void* x_dev,
                         void* dy_dev, void* y_dev, void* dx_dev, const float* w_router, const float* router_bias,
                         const int32_t* resident_ids, int32_t n_res, const fomoe_route_state* route, const void* w_gate,

@@ -243,4 +243,11 @@ int umma_router_bwd(const fomoe_config& c, const void* x, const float* w_router,
 int launch_pack(const float* const w_now[3], const float* const w_start[3], int n_res, int64_t eg, int64_t eu, int64_t ed,
                 const int32_t* pack_slots, int n_pack, float* payload, cudaStream_t st);
 
+// optimizer steps around the pack (optim.cu)
+int launch_adamw(float* const w[3], const void* const g[3], float* const m[3], float* const v[3], void* const wc[3], int dtype,
+                 int n_res, const int64_t elems[3], int step, float lr, float b1, float b2, float eps, float wd, cudaStream_t st);
+int launch_outer_nesterov(float* const w_start[3], float* const w_now[3], float* const buf[3], void* const wc[3], int dtype,
+                          const float* payload, const int64_t elems[3], const int32_t* pack_slots, int n_pack, float lr, float mu,
+                          cudaStream_t st);
+
 }  // namespace fomoe
