@@ -158,11 +158,23 @@ def oracle_sample_time(w: W.MoEWorkload, n_res: int, sample_tokens: int, reps: i
     return times, o.threads()
 
 
+def sized_sample(w, n_res, target_s: float, cap_tokens: int) -> int:
+    """Tokens of the workload the oracle gets through in about `target_s` seconds on this box: a 64-token probe, then scale."""
+    probe = min(w.T, 64)
+    times, _ = oracle_sample_time(w, n_res, probe)
+    rate = probe / max(times[0], 1e-6)
+    n = int(rate * target_s)
+    n = max(64, min(cap_tokens, w.T, (n // 64) * 64 if n >= 64 else 64))
+    return n
+
+
 def run_reference(args, w, n_res):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    sample = min(w.T, args.ref_tokens)
+    # every step is a bounded sample of the workload, sized so that the whole run ends within a few minutes
+    per_step_s = max(0.5, min(15.0, 150.0 / max(1, args.steps + args.warmup)))
+    sample = sized_sample(w, n_res, per_step_s, args.ref_tokens)
     times, cores = oracle_sample_time(w, n_res, sample, reps=args.warmup + args.steps)
     timed = times[args.warmup:]
     ms = 1e3 * sum(timed) / len(timed)
@@ -436,7 +448,7 @@ def run_gpu(args, w, n_res):
 
         # ---- the oracle, as it stands, on the host cores (reported baseline, not the target) ----
         if not args.no_cpu_baseline:
-            sample = min(w.T, args.ref_tokens)
+            sample = sized_sample(w, n_res, 15.0, args.ref_tokens)     # about 15 s of CPU work
             times, cores = oracle_sample_time(w, n_res, sample)
             out["cpu_baseline"] = {"value": sample / times[0], "unit": UNIT, "cores": cores, "kind": "oracle",
                                    "sample": f"first {sample} of {w.T} tokens, all {n_res} resident experts' weights, "
@@ -455,7 +467,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C2", choices=sorted(W.CONFIGS))
     ap.add_argument("--n-res", type=int, default=None)
-    ap.add_argument("--ref-tokens", type=int, default=1024, help="tokens per step of the CPU oracle sample")
+    ap.add_argument("--ref-tokens", type=int, default=16384, help="upper bound on the tokens per step of the CPU oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-all-resident", action="store_true")
     ap.add_argument("--ghost-sweep", action="store_true", help="also time the step for n_res = E, 3E/4, E/2, E/4, E/8 (Fig. 11 analogue)")
