@@ -480,7 +480,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
         for (int kb = 0; kb < t.num_kb; ++kb) {
           mbar_wait(smem_u32(&empty_bar[stage]), phase ^ 1);
           const uint32_t sa = smem_u32(smem + stage * kStageBytes), sb = sa + kABytes;
-          const uint32_t fb = mapa_u32(smem_u32(&full_bar[stage]), 0);
+          const uint32_t fb = smem_u32(&full_bar[stage]) & 0xFEFFFFFFu;   // peer bit cleared: the pair leader's barrier
           // a pair whose second row tile does not exist (odd tile count of a slot, or the dense tail) skips CTA 1's A load:
           // the MMA then reads stale shared memory for rows nobody stores.  `peer_live` is what CTA 1 decodes as t.live
           if (rank == 0) mbar_expect_tx(smem_u32(&full_bar[stage]), 2 * kStageBytes - (peer_live ? 0 : kABytes));
@@ -569,7 +569,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
     const int q = warp & 3;               // TMEM lane quarter of this warp
     const int half = (warp >> 2) - 1;     // which of the two warps of the quarter: takes chunks half, half + 2, ...
     const uint32_t stg0 = smem_u32(stg_base) + (uint32_t)((warp - 4) * (kStgTilesPerWarp * kStgTile));
-    const uint32_t tempty_leader = mapa_u32(smem_u32(&tempty_bar[0]), 0);  // + 8 * stage
+    const uint32_t tempty_leader = smem_u32(&tempty_bar[0]) & 0xFEFFFFFFu;  // the pair leader's barrier (peer bit cleared); + 8 * stage
     if (MODE == ROUTE) {
       RouteSmem* rs = reinterpret_cast<RouteSmem*>(stg_base);
       {  // slot map and cleared histograms, visible to all epilogue warps before the first tile
