@@ -10,7 +10,10 @@
  * General conventions (every entry point):
  *   - Pointers are DEVICE pointers unless the parameter is documented as "host".  The `cfg` structs and
  *     `fomoe_route_state` themselves live on the host; the pointers inside them are device pointers.
- *   - Every buffer is caller-owned.  The library never allocates, frees or keeps a pointer after return.
+ *   - Every buffer is caller-owned.  The library never allocates device memory, frees or keeps a pointer after return.
+ *     (Its only own state: one internal non-blocking stream and two events per host thread, created on first use by
+ *     fomoe_moe_bwd, which forks the router's backward onto it and joins before returning work to `stream`; the fork /
+ *     join are event dependencies, so a step stays capturable in a CUDA graph.  FOMOE_SIDE_STREAM=0 disables it.)
  *     Workspace sizes come from fomoe_workspace_bytes().  All device pointers must be 16-byte aligned.
  *   - Tensors are dense row-major.  Weights are [out,in].  Expert weights are stored ONLY for resident
  *     experts ("the per-worker memory footprint for expert weights decreases") and are

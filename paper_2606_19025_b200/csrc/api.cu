@@ -36,6 +36,34 @@ int set_cuda_error(cudaError_t e, const char* where) {
   return FOMOE_ERR_CUDA;
 }
 
+// The one piece of state the library owns: a side stream and two events per host thread, used by fomoe_moe_bwd to run the
+// router's backward chain (gate_bwd, dz W_r^T, x^T dz) beside the expert GEMMs.  Fork / join through events, so the pattern
+// is capturable in a CUDA graph.  FOMOE_SIDE_STREAM=0 in the environment turns it off.
+struct SideStream {
+  int dev = -1;
+  cudaStream_t s = nullptr;
+  cudaEvent_t fork = nullptr, join = nullptr;
+};
+static thread_local SideStream g_side;
+static bool side_enabled() {
+  static const bool on = [] { const char* e = getenv("FOMOE_SIDE_STREAM"); return !(e && e[0] == '0'); }();
+  return on;
+}
+static SideStream* side_stream() {
+  if (!side_enabled() || g_prof_on) return nullptr;   // per-kernel timing needs one serial stream
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) return nullptr;
+  if (g_side.dev != dev) {
+    g_side = SideStream{};
+    if (cudaStreamCreateWithFlags(&g_side.s, cudaStreamNonBlocking) != cudaSuccess) return nullptr;
+    if (cudaEventCreateWithFlags(&g_side.fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&g_side.join, cudaEventDisableTiming) != cudaSuccess)
+      return nullptr;
+    g_side.dev = dev;
+  }
+  return &g_side;
+}
+
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 static int check_cfg(const fomoe_config* c, int n_res) {
@@ -178,18 +206,37 @@ int fomoe_moe_bwd(const fomoe_config* cfg, const void* dy, const void* x, const 
   } else {
     FOMOE_CUDA_OK(cudaMemsetAsync(sws.dgate, 0, sizeof(float) * (size_t)cfg->T * cfg->top_k, st));
   }
+  // B6, B7 depend only on dgate (B1): on the tensor-core path they run on the side stream, beside B2-B4
+  const bool tc_router = use_umma(*cfg) && cfg->T > 0;
+  SideStream* side = tc_router ? side_stream() : nullptr;
+  cudaStream_t rst = st;
+  if (side) {
+    FOMOE_CUDA_OK(cudaEventRecord(side->fork, st));
+    FOMOE_CUDA_OK(cudaStreamWaitEvent(side->s, side->fork, 0));
+    rst = side->s;
+  }
+  auto router_bwd = [&]() -> int {
+    int r = launch_gate_bwd(*cfg, *route, rws, sws.dgate, sws.dz, tc_router ? sws.dz_bf : nullptr, sws.Ez, rst);
+    if (r != FOMOE_OK) return r;
+    // (the tensor-core router of fomoe_route left W_r in bf16 in the route workspace)
+    return tc_router ? umma_router_bwd(*cfg, x, w_router, route_umma_supported(*cfg) ? rws.wr_bf : nullptr, sws, dw_router, rst)
+                     : simt_router_bwd(*cfg, x, w_router, sws, dw_router, rst);
+  };
+  if (side) {
+    rc = router_bwd();
+    if (rc != FOMOE_OK) return rc;
+    FOMOE_CUDA_OK(cudaEventRecord(side->join, side->s));
+  }
   // B2-B4 (+ shared experts)
   rc = use_umma(*cfg) ? umma_ffn_bwd(*cfg, n_res, x, dy, rws, aws, sws, w, dw_gate, dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, st)
                       : simt_ffn_bwd(*cfg, n_res, x, dy, rws, aws, sws, w, dw_gate, dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, st);
   if (rc != FOMOE_OK) return rc;
-  // B6, B7
-  const bool tc_router = use_umma(*cfg) && cfg->T > 0;
-  rc = launch_gate_bwd(*cfg, *route, rws, sws.dgate, sws.dz, tc_router ? sws.dz_bf : nullptr, sws.Ez, st);
-  if (rc != FOMOE_OK) return rc;
-  // (the tensor-core router of fomoe_route left W_r in bf16 in the route workspace)
-  rc = tc_router ? umma_router_bwd(*cfg, x, w_router, route_umma_supported(*cfg) ? rws.wr_bf : nullptr, sws, dw_router, st)
-                 : simt_router_bwd(*cfg, x, w_router, sws, dw_router, st);
-  if (rc != FOMOE_OK) return rc;
+  if (side) {
+    FOMOE_CUDA_OK(cudaStreamWaitEvent(st, side->join, 0));
+  } else {
+    rc = router_bwd();
+    if (rc != FOMOE_OK) return rc;
+  }
   // B5
   return launch_dx_sum(*cfg, rws, sws.dxp, cfg->n_shared > 0 ? sws.dx_sh : nullptr, tc_router ? nullptr : sws.dx_r,
                        tc_router ? (const void*)sws.dx_r : nullptr, dx, st);
