@@ -197,32 +197,47 @@ __global__ void perm_scan_kernel(int32_t* __restrict__ blk_hist, int n_blk, int 
     if (lane == 0) { counts[s] = run; s_cnt[s] = run; }
   }
   __syncthreads();
-  if (threadIdx.x == 0) {
+  // exclusive scans over the slots of (count, padded count, tile pairs): warp 0, 32 slots per shuffle scan
+  if (warp == 0) {
     int off = 0, pad = 0, pairs = 0;
-    for (int s = 0; s < n_res; ++s) {
-      offsets[s] = off;
-      pad_offsets[s] = pad;
-      pad_end64[s] = pad + (s_cnt[s] + 63) / 64 * 64;
-      s_pad[s] = pad;
-      s_pair[s] = pairs;
-      off += s_cnt[s];
-      const int tiles = (s_cnt[s] + kTileM - 1) / kTileM;
-      pad += tiles * kTileM;
-      pairs += (tiles + 1) / 2;
+    for (int s0 = 0; s0 < n_res; s0 += 32) {
+      const int s = s0 + lane;
+      const int c = s < n_res ? s_cnt[s] : 0;
+      const int tiles = (c + kTileM - 1) / kTileM;
+      int ic = c, ip = tiles * kTileM, iq = (tiles + 1) / 2;
+      const int pc = ip, qc = iq;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int vc = __shfl_up_sync(0xffffffffu, ic, o), vp = __shfl_up_sync(0xffffffffu, ip, o), vq = __shfl_up_sync(0xffffffffu, iq, o);
+        if (lane >= o) { ic += vc; ip += vp; iq += vq; }
+      }
+      if (s < n_res) {
+        offsets[s] = off + ic - c;
+        pad_offsets[s] = pad + ip - pc;
+        pad_end64[s] = pad + ip - pc + (c + 63) / 64 * 64;
+        s_pad[s] = pad + ip - pc;
+        s_pair[s] = pairs + iq - qc;
+      }
+      off += __shfl_sync(0xffffffffu, ic, 31);
+      pad += __shfl_sync(0xffffffffu, ip, 31);
+      pairs += __shfl_sync(0xffffffffu, iq, 31);
     }
-    offsets[n_res] = off;
-    pad_offsets[n_res] = pad;
-    s_pad[n_res] = pad;
-    s_pair[n_res] = pairs;
-    n_mtiles[0] = pad / kTileM;
-    n_mtiles[1] = pad;
-    n_mtiles[2] = pairs;
+    if (lane == 0) {
+      offsets[n_res] = off;
+      pad_offsets[n_res] = pad;
+      s_pad[n_res] = pad;
+      s_pair[n_res] = pairs;
+      n_mtiles[0] = pad / kTileM;
+      n_mtiles[1] = pad;
+      n_mtiles[2] = pairs;
+    }
   }
   __syncthreads();
-  for (int s = 0; s < n_res; ++s) {
+  // row tile -> slot and the pair schedule: one warp per slot
+  for (int s = warp; s < n_res; s += n_warps) {
     const int t0 = s_pad[s] / kTileM, t1 = s_pad[s + 1] / kTileM;
-    for (int i = t0 + threadIdx.x; i < t1; i += blockDim.x) tile_slot[i] = s;
-    for (int i = threadIdx.x; i < s_pair[s + 1] - s_pair[s]; i += blockDim.x)
+    for (int i = t0 + lane; i < t1; i += 32) tile_slot[i] = s;
+    for (int i = lane; i < s_pair[s + 1] - s_pair[s]; i += 32)
       pair_info[s_pair[s] + i] = 2 * (t0 + 2 * i) + (t0 + 2 * i + 1 < t1 ? 1 : 0);
   }
 }
