@@ -109,6 +109,27 @@ def test_large_E_topk8(oracle64):
     run_and_compare(H.Problem(w), oracle64)
 
 
+def test_wide_router_feeds_tensor_core_gemms(oracle64):
+    """E = 192 > 128: the fp32 SIMT router (any E <= 512) in front of the tcgen05 expert GEMMs and tensor-core router backward."""
+    w = W.MoEWorkload("wideE", T=520, d=128, E=192, k=4, F=128, n_res=40, dtype="bf16", gate_fn=W.GATE_SIGMOID, seed=10)
+    errs, _ = run_and_compare(H.Problem(w), oracle64)
+    print("wideE", errs)
+
+
+def test_empty_batch_bf16(oracle64):
+    """T = 0 on the tensor-core path: counts / offsets zero, weight gradients exactly zero, nothing hangs."""
+    import torch
+    p = H.Problem(W.MoEWorkload("empty_bf16", T=0, d=128, E=8, k=2, F=128, n_res=4, n_sh=1, F_sh=64, dtype="bf16", seed=6))
+    layer = H.make_layer(p)
+    x = layer.to_dev(p.x)
+    layer.step(x, x)
+    torch.cuda.synchronize()
+    g = layer.routing_numpy()
+    assert g["P"] == 0 and not g["counts"].any()
+    for t in (layer.dw_router, layer.dw_gate, layer.dw_up, layer.dw_down, *layer.d_shared):
+        assert not t.float().abs().max().item() > 0
+
+
 def test_routing_is_deterministic(oracle64):
     import torch
     p = H.Problem(W.MoEWorkload("det", T=2048, d=128, E=16, k=2, F=64, n_res=8, dtype="bf16", seed=8))
