@@ -182,6 +182,28 @@ FOMOE_API int fomoe_pack_resident_deltas(const float* const w_now[3], const floa
                                const int32_t* pack_slots, int32_t n_pack, float* payload, void* stream);
 
 /*
+ * Peripheral LayerNorm either side of the MoE block:  x_{l+1} = x_l + alpha LN(F(LN(x_l)))
+ * (Eq. 15, "normalization exclusively to the residual branches"; depth multiplier alpha on the block
+ * output, Fig. 12).  The paper gives no LN formula: standard LayerNorm over d_model with gain, bias and eps
+ * (R14).  x, residual, out, dout, dresidual, dx: [T,d_model] in `dtype`; gamma, beta, dgamma, dbeta: fp32 [d_model];
+ * stats: fp32 [T,2] = (mean, 1/sqrt(var + eps)) of each row, written by the forward and read by the backward.
+ *   fomoe_periln_fwd:  out = (residual ? residual : 0) + alpha (gamma xhat + beta)
+ *       pre-LN:  fomoe_periln_fwd(x, g1, b1, residual = NULL, alpha = 1) -> the tokens fomoe_route / fomoe_moe_fwd consume
+ *       post-LN: fomoe_periln_fwd(y, g2, b2, residual = x, alpha)        -> x_{l+1}
+ *   fomoe_periln_bwd:  dx = (dresidual ? dresidual : 0) + d/dx of alpha (gamma xhat + beta) contracted with dout;
+ *                      dgamma, dbeta overwritten (fixed-order reduction: run-to-run identical)
+ *       post-LN: fomoe_periln_bwd(dout, y, stats2, g2, alpha, dresidual = NULL) -> dy, the dy of fomoe_moe_bwd
+ *       pre-LN:  fomoe_periln_bwd(dxn, x, stats1, g1, 1, dresidual = dout)      -> dx of the whole block (residual path added)
+ * partials: device workspace of fomoe_periln_workspace_bytes(T, d_model) bytes.  d_model <= 12800.
+ */
+FOMOE_API int fomoe_periln_workspace_bytes(int32_t T, int32_t d_model, size_t* partials);
+FOMOE_API int fomoe_periln_fwd(int32_t T, int32_t d_model, int32_t dtype, const void* x, const float* gamma, const float* beta, float eps,
+                     const void* residual, float alpha, void* out, float* stats, void* stream);
+FOMOE_API int fomoe_periln_bwd(int32_t T, int32_t d_model, int32_t dtype, const void* dout, const void* x, const float* stats,
+                     const float* gamma, float alpha, const void* dresidual, void* dx, float* dgamma, float* dbeta, float* partials,
+                     void* stream);
+
+/*
  * Fused local AdamW over the resident experts ("workers execute AdamW locally on their
  * parameter subsets ... workers maintain history only for their own experts"; Table 7: weight decay 0,
  * betas (0.9, 0.95), eps 1e-8).  The paper prints no formula; this is Loshchilov & Hutter's (R13), in fp32:

@@ -25,7 +25,7 @@ FOMOE_EXPERT_SWIGLU, FOMOE_EXPERT_SILU = 0, 1
 FOMOE_ROUTE_SKIP_TOKEN, FOMOE_ROUTE_FORCED_LOCAL = 0, 1
 
 EXPORTS = ("fomoe_workspace_bytes", "fomoe_route", "fomoe_moe_fwd", "fomoe_moe_bwd", "fomoe_pack_resident_deltas",
-           "fomoe_adamw_resident", "fomoe_outer_nesterov",
+           "fomoe_adamw_resident", "fomoe_outer_nesterov", "fomoe_periln_workspace_bytes", "fomoe_periln_fwd", "fomoe_periln_bwd",
            "fomoe_moe_step_host", "fomoe_last_launch_count", "fomoe_last_cuda_error", "fomoe_abi_version",
            "fomoe_set_force_simt", "fomoe_profile_enable", "fomoe_profile_collect")
 
@@ -156,6 +156,28 @@ def fomoe_pack_resident_deltas(w_now, w_start, pack_slots, payload, stream=None)
     _check(lib().fomoe_pack_resident_deltas(now, start, C.c_int32(n_res), C.c_int64(elems[0]), C.c_int64(elems[1]),
                                             C.c_int64(elems[2]), _p(pack_slots), C.c_int32(n_pack), _p(payload), _stream(stream)),
            "fomoe_pack_resident_deltas")
+
+
+def _dt(t: torch.Tensor) -> int:
+    return FOMOE_BF16 if t.dtype == torch.bfloat16 else FOMOE_F32
+
+
+def fomoe_periln_workspace_bytes(T: int, d_model: int) -> int:
+    n = C.c_size_t(0)
+    _check(lib().fomoe_periln_workspace_bytes(C.c_int32(T), C.c_int32(d_model), C.byref(n)), "fomoe_periln_workspace_bytes")
+    return n.value
+
+
+def fomoe_periln_fwd(x, gamma, beta, out, stats, residual=None, alpha=1.0, eps=1e-5, stream=None) -> None:
+    T, d = x.shape
+    _check(lib().fomoe_periln_fwd(C.c_int32(T), C.c_int32(d), C.c_int32(_dt(x)), _p(x), _p(gamma), _p(beta), C.c_float(eps), _p(residual),
+                                  C.c_float(alpha), _p(out), _p(stats), _stream(stream)), "fomoe_periln_fwd")
+
+
+def fomoe_periln_bwd(dout, x, stats, gamma, dx, dgamma, dbeta, partials, dresidual=None, alpha=1.0, stream=None) -> None:
+    T, d = x.shape
+    _check(lib().fomoe_periln_bwd(C.c_int32(T), C.c_int32(d), C.c_int32(_dt(x)), _p(dout), _p(x), _p(stats), _p(gamma), C.c_float(alpha),
+                                  _p(dresidual), _p(dx), _p(dgamma), _p(dbeta), _p(partials), _stream(stream)), "fomoe_periln_bwd")
 
 
 def _arr3(ts):

@@ -260,6 +260,32 @@ int fomoe_pack_resident_deltas(const float* const w_now[3], const float* const w
   return launch_pack(w_now, w_start, n_res, elems_gate, elems_up, elems_down, pack_slots, n_pack, payload, (cudaStream_t)stream);
 }
 
+int fomoe_periln_workspace_bytes(int32_t T, int32_t d_model, size_t* partials) {
+  if (T < 0 || d_model <= 0 || !partials) return FOMOE_ERR_BADARG;
+  *partials = sizeof(float) * 2 * (size_t)periln_blocks(T) * (size_t)d_model;
+  return FOMOE_OK;
+}
+
+int fomoe_periln_fwd(int32_t T, int32_t d_model, int32_t dtype, const void* x, const float* gamma, const float* beta, float eps,
+                     const void* residual, float alpha, void* out, float* stats, void* stream) {
+  g_launches = 0;
+  if (T < 0 || d_model <= 0 || (dtype != FOMOE_F32 && dtype != FOMOE_BF16) || !gamma || !beta || !(eps >= 0.f)) return FOMOE_ERR_BADARG;
+  if (T > 0 && (!x || !out || !stats)) return FOMOE_ERR_BADARG;
+  if ((size_t)d_model * 16 > 200 * 1024) return FOMOE_ERR_UNSUPPORTED;   // the backward stages 4 fp32 rows in shared memory
+  note_api_entry("@fomoe_periln_fwd", (cudaStream_t)stream);
+  return launch_periln_fwd(T, d_model, dtype, x, gamma, beta, eps, residual, alpha, out, stats, (cudaStream_t)stream);
+}
+
+int fomoe_periln_bwd(int32_t T, int32_t d_model, int32_t dtype, const void* dout, const void* x, const float* stats, const float* gamma,
+                     float alpha, const void* dresidual, void* dx, float* dgamma, float* dbeta, float* partials, void* stream) {
+  g_launches = 0;
+  if (T < 0 || d_model <= 0 || (dtype != FOMOE_F32 && dtype != FOMOE_BF16) || !gamma || !dgamma || !dbeta || !partials) return FOMOE_ERR_BADARG;
+  if (T > 0 && (!dout || !x || !stats || !dx)) return FOMOE_ERR_BADARG;
+  if ((size_t)d_model * 16 > 200 * 1024) return FOMOE_ERR_UNSUPPORTED;
+  note_api_entry("@fomoe_periln_bwd", (cudaStream_t)stream);
+  return launch_periln_bwd(T, d_model, dtype, dout, x, stats, gamma, alpha, dresidual, dx, dgamma, dbeta, partials, (cudaStream_t)stream);
+}
+
 int fomoe_adamw_resident(float* const w_master[3], const void* const grad[3], float* const m[3], float* const v[3],
                          void* const w_compute[3], int32_t dtype, int32_t n_res, int64_t elems_gate, int64_t elems_up,
                          int64_t elems_down, int32_t step, float lr, float beta1, float beta2, float eps, float weight_decay,

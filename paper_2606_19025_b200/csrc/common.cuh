@@ -243,6 +243,13 @@ int umma_router_bwd(const fomoe_config& c, const void* x, const float* w_router,
 int launch_pack(const float* const w_now[3], const float* const w_start[3], int n_res, int64_t eg, int64_t eu, int64_t ed,
                 const int32_t* pack_slots, int n_pack, float* payload, cudaStream_t st);
 
+// Peri-LN either side of the block (periln.cu)
+int periln_blocks(int T);
+int launch_periln_fwd(int T, int d, int dtype, const void* x, const float* gamma, const float* beta, float eps, const void* residual,
+                      float alpha, void* out, float* stats, cudaStream_t st);
+int launch_periln_bwd(int T, int d, int dtype, const void* dout, const void* x, const float* stats, const float* gamma, float alpha,
+                      const void* dresidual, void* dx, float* dgamma, float* dbeta, float* partials, cudaStream_t st);
+
 // optimizer steps around the pack (optim.cu)
 int launch_adamw(float* const w[3], const void* const g[3], float* const m[3], float* const v[3], void* const wc[3], int dtype,
                  int n_res, const int64_t elems[3], int step, float lr, float b1, float b2, float eps, float wd, cudaStream_t st);

@@ -1,0 +1,104 @@
+"""Parity of the Peri-LN kernels (fomoe_periln_fwd / _bwd) against oracle/periln_oracle.py through the C ABI, and of the whole
+block of PAPER.md:571 Eq. 15 — x + alpha LN(MoE(LN(x))) — assembled from the C-ABI calls against the same assembly of the
+two oracles.  fp32: max|err|/max|ref| <= 1e-4; bf16: <= 2e-2."""
+import numpy as np
+import pytest
+
+import helpers as H
+from oracle import periln_oracle as PO
+from paper_2606_19025_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("dtype,T,d", [("f32", 257, 200), ("bf16", 1000, 1024), ("bf16", 3, 64), ("f32", 700, 4096)])
+def test_periln_fwd_bwd(dtype, T, d):
+    import torch
+    from paper_2606_19025_b200 import binding as B
+    rng = np.random.default_rng(0)
+    td = torch.bfloat16 if dtype == "bf16" else torch.float32
+    tol = 2e-2 if dtype == "bf16" else 1e-4
+    st = lambda a: W.bf16_round(a) if dtype == "bf16" else a.astype(np.float32)
+    x, res, dout = (st(rng.standard_normal((T, d)) * s + o) for s, o in ((2.0, 0.3), (1.0, 0.0), (1.0, 0.0)))
+    gamma, beta = (rng.standard_normal(d) * 0.2 + 1.0).astype(np.float32), (rng.standard_normal(d) * 0.1).astype(np.float32)
+    dev = lambda a, dt=td: torch.from_numpy(np.ascontiguousarray(a)).cuda().to(dt)
+    xd, rd, dd, gd, bd = dev(x), dev(res), dev(dout), dev(gamma, torch.float32), dev(beta, torch.float32)
+    out, stats = torch.empty_like(xd), torch.empty((T, 2), dtype=torch.float32, device="cuda")
+    alpha = 0.6
+    B.fomoe_periln_fwd(xd, gd, bd, out, stats, residual=rd, alpha=alpha)
+    ref, mean, rstd = PO.periln_post_fwd(res, x, gamma, beta, alpha)
+    assert H.rel_err(H.t2n(out), ref) <= tol
+    assert H.rel_err(H.t2n(stats)[:, 0], mean) <= 1e-5 and H.rel_err(H.t2n(stats)[:, 1], rstd) <= 1e-5
+    dx, dg, db = torch.empty_like(xd), torch.empty(d, device="cuda"), torch.empty(d, device="cuda")
+    part = torch.empty(B.fomoe_periln_workspace_bytes(T, d), dtype=torch.uint8, device="cuda")
+    B.fomoe_periln_bwd(dd, xd, stats, gd, dx, dg, db, part, dresidual=rd, alpha=alpha)
+    torch.cuda.synchronize()
+    dxr, dgr, dbr = PO.ln_bwd(alpha * dout, x, mean, rstd, gamma)
+    assert H.rel_err(H.t2n(dx), dxr + res) <= tol
+    assert H.rel_err(H.t2n(dg), dgr) <= 1e-4 and H.rel_err(H.t2n(db), dbr) <= 1e-4
+    dg1 = dg.clone()
+    B.fomoe_periln_bwd(dd, xd, stats, gd, dx, dg, db, part, dresidual=rd, alpha=alpha)     # fixed-order reduction
+    torch.cuda.synchronize()
+    assert torch.equal(dg, dg1)
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_eq15_block_around_the_moe_layer(oracle64, dtype):
+    """out = x + alpha LN2(MoE(LN1(x))) and its backward, CUDA path vs the two oracles chained the same way."""
+    import torch
+    from paper_2606_19025_b200 import binding as B
+    tol = 2e-2 if dtype == "bf16" else 1e-4
+    td = torch.bfloat16 if dtype == "bf16" else torch.float32
+    st = lambda a: W.bf16_round(a) if dtype == "bf16" else a.astype(np.float32)
+    dev = lambda a, dt=td: torch.from_numpy(np.ascontiguousarray(a)).cuda().to(dt)
+    f32 = torch.float32
+    alpha = 0.8
+    for seed in range(11, 40):      # the first seed whose normalised tokens keep every top-k margin above the bar
+        w = W.MoEWorkload("periln_blk", T=384, d=128, E=8, k=2, F=128, n_res=5, dtype=dtype, gate_fn=W.GATE_SIGMOID,
+                          expert_fn=W.EXPERT_SILU, seed=seed)
+        p = H.Problem(w)
+        rng = np.random.default_rng(seed)
+        x_in = st(rng.standard_normal((w.T, w.d)) * 1.7 + 0.2)
+        g1, b1, g2, b2 = ((rng.standard_normal(w.d) * 0.1 + o).astype(np.float32) for o in (1.0, 0.0, 1.0, 0.0))
+        xd, g1d, b1d, g2d, b2d = dev(x_in), dev(g1, f32), dev(b1, f32), dev(g2, f32), dev(b2, f32)
+        # ---- CUDA path: pre-LN -> route/fwd -> post-LN + residual ----
+        xn = torch.empty_like(xd)
+        s1 = torch.empty((w.T, 2), dtype=f32, device="cuda")
+        s2 = torch.empty_like(s1)
+        B.fomoe_periln_fwd(xd, g1d, b1d, xn, s1)
+        torch.cuda.synchronize()
+        p.x = H.t2n(xn).astype(np.float32)          # the oracle layer consumes the same normalised tokens (storage-exact)
+        r, y_ref, _ = H.oracle_all(p, oracle64, bwd=False)
+        if not (H.margins(r["logits"], w.k) < 2 * H.MARGIN).any():
+            break
+    else:
+        raise AssertionError("no seed with clean margins")
+    layer = H.make_layer(p)
+    layer.route(xn)
+    layer.forward(xn)
+    out = torch.empty_like(xd)
+    B.fomoe_periln_fwd(layer.y, g2d, b2d, out, s2, residual=xd, alpha=alpha)
+    # ---- backward ----
+    dout = st(rng.standard_normal((w.T, w.d)))
+    dd = dev(dout)
+    part = torch.empty(B.fomoe_periln_workspace_bytes(w.T, w.d), dtype=torch.uint8, device="cuda")
+    dy, dx = torch.empty_like(xd), torch.empty_like(xd)
+    dg2, db2, dg1, db1 = (torch.empty(w.d, device="cuda") for _ in range(4))
+    B.fomoe_periln_bwd(dd, layer.y, s2, g2d, dy, dg2, db2, part, alpha=alpha)
+    layer.backward(dy, xn)
+    B.fomoe_periln_bwd(layer.dx, xd, s1, g1d, dx, dg1, db1, part, dresidual=dd)
+    torch.cuda.synchronize()
+    # ---- oracles chained the same way (fp64) ----
+    xn_ref, m1, r1 = PO.ln_fwd(x_in, g1, b1)
+    assert H.rel_err(H.t2n(xn), xn_ref) <= tol
+    out_ref, m2, r2 = PO.periln_post_fwd(x_in, y_ref, g2, b2, alpha)
+    assert H.rel_err(H.t2n(out), out_ref) <= tol
+    dy_ref, dg2_ref, db2_ref = PO.periln_post_bwd(dout, y_ref, m2, r2, g2, alpha)
+    b = oracle64.moe_bwd(p.x, dy_ref, p.w_router, r, p.resident, p.wg, p.wu, p.wd, p.shared, w.gate_fn, w.gate_rule, w.temperature,
+                         expert_fn=w.expert_fn)
+    dx_ref, dg1_ref, db1_ref = PO.periln_pre_bwd(b["dx"], x_in, m1, r1, g1, dout)
+    errs = dict(dy=H.rel_err(H.t2n(dy), dy_ref), dx=H.rel_err(H.t2n(dx), dx_ref), dg2=H.rel_err(H.t2n(dg2), dg2_ref),
+                db2=H.rel_err(H.t2n(db2), db2_ref), dg1=H.rel_err(H.t2n(dg1), dg1_ref), db1=H.rel_err(H.t2n(db1), db1_ref),
+                dw_up=H.rel_err(H.t2n(layer.dw_up), b["dw_up"]), dw_router=H.rel_err(H.t2n(layer.dw_router), b["dw_router"]))
+    print("eq15", dtype, errs)
+    assert all(v <= tol for v in errs.values()), errs
