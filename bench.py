@@ -409,6 +409,25 @@ def run_gpu(args, w, n_res):
             del grads, m1, v1, wc
         except Exception as e:   # never let the side measurements take the headline down
             out["optim"] = {"error": str(e)}
+        # ---- Peri-LN either side of the block (Eq. 15): two streaming row kernels ----
+        try:
+            gam, bet = torch.ones(w.d, device="cuda"), torch.zeros(w.d, device="cuda")
+            stats = torch.empty((w.T, 2), dtype=torch.float32, device="cuda")
+            lo, ldx = torch.empty_like(x), torch.empty_like(x)
+            dgm, dbt = torch.empty(w.d, device="cuda"), torch.empty(w.d, device="cuda")
+            part = torch.empty(B.fomoe_periln_workspace_bytes(w.T, w.d), dtype=torch.uint8, device="cuda")
+            es = x.element_size()
+            ft = timed_steps(lambda: B.fomoe_periln_fwd(x, gam, bet, lo, stats, residual=dy, alpha=0.8), max(args.steps, 10), 3)
+            bt = timed_steps(lambda: B.fomoe_periln_bwd(dy, x, stats, gam, ldx, dgm, dbt, part, dresidual=dy, alpha=0.8), max(args.steps, 10), 3)
+            fms, bms = sum(ft) / len(ft), sum(bt) / len(bt)
+            fby, bby = 3.0 * w.T * w.d * es, 4.0 * w.T * w.d * es       # post-LN + residual: read y, x, write out; bwd: read dout, x, dres, write dx
+            out["periln"] = {"post_fwd": {"bound": "hbm", "achieved": fby / (fms / 1e3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                          "frac": fby / (fms / 1e3) / 1e9 / peaks["hbm_gbs"], "ms": fms, "bytes": fby},
+                             "pre_bwd": {"bound": "hbm", "achieved": bby / (bms / 1e3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                         "frac": bby / (bms / 1e3) / 1e9 / peaks["hbm_gbs"], "ms": bms, "bytes": bby}}
+            del lo, ldx, part
+        except Exception as e:
+            out["periln"] = {"error": str(e)}
         del now, start, payload
 
         # ---- skip-token speed-up against the same kernels with every expert resident ----

@@ -11,7 +11,8 @@ from paper_2606_19025_b200 import workloads as W
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("dtype,T,d", [("f32", 257, 200), ("bf16", 1000, 1024), ("bf16", 3, 64), ("f32", 700, 4096)])
+@pytest.mark.parametrize("dtype,T,d", [("f32", 257, 200), ("bf16", 1000, 1024), ("bf16", 3, 64), ("f32", 700, 4096), ("bf16", 300, 4096),
+                                       ("f32", 130, 50), ("bf16", 77, 36), ("bf16", 40, 10240)])
 def test_periln_fwd_bwd(dtype, T, d):
     import torch
     from paper_2606_19025_b200 import binding as B
