@@ -90,7 +90,7 @@ class ClockSampler:
             try:
                 sm = float(n.nvmlDeviceGetClockInfo(self.handle, n.NVML_CLOCK_SM))
                 r = int(n.nvmlDeviceGetCurrentClocksThrottleReasons(self.handle))
-                self.rows.append((sm, mx, [nm for b, nm in bits if r & b]))
+                self.rows.append((sm, mx, [nm for b, nm in bits if r & b], time.perf_counter()))
             except Exception:
                 pass
             time.sleep(0.002)
@@ -111,11 +111,14 @@ class ClockSampler:
         for line in self.proc.stdout:
             c = [v.strip() for v in line.split(",")]
             try:
-                self.rows.append((float(c[0]), float(c[1]), [nm for nm, v in zip(self.NAMES, c[3:7]) if v.lower().startswith("active")]))
+                self.rows.append((float(c[0]), float(c[1]), [nm for nm, v in zip(self.NAMES, c[3:7]) if v.lower().startswith("active")],
+                                  time.perf_counter()))
             except Exception:
                 continue
 
-    def stop(self):
+    def stop(self, window=None):
+        """window = (t0, t1) perf_counter bounds of the timed region: only samples inside it count (the sampler is started
+        before the warm-up so that a short region still has samples; if none fell inside, the two nearest ones are used)."""
         if self.thread is not None:
             self.stop_flag = True
             self.thread.join()
@@ -126,9 +129,16 @@ class ClockSampler:
             src = "nvidia-smi -lms 100"
         else:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml and nvidia-smi unavailable"]}
-        sm = [r[0] for r in self.rows]
-        mx = [r[1] for r in self.rows]
-        reasons = sorted({nm for r in self.rows for nm in r[2]})
+        rows = self.rows
+        if window is not None and rows:
+            inside = [r for r in rows if window[0] <= r[3] <= window[1]]
+            if not inside:
+                mid = 0.5 * (window[0] + window[1])
+                inside = sorted(rows, key=lambda r: abs(r[3] - mid))[:2]
+            rows = inside
+        sm = [r[0] for r in rows]
+        mx = [r[1] for r in rows]
+        reasons = sorted({nm for r in rows for nm in r[2]})
         # under load = samples in the upper half of what was seen (idle samples at the edges are dropped)
         load = [v for v in sm if v >= 0.5 * max(sm)] if sm else []
         return {"sm_mhz": statistics.median(load) if load else None, "sm_max_mhz": max(mx) if mx else None,
@@ -251,6 +261,8 @@ def run_gpu(args, w, n_res):
         replicas.barrier()
         torch.cuda.synchronize()
 
+    window = [0.0, 0.0]   # perf_counter bounds of the most recent timed region
+
     def timed_steps(fn, steps, warmup, collective=False):
         """Per-step CUDA events on the launching stream; L2 flushed between steps, outside the event pairs.
         collective=True brackets the region with a barrier over all ranks (the headline measurement)."""
@@ -258,6 +270,7 @@ def run_gpu(args, w, n_res):
         for _ in range(warmup):
             fn()
         barrier()
+        window[0] = time.perf_counter()
         evs = []
         for _ in range(steps):
             flush.zero_()
@@ -267,6 +280,7 @@ def run_gpu(args, w, n_res):
             e1.record()
             evs.append((e0, e1))
         barrier()
+        window[1] = time.perf_counter()
         return [a.elapsed_time(b) for a, b in evs]
 
     launches = [0]
@@ -282,7 +296,7 @@ def run_gpu(args, w, n_res):
     sampler = ClockSampler(local)
     sampler.start()
     ms_list = timed_steps(step, args.steps, args.warmup, collective=True)
-    clocks = sampler.stop()
+    clocks = sampler.stop(tuple(window))
     ms = replicas.max_over_ranks(sum(ms_list) / len(ms_list), "cuda")
     value = replicas.whole_job_tokens_per_s(w.T, ms)
 
