@@ -286,22 +286,34 @@ periln_bwd_reg_kernel(const T* __restrict__ dout, const T* __restrict__ x, const
   }
 }
 
-// dgamma / dbeta = sum over the CTAs' partials, in a fixed order: a CTA owns 32 columns; 8 row groups each sum every 8th
-// partial, then group 0 adds the 8 group sums in order
-__global__ void __launch_bounds__(256)
+// dgamma / dbeta = sum over the CTAs' partials, in a fixed order: a CTA owns 32 columns; 32 row groups each sum every 32nd
+// partial (loads batched 4 deep), then group 0 adds the 32 group sums in order
+__global__ void __launch_bounds__(1024)
 periln_reduce_kernel(const float* __restrict__ partials, int n_blk, int d, float* __restrict__ dgamma, float* __restrict__ dbeta) {
-  __shared__ float sg[8][32], sb[8][32];
+  __shared__ float sg[32][33], sb[32][33];
   const int col = threadIdx.x & 31, grp = threadIdx.x >> 5, c = blockIdx.x * 32 + col;
   float g = 0.f, b = 0.f;
-  if (c < d)
-    for (int i = grp; i < n_blk; i += 8) { g += partials[((size_t)i * 2) * d + c]; b += partials[((size_t)i * 2 + 1) * d + c]; }
+  if (c < d) {
+    int i = grp;
+    for (; i + 96 < n_blk; i += 128) {
+      float gv[4], bv[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        gv[u] = partials[((size_t)(i + 32 * u) * 2) * d + c];
+        bv[u] = partials[((size_t)(i + 32 * u) * 2 + 1) * d + c];
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) { g += gv[u]; b += bv[u]; }
+    }
+    for (; i < n_blk; i += 32) { g += partials[((size_t)i * 2) * d + c]; b += partials[((size_t)i * 2 + 1) * d + c]; }
+  }
   sg[grp][col] = g;
   sb[grp][col] = b;
   __syncthreads();
   if (grp == 0 && c < d) {
     float tg = 0.f, tb = 0.f;
 #pragma unroll
-    for (int k = 0; k < 8; ++k) { tg += sg[k][col]; tb += sb[k][col]; }
+    for (int k = 0; k < 32; ++k) { tg += sg[k][col]; tb += sb[k][col]; }
     dgamma[c] = tg;
     dbeta[c] = tb;
   }
@@ -378,7 +390,7 @@ int launch_periln_bwd(int T, int d, int dtype, const void* dout, const void* x, 
                                  : periln_bwd_t<float>(T, d, nb, dout, x, stats, gamma, alpha, dresidual, dx, partials, st);
     if (rc != FOMOE_OK) return rc;
   }
-  periln_reduce_kernel<<<ceil_div(d, 32), 256, 0, st>>>(partials, T > 0 ? nb : 0, d, dgamma, dbeta);
+  periln_reduce_kernel<<<ceil_div(d, 32), 1024, 0, st>>>(partials, T > 0 ? nb : 0, d, dgamma, dbeta);
   FOMOE_LAUNCH_OK("periln_reduce_kernel");
   return FOMOE_OK;
 }
