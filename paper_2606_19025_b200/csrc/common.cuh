@@ -159,12 +159,14 @@ struct ScratchWs {
   void* dsu;       // [T, n_sh*F_sh]
   void* dx_sh;     // [T, d]
   float* dwr_part; // [kRouterSplit, d, Ez] fp32 split-K partials of dW_r
+  float* wg_tail;  // [74 * 2, 128, 256] fp32 K pieces of the tail tiles of the shared-expert weight gradients (umma_gemm.cu)
   void* dz_bf;     // [T, Ez] bf16 dz, Ez = E rounded up to 64 (tensor-core router backward)
   void* wr_bf;     // [d, Ez] bf16 W_r
   int Ez;
   size_t bytes;
 };
 constexpr int kRouterSplit = 32;
+constexpr int kTailSplitMax = 4;
 inline ScratchWs carve_scratch_ws(const fomoe_config& c, int R_cap, void* base) {
   ScratchWs w{};
   size_t es = c.dtype == FOMOE_BF16 ? 2 : 4;
@@ -185,6 +187,7 @@ inline ScratchWs carve_scratch_ws(const fomoe_config& c, int R_cap, void* base) 
   w.dx_sh = take(es * (size_t)c.T * c.d_model);
   w.Ez = (c.E + 63) / 64 * 64;
   w.dwr_part = (float*)take(sizeof(float) * (size_t)kRouterSplit * c.d_model * w.Ez);
+  w.wg_tail = (float*)take(c.n_shared > 0 ? sizeof(float) * (size_t)80 * 2 * 128 * 256 : 0);
   w.dz_bf = take(sizeof(__nv_bfloat16) * (size_t)c.T * w.Ez);
   w.wr_bf = take(sizeof(__nv_bfloat16) * (size_t)c.d_model * w.Ez);
   w.bytes = off;

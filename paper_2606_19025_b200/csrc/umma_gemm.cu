@@ -86,6 +86,11 @@ struct UmmaParams {
   int ksegs;                   // DX: K segments (2: dA W_gate + dU W_up; 1: dA W_up, two-matrix expert)
   int k_chunk;                 // WGRAD dense: > 0 = split-K, group g reduces rows [g*k_chunk, (g+1)*k_chunk)
   float* out_f32;              // WGRAD: if set, fp32 output [n_groups, M, N] instead of out0
+  // WGRAD dense, tail split: the tiles of the last, partially filled round of the persistent schedule (tile ids >= tail_first)
+  // are cut into tail_ks K ranges of tail_chunk rows each, so that round takes 1 / tail_ks of a tile time; the pieces go to
+  // tail_part as fp32 [piece][cta][128][256] and wgrad_tail_fixup_kernel adds them in a fixed order
+  int tail_first, tail_ks, tail_chunk;
+  float* tail_part;
   bf16 *out0, *out1, *out2;    // FWD1: a,u,h | FWD2/DX: out | DH: da,du | WGRAD: dW
   const bf16 *in0, *in1;       // DH: a,u
   RouteEpi r;                  // ROUTE
@@ -159,6 +164,7 @@ struct Tile {
   int slot, part, group;  // group: WGRAD only
   int num_kb;      // 64-wide K blocks
   int k_row0;      // WGRAD: first row of the K range
+  int piece;       // WGRAD tail split: index of this K piece in tail_part, -1 = a whole tile
 };
 
 template <int MODE>
@@ -174,6 +180,7 @@ struct Sched {
       n_tiles_n = (p.N + BN - 1) / BN;
       ntn_total = n_tiles_n;
       total = (long)p.n_groups * m_pairs * n_tiles_n;
+      if (p.tail_ks > 1) total = p.tail_first + (total - p.tail_first) * p.tail_ks;
     } else {
       m_pairs = dense ? (p.dense_rows + 2 * BM - 1) / (2 * BM) : p.n_mtiles[2];
       const int n_extent = (MODE == FWD1 || MODE == FWD1S || MODE == DH) ? p.F : p.d;
@@ -187,6 +194,13 @@ struct Sched {
     Tile t;
     const bool dense = p.n_mtiles == nullptr;
     if (MODE == WGRAD) {
+      t.piece = -1;
+      int kpart = 0;
+      if (p.tail_ks > 1 && id >= p.tail_first) {
+        t.piece = (int)(id - p.tail_first);
+        kpart = t.piece % p.tail_ks;
+        id = p.tail_first + t.piece / p.tail_ks;
+      }
       t.group = (int)(id / ((long)m_pairs * n_tiles_n));
       int rem = (int)(id % ((long)m_pairs * n_tiles_n));
       t.row0 = (rem / n_tiles_n) * 2 * BM + rank * BM;
@@ -199,6 +213,7 @@ struct Sched {
       if (p.pad_offsets) { r0 = p.pad_offsets[t.group]; r1 = p.pad_end64[t.group]; }
       else if (p.k_chunk > 0) { r0 = min(t.group * p.k_chunk, p.dense_rows); r1 = min(r0 + p.k_chunk, p.dense_rows); }
       else { r0 = 0; r1 = p.dense_rows; }
+      if (t.piece >= 0) { r0 = min(kpart * p.tail_chunk, p.dense_rows); r1 = min(r0 + p.tail_chunk, p.dense_rows); }
       t.k_row0 = r0;
       t.num_kb = (r1 - r0 + BK - 1) / BK;
     } else {
@@ -709,6 +724,14 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
 #pragma unroll
             for (int i = 0; i < 32; ++i) v[i] = 0.f;
           }
+          if (t.piece >= 0) {  // K piece of a tail tile: fp32, tile-local layout [piece][cta][128][256]
+            if (lane < rows_valid) {
+              float4* dst = reinterpret_cast<float4*>(p.tail_part + (((size_t)t.piece * 2 + rank) * BM + q * 32 + lane) * BN + cc * 32);
+#pragma unroll
+              for (int i = 0; i < 8; ++i) dst[i] = make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
+            }
+            continue;
+          }
           if (p.out_f32) {  // split-K partials (small): one 128-byte row segment per thread
             if (lane < rows_valid) {
               float4* dst = reinterpret_cast<float4*>(p.out_f32 + ((size_t)t.group * p.M + row0 + lane) * p.N + n);
@@ -806,6 +829,32 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
   cluster_sync_all();
   if (warp == 2) {
     asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kTmemCols) : "memory");
+  }
+}
+
+// Adds the K pieces of the tail tiles (fixed order) and writes them as bf16 into dW.  grid = (tail tiles, 2 CTAs of a pair, 8 row slabs).
+__global__ void __launch_bounds__(256)
+wgrad_tail_fixup_kernel(const float* __restrict__ part, int tail_first, int ks, int m_pairs, int n_tiles_n, int M, int N,
+                        bf16* __restrict__ out) {
+  pdl_launch_dependents();
+  pdl_wait();
+  const int u = blockIdx.x, rank = blockIdx.y;
+  const long tile = (long)tail_first + u;
+  const int group = (int)(tile / ((long)m_pairs * n_tiles_n)), rem = (int)(tile % ((long)m_pairs * n_tiles_n));
+  const int row0 = (rem / n_tiles_n) * 2 * BM + rank * BM, n0 = (rem % n_tiles_n) * BN;
+  // blockIdx.z: 16-row slab of the CTA's 128 rows
+  for (int e = blockIdx.z * 16 * BN + threadIdx.x * 4; e < (blockIdx.z + 1) * 16 * BN; e += 256 * 4) {
+    const int r = e / BN, cidx = e % BN;
+    if (row0 + r >= M || n0 + cidx >= N) continue;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int j = 0; j < ks; ++j) {
+      const float4 v = *reinterpret_cast<const float4*>(part + (((size_t)(u * ks + j) * 2 + rank) * BM + r) * BN + cidx);
+      acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
+    }
+    uint2 o;
+    o.x = pack_bf16x2(acc.x, acc.y);
+    o.y = pack_bf16x2(acc.z, acc.w);
+    *reinterpret_cast<uint2*>(out + ((size_t)group * M + row0 + r) * N + n0 + cidx) = o;
   }
 }
 
@@ -1023,8 +1072,24 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
       m.m[2] = m.m[3] = m.m[0];
       UmmaParams q = p;
       q.n_groups = ns; q.M = j.M; q.N = j.N; q.a_gcol = j.a_gcol; q.b_gcol = j.b_gcol; q.out0 = (bf16*)j.out;
+      // few long tiles (K = T): cut the tiles of the last, partially filled round into K pieces so that it fills the pairs
+      const int m_pairs = ceil_div(j.M, 2 * BM), ntn = ceil_div(j.N, BN), tiles = ns * m_pairs * ntn, pairs = (num_sms() & ~1) / 2;
+      const int tail = tiles % pairs;
+      int ks = tail > 0 ? pairs / tail : 1;
+      if (ks > kTailSplitMax) ks = kTailSplitMax;
+      while (ks > 1 && c.T / ks < 2048) --ks;
+      if (ks > 1 && j.N % 4 == 0) {
+        q.tail_first = tiles - tail; q.tail_ks = ks; q.tail_chunk = ceil_div(ceil_div(c.T, ks), BK) * BK; q.tail_part = sws.wg_tail;
+      } else {
+        ks = 1;
+      }
       int rc = launch<WGRAD>(m, q, st, "umma_grouped_kernel<WGRAD,shared>");
       if (rc != FOMOE_OK) return rc;
+      if (ks > 1) {
+        FOMOE_CUDA_OK(launch_pdl(wgrad_tail_fixup_kernel, dim3(tail, 2, 8), 256, 0, st, (const float*)sws.wg_tail, tiles - tail, ks, m_pairs, ntn,
+                                 j.M, j.N, (bf16*)j.out));
+        FOMOE_LAUNCH_OK("wgrad_tail_fixup_kernel");
+      }
     }
   }
   return FOMOE_OK;
