@@ -210,6 +210,8 @@ def gemm_flops(mode: str, P: int, T: int, w: W.MoEWorkload) -> float:
     shared = "shared" in mode
     rows, F = (T * w.n_sh, w.F_sh) if shared else (P, w.F)
     mult = 4 if (("FWD1" in mode and "FWD1S" not in mode) or ("DX" in mode and w.expert_fn == W.EXPERT_SWIGLU)) else 2
+    if "WGRAD" in mode and not shared:   # one launch computes every weight gradient of the routed experts (dW_down, dW_gate, dW_up)
+        mult = 2 * (3 if w.expert_fn == W.EXPERT_SWIGLU else 2)
     return float(mult) * rows * w.d * F
 
 
@@ -352,7 +354,7 @@ def run_gpu(args, w, n_res):
             kernels.append(k)
         out["kernels"] = kernels
         traffic = None
-        tf = ROOT / "profiles" / "r1d_traffic.csv"   # DRAM bytes per launch from the committed ncu --set full captures
+        tf = ROOT / "profiles" / "r1g_traffic.csv"   # DRAM bytes per launch from the committed ncu --set full captures
         traffic_rows = {}
         if tf.exists():
             for line in tf.read_text().splitlines()[1:]:

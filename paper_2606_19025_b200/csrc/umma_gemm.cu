@@ -55,7 +55,7 @@ __host__ __device__ constexpr int smem_bytes_of(int mode) {
 constexpr int kTmemCols = 512;
 
 struct TmaMaps {
-  CUtensorMap m[4];
+  CUtensorMap m[6];   // WGRAD with several jobs: (A, B) of job j at m[2j], m[2j+1]
 };
 
 // ROUTE mode (rows F1-F4 + the per-block histogram of F5): everything the router epilogue needs
@@ -94,6 +94,12 @@ struct UmmaParams {
   bf16 *out0, *out1, *out2;    // FWD1: a,u,h | FWD2/DX: out | DH: da,du | WGRAD: dW
   const bf16 *in0, *in1;       // DH: a,u
   RouteEpi r;                  // ROUTE
+  // WGRAD, several weight gradients of the same row groups in ONE launch (dW_down, dW_gate, dW_up): n_jobs > 0 overrides
+  // M, N, out0; job j reads tensor maps m[2j] (A) and m[2j+1] (B).  One launch instead of three saves two kernel prologues
+  // and tails and lets the jobs fill each other's last scheduler round.
+  int n_jobs;
+  int job_M[3], job_N[3];
+  bf16* job_out[3];
 };
 
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, bool valid) {
@@ -164,6 +170,8 @@ struct Tile {
   int slot, part, group;  // group: WGRAD only
   int num_kb;      // 64-wide K blocks
   int k_row0;      // WGRAD: first row of the K range
+  int job;         // WGRAD: job index (0 when the launch has a single weight gradient)
+  int M, N;        // WGRAD: output extent of the job
   int piece;       // WGRAD tail split: index of this K piece in tail_part, -1 = a whole tile
 };
 
@@ -181,6 +189,11 @@ struct Sched {
       ntn_total = n_tiles_n;
       total = (long)p.n_groups * m_pairs * n_tiles_n;
       if (p.tail_ks > 1) total = p.tail_first + (total - p.tail_first) * p.tail_ks;
+      if (p.n_jobs > 0) {
+        total = 0;
+        for (int j = 0; j < p.n_jobs; ++j)
+          total += (long)p.n_groups * ((p.job_M[j] + 2 * BM - 1) / (2 * BM)) * ((p.job_N[j] + BN - 1) / BN);
+      }
     } else {
       m_pairs = dense ? (p.dense_rows + 2 * BM - 1) / (2 * BM) : p.n_mtiles[2];
       const int n_extent = (MODE == FWD1 || MODE == FWD1S || MODE == DH) ? p.F : p.d;
@@ -201,13 +214,23 @@ struct Sched {
         kpart = t.piece % p.tail_ks;
         id = p.tail_first + t.piece / p.tail_ks;
       }
-      t.group = (int)(id / ((long)m_pairs * n_tiles_n));
-      int rem = (int)(id % ((long)m_pairs * n_tiles_n));
-      t.row0 = (rem / n_tiles_n) * 2 * BM + rank * BM;
-      t.live = t.row0 < p.M;
+      int mp = m_pairs, ntn = n_tiles_n;
+      t.job = 0; t.M = p.M; t.N = p.N;
+      for (int j = 0; j < p.n_jobs; ++j) {      // which job: tiles are numbered job after job
+        t.job = j; t.M = p.job_M[j]; t.N = p.job_N[j];
+        mp = (t.M + 2 * BM - 1) / (2 * BM);
+        ntn = (t.N + BN - 1) / BN;
+        const long nj = (long)p.n_groups * mp * ntn;
+        if (id < nj) break;
+        id -= nj;
+      }
+      t.group = (int)(id / ((long)mp * ntn));
+      int rem = (int)(id % ((long)mp * ntn));
+      t.row0 = (rem / ntn) * 2 * BM + rank * BM;
+      t.live = t.row0 < t.M;
       t.peer_live = true;
-      t.n_tile = rem % n_tiles_n;
-      t.n_mma = (p.N - t.n_tile * BN <= BN / 2) ? BN / 2 : BN;
+      t.n_tile = rem % ntn;
+      t.n_mma = (t.N - t.n_tile * BN <= BN / 2) ? BN / 2 : BN;
       t.slot = t.part = t.group;
       int r0, r1;
       if (p.pad_offsets) { r0 = p.pad_offsets[t.group]; r1 = p.pad_end64[t.group]; }
@@ -463,6 +486,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
   if (warp == 0 && lane == 0) {
 #pragma unroll
     for (int i = 0; i < 4; ++i) prefetch_tmap(&maps.m[i]);
+    if (MODE == WGRAD && p.n_jobs > 2) { prefetch_tmap(&maps.m[4]); prefetch_tmap(&maps.m[5]); }   // (zero-filled otherwise)
   }
   if (warp == 1 && lane == 0) {
     for (int i = 0; i < kStages; ++i) { mbar_init(smem_u32(&full_bar[i]), 1); mbar_init(smem_u32(&empty_bar[i]), 1); }
@@ -529,10 +553,10 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
           } else {  // WGRAD
             const int r = t.k_row0 + kb * BK;
 #pragma unroll
-            for (int i = 0; i < BM / 64; ++i) tma_load_2d_2sm(sa + i * 8192, &maps.m[0], fb, t.group * p.a_gcol + m0 + 64 * i, r);
+            for (int i = 0; i < BM / 64; ++i) tma_load_2d_2sm(sa + i * 8192, &maps.m[2 * t.job], fb, t.group * p.a_gcol + m0 + 64 * i, r);
 #pragma unroll
             for (int j = 0; j < BN / 128; ++j)
-              tma_load_2d_2sm(sb + j * 8192, &maps.m[1], fb, t.group * p.b_gcol + t.n_tile * BN + rank * nh + 64 * j, r);
+              tma_load_2d_2sm(sb + j * 8192, &maps.m[2 * t.job + 1], fb, t.group * p.b_gcol + t.n_tile * BN + rank * nh + 64 * j, r);
           }
           if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
@@ -712,12 +736,12 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
       const int row0 = t.row0 + q * 32;   // first row (or WGRAD output row m) of this warp
       if (have_acc) { mbar_wait(smem_u32(&tfull_bar[as]), aphase); tc_fence_after(); }
       if (MODE == WGRAD) {
-        const int rows_valid = !t.live ? 0 : min(32, p.M - row0);
-        bf16* obase = p.out0 + ((size_t)t.group * p.M + row0) * p.N;
+        const int rows_valid = !t.live ? 0 : min(32, t.M - row0);
+        bf16* obase = (p.n_jobs > 0 ? p.job_out[t.job] : p.out0) + ((size_t)t.group * t.M + row0) * t.N;
 #pragma unroll 1
         for (int cc = half; cc < BN / 32 && rows_valid > 0; cc += 2) {
           const int n = t.n_tile * BN + cc * 32;
-          if (n >= p.N) break;
+          if (n >= t.N) break;
           float v[32];
           if (have_acc) { tmem_ld32(taddr + cc * 32, v); tmem_ld_wait(); }
           else {
@@ -742,7 +766,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
           }
           stg_put_row(stg0, lane, v);
           __syncwarp();
-          stg_to_global(stg0, obase + n, p.N, lane, rows_valid);
+          stg_to_global(stg0, obase + n, t.N, lane, rows_valid);
           __syncwarp();
         }
       } else {
@@ -1015,14 +1039,18 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
     struct WG { const void* A; int lda; const void* B; int ldb; int M, N; void* out; };
     const WG jobs[3] = {{sws.dop, d, aws.h, F, d, F, dw_down}, {sws.da, F, aws.xp, d, F, d, silu ? dw_up : dw_gate},
                         {sws.du, F, aws.xp, d, F, d, dw_up}};
-    for (int ji = 0; ji < (silu ? 2 : 3); ++ji) {
-      const WG& j = jobs[ji];
+    {   // one launch for all of them (same row groups, same K ranges)
       TmaMaps m{};
-      MAP_OK(make_map(&m.m[0], j.A, j.lda, R, j.lda, 64));
-      MAP_OK(make_map(&m.m[1], j.B, j.ldb, R, j.ldb, 64));
-      m.m[2] = m.m[3] = m.m[0];
       UmmaParams q = p;
-      q.n_groups = n_res; q.M = j.M; q.N = j.N; q.a_gcol = 0; q.b_gcol = 0; q.out0 = (bf16*)j.out;
+      const int nj = silu ? 2 : 3;
+      for (int ji = 0; ji < nj; ++ji) {
+        const WG& j = jobs[ji];
+        MAP_OK(make_map(&m.m[2 * ji], j.A, j.lda, R, j.lda, 64));
+        MAP_OK(make_map(&m.m[2 * ji + 1], j.B, j.ldb, R, j.ldb, 64));
+        q.job_M[ji] = j.M; q.job_N[ji] = j.N; q.job_out[ji] = (bf16*)j.out;
+      }
+      for (int i = 2 * nj; i < 6; ++i) m.m[i] = m.m[0];
+      q.n_jobs = nj; q.n_groups = n_res; q.M = jobs[0].M; q.N = jobs[0].N; q.a_gcol = 0; q.b_gcol = 0; q.out0 = (bf16*)jobs[0].out;
       int rc = launch<WGRAD>(m, q, st, "umma_grouped_kernel<WGRAD>");
       if (rc != FOMOE_OK) return rc;
     }
