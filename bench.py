@@ -201,7 +201,7 @@ def run_reference(args, w, n_res):
 # ------------------------------------------------------------------------------------------------------------------
 # GPU arm
 # ------------------------------------------------------------------------------------------------------------------
-def gemm_flops(mode: str, P: int, T: int, w: W.MoEWorkload) -> float:
+def gemm_flops(mode: str, P: int, T: int, w: W.MoEWorkload, launches_per_step: float = 1.0) -> float:
     """Algorithmic flops of one launch: 2*rows*d*F per GEMM; FWD1 and DX are two GEMMs."""
     if "ROUTE" in mode:    # logits x W_r (the bf16 split of W_r multiplies the tensor work, not the algorithmic flops)
         return 2.0 * T * w.d * w.E
@@ -210,8 +210,9 @@ def gemm_flops(mode: str, P: int, T: int, w: W.MoEWorkload) -> float:
     shared = "shared" in mode
     rows, F = (T * w.n_sh, w.F_sh) if shared else (P, w.F)
     mult = 4 if (("FWD1" in mode and "FWD1S" not in mode) or ("DX" in mode and w.expert_fn == W.EXPERT_SWIGLU)) else 2
-    if "WGRAD" in mode and not shared:   # one launch computes every weight gradient of the routed experts (dW_down, dW_gate, dW_up)
-        mult = 2 * (3 if w.expert_fn == W.EXPERT_SWIGLU else 2)
+    if "WGRAD" in mode:   # one launch computes every weight gradient of the experts (dW_down, dW_gate, dW_up)
+        per = 3 if w.expert_fn == W.EXPERT_SWIGLU else 2
+        mult = 2 * per if (not shared or launches_per_step < 1.5) else 2
     return float(mult) * rows * w.d * F
 
 
@@ -348,7 +349,7 @@ def run_gpu(args, w, n_res):
                 k["frac"] = k["achieved"] / peaks["hbm_gbs"]
                 k["frac_of_nominal_8000"] = k["achieved"] / 8000.0
             elif name.startswith("umma_grouped_kernel"):
-                fl = gemm_flops(name, P, w.T, w)
+                fl = gemm_flops(name, P, w.T, w, n / args.steps)
                 k.update(bound="tensor", achieved=fl / (tt / n / 1e3) / 1e12, unit="TFLOP/s")
                 k["frac"] = k["achieved"] / tc_peak
             kernels.append(k)

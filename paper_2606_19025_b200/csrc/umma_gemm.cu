@@ -98,7 +98,7 @@ struct UmmaParams {
   // M, N, out0; job j reads tensor maps m[2j] (A) and m[2j+1] (B).  One launch instead of three saves two kernel prologues
   // and tails and lets the jobs fill each other's last scheduler round.
   int n_jobs;
-  int job_M[3], job_N[3];
+  int job_M[3], job_N[3], job_agcol[3], job_bgcol[3];   // (per-group column offsets into A / B: dense rows, shared experts)
   bf16* job_out[3];
 };
 
@@ -172,6 +172,7 @@ struct Tile {
   int k_row0;      // WGRAD: first row of the K range
   int job;         // WGRAD: job index (0 when the launch has a single weight gradient)
   int M, N;        // WGRAD: output extent of the job
+  int a_gcol, b_gcol;  // WGRAD: per-group column offsets of the job's operands
   int piece;       // WGRAD tail split: index of this K piece in tail_part, -1 = a whole tile
 };
 
@@ -215,9 +216,9 @@ struct Sched {
         id = p.tail_first + t.piece / p.tail_ks;
       }
       int mp = m_pairs, ntn = n_tiles_n;
-      t.job = 0; t.M = p.M; t.N = p.N;
+      t.job = 0; t.M = p.M; t.N = p.N; t.a_gcol = p.a_gcol; t.b_gcol = p.b_gcol;
       for (int j = 0; j < p.n_jobs; ++j) {      // which job: tiles are numbered job after job
-        t.job = j; t.M = p.job_M[j]; t.N = p.job_N[j];
+        t.job = j; t.M = p.job_M[j]; t.N = p.job_N[j]; t.a_gcol = p.job_agcol[j]; t.b_gcol = p.job_bgcol[j];
         mp = (t.M + 2 * BM - 1) / (2 * BM);
         ntn = (t.N + BN - 1) / BN;
         const long nj = (long)p.n_groups * mp * ntn;
@@ -553,10 +554,10 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
           } else {  // WGRAD
             const int r = t.k_row0 + kb * BK;
 #pragma unroll
-            for (int i = 0; i < BM / 64; ++i) tma_load_2d_2sm(sa + i * 8192, &maps.m[2 * t.job], fb, t.group * p.a_gcol + m0 + 64 * i, r);
+            for (int i = 0; i < BM / 64; ++i) tma_load_2d_2sm(sa + i * 8192, &maps.m[2 * t.job], fb, t.group * t.a_gcol + m0 + 64 * i, r);
 #pragma unroll
             for (int j = 0; j < BN / 128; ++j)
-              tma_load_2d_2sm(sb + j * 8192, &maps.m[2 * t.job + 1], fb, t.group * p.b_gcol + t.n_tile * BN + rank * nh + 64 * j, r);
+              tma_load_2d_2sm(sb + j * 8192, &maps.m[2 * t.job + 1], fb, t.group * t.b_gcol + t.n_tile * BN + rank * nh + 64 * j, r);
           }
           if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
@@ -1047,7 +1048,7 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
         const WG& j = jobs[ji];
         MAP_OK(make_map(&m.m[2 * ji], j.A, j.lda, R, j.lda, 64));
         MAP_OK(make_map(&m.m[2 * ji + 1], j.B, j.ldb, R, j.ldb, 64));
-        q.job_M[ji] = j.M; q.job_N[ji] = j.N; q.job_out[ji] = (bf16*)j.out;
+        q.job_M[ji] = j.M; q.job_N[ji] = j.N; q.job_out[ji] = (bf16*)j.out; q.job_agcol[ji] = 0; q.job_bgcol[ji] = 0;
       }
       for (int i = 2 * nj; i < 6; ++i) m.m[i] = m.m[0];
       q.n_jobs = nj; q.n_groups = n_res; q.M = jobs[0].M; q.N = jobs[0].N; q.a_gcol = 0; q.b_gcol = 0; q.out0 = (bf16*)jobs[0].out;
@@ -1092,7 +1093,27 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
     const WG jobs[3] = {{dy, d, 0, aws.sh, ld, Fs, d, Fs, d_sh_down},
                         {sws.dsa, ld, Fs, x, d, 0, Fs, d, silu ? d_sh_up : d_sh_gate},
                         {sws.dsu, ld, Fs, x, d, 0, Fs, d, d_sh_up}};
-    for (int ji = 0; ji < (silu ? 2 : 3); ++ji) {
+    // All weight gradients in ONE launch when their tiles together fill the scheduler rounds (C3: 3 x 96 tiles = 3.9 rounds of
+    // 74 pairs); otherwise one launch each, with the last round cut into K pieces.
+    const int nj = silu ? 2 : 3, pairs_all = (num_sms() & ~1) / 2;
+    long tiles_all = 0;
+    for (int ji = 0; ji < nj; ++ji) tiles_all += (long)ns * ceil_div(jobs[ji].M, 2 * BM) * ceil_div(jobs[ji].N, BN);
+    const bool merged = (double)tiles_all / (double)(((tiles_all + pairs_all - 1) / pairs_all) * pairs_all) >= 0.85;
+    if (merged) {
+      TmaMaps m{};
+      UmmaParams q = p;
+      for (int ji = 0; ji < nj; ++ji) {
+        const WG& j = jobs[ji];
+        MAP_OK(make_map(&m.m[2 * ji], j.A, j.lda, c.T, j.lda, 64));
+        MAP_OK(make_map(&m.m[2 * ji + 1], j.B, j.ldb, c.T, j.ldb, 64));
+        q.job_M[ji] = j.M; q.job_N[ji] = j.N; q.job_out[ji] = (bf16*)j.out; q.job_agcol[ji] = j.a_gcol; q.job_bgcol[ji] = j.b_gcol;
+      }
+      for (int i = 2 * nj; i < 6; ++i) m.m[i] = m.m[0];
+      q.n_jobs = nj; q.n_groups = ns; q.M = jobs[0].M; q.N = jobs[0].N; q.out0 = (bf16*)jobs[0].out;
+      int rc = launch<WGRAD>(m, q, st, "umma_grouped_kernel<WGRAD,shared>");
+      if (rc != FOMOE_OK) return rc;
+    }
+    for (int ji = 0; ji < (merged ? 0 : nj); ++ji) {
       const WG& j = jobs[ji];
       TmaMaps m{};
       MAP_OK(make_map(&m.m[0], j.A, j.lda, c.T, j.lda, 64));
