@@ -130,6 +130,14 @@ def test_empty_batch_bf16(oracle64):
         assert not t.float().abs().max().item() > 0
 
 
+def test_long_K_shared_wgrad_tail_split(oracle64):
+    """Few, long shared-expert wgrad tiles (K = T = 8192, one 256 x 256 tile per weight matrix): each launch cuts its only
+    round into 4 K pieces that wgrad_tail_fixup_kernel adds in a fixed order."""
+    w = W.MoEWorkload("tail", T=8192, d=256, E=8, k=2, F=128, n_res=2, n_sh=1, F_sh=256, dtype="bf16", seed=12)
+    errs, layer = run_and_compare(H.Problem(w), oracle64)
+    print("tail", errs)
+
+
 def test_routing_is_deterministic(oracle64):
     import torch
     p = H.Problem(W.MoEWorkload("det", T=2048, d=128, E=16, k=2, F=64, n_res=8, dtype="bf16", seed=8))
