@@ -113,7 +113,8 @@ typedef struct fomoe_route_state {
 /*
  * Sizes (bytes) of the three caller-allocated workspaces for (cfg, n_res):
  *   route_internal : fomoe_route_state.internal
- *   saved_acts     : written by fomoe_moe_fwd, read by fomoe_moe_bwd (gathered x rows, a, u, h, o per row)
+ *   saved_acts     : written by fomoe_moe_fwd, read by fomoe_moe_bwd (per padded row: the gathered x row, h, o and the two
+ *                    factors the SwiGLU backward multiplies dh with); opaque to the caller
  *   scratch        : temporary inside one fwd or bwd call (may be shared by both, and across layers)
  * Sizes are worst case (every pair kept): rows = T*k + 127*n_res, rounded up to 128.
  * Any out pointer may be NULL.  Returns FOMOE_ERR_BADARG / FOMOE_ERR_UNSUPPORTED for a config the library rejects.
