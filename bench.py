@@ -484,7 +484,7 @@ def run_gpu(args, w, n_res):
 
         # ---- the oracle, as it stands, on the host cores (reported baseline, not the target) ----
         if not args.no_cpu_baseline:
-            sample = sized_sample(w, n_res, 20.0, args.ref_tokens)     # 10-30 s of CPU work (the probe over-estimates the rate a little)
+            sample = sized_sample(w, n_res, 30.0, args.ref_tokens)     # 10-30 s of CPU work (the probe over-estimates the rate a little)
             times, cores = oracle_sample_time(w, n_res, sample)
             out["cpu_baseline"] = {"value": sample / times[0], "unit": UNIT, "cores": cores, "kind": "oracle",
                                    "sample": f"first {sample} of {w.T} tokens, all {n_res} resident experts' weights, "
