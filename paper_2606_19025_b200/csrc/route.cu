@@ -169,35 +169,43 @@ __global__ void perm_hist_kernel(const int32_t* __restrict__ topk_idx, const int
   for (int i = threadIdx.x; i < n_res; i += blockDim.x) blk_hist[(size_t)blockIdx.x * n_res + i] = hist[i];
 }
 
-// One block.  Per slot: exclusive scan of the per-block counts (in place) -> counts; then offsets, tile-padded
-// offsets, the row-tile -> slot map and the number of tiles in use.  One warp per slot, 32 blocks per shuffle scan.
-__global__ void perm_scan_kernel(int32_t* __restrict__ blk_hist, int n_blk, int n_res, int32_t* __restrict__ counts,
-                                 int32_t* __restrict__ offsets, int32_t* __restrict__ pad_offsets, int32_t* __restrict__ pad_end64,
-                                 int32_t* __restrict__ n_mtiles, int32_t* __restrict__ tile_slot, int32_t* __restrict__ pair_info) {
-  __shared__ int32_t s_pad[kMaxE + 1];
-  __shared__ int32_t s_pair[kMaxE + 1];  // first tile pair of slot s (a pair = two row tiles of ONE slot, the last may be single)
-  __shared__ int32_t s_cnt[kMaxE];
+constexpr int kPermThreads = 256;
+
+// Scan + scatter in ONE launch: every block re-derives, from the per-block histograms, its own exclusive base per slot and
+// the slot totals (n_blk x n_res integers, L2-resident), the offsets by a warp scan over the slots, and then scatters its
+// pairs; block 0 also publishes counts / offsets / padded offsets / K-range ends / tile maps.  Saves the single-block scan
+// launch that sat on the critical path between the router and the gather.
+__global__ void __launch_bounds__(kPermThreads)
+perm_scan_scatter_kernel(const int32_t* __restrict__ topk_idx, const float* __restrict__ gate, const int32_t* __restrict__ slot_of,
+                         const int32_t* __restrict__ blk_hist, int n_blk, long n_pairs, int pairs_per_blk, int k, int n_res,
+                         int32_t* __restrict__ counts, int32_t* __restrict__ offsets, int32_t* __restrict__ pad_offsets,
+                         int32_t* __restrict__ pad_end64, int32_t* __restrict__ n_mtiles, int32_t* __restrict__ tile_slot,
+                         int32_t* __restrict__ pair_info, int32_t* __restrict__ row_token, int32_t* __restrict__ pair_row,
+                         int32_t* __restrict__ prow_token, float* __restrict__ prow_gate, int32_t* __restrict__ prow_pair,
+                         int32_t* __restrict__ pair_prow) {
+  extern __shared__ int32_t sm[];
+  __shared__ int32_t s_cnt[kMaxE], s_off[kMaxE + 1], s_pad[kMaxE + 1], s_pair[kMaxE + 1];
   pdl_launch_dependents();
   pdl_wait();
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, n_warps = blockDim.x >> 5;
+  int32_t* running = sm;                 // [n_res] rows of slot s taken by earlier blocks and by this block so far
+  int32_t* warp_cnt = sm + n_res;        // [8][n_res]
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  constexpr int n_warps = kPermThreads / 32;
+  // (a) this block's exclusive base and the total of every slot
   for (int s = warp; s < n_res; s += n_warps) {
-    int run = 0;
-    for (int b0 = 0; b0 < n_blk; b0 += 32) {
-      const int b = b0 + lane;
-      const int c = b < n_blk ? blk_hist[(size_t)b * n_res + s] : 0;
-      int inc = c;
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const int v = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= o) inc += v;
-      }
-      if (b < n_blk) blk_hist[(size_t)b * n_res + s] = run + inc - c;
-      run += __shfl_sync(0xffffffffu, inc, 31);
+    int base = 0, tot = 0;
+    for (int b = lane; b < n_blk; b += 32) {
+      const int c = blk_hist[(size_t)b * n_res + s];
+      tot += c;
+      if (b < (int)blockIdx.x) base += c;
     }
-    if (lane == 0) { counts[s] = run; s_cnt[s] = run; }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { base += __shfl_xor_sync(0xffffffffu, base, o); tot += __shfl_xor_sync(0xffffffffu, tot, o); }
+    if (lane == 0) { running[s] = base; s_cnt[s] = tot; }
   }
+  for (int i = threadIdx.x; i < 8 * n_res; i += kPermThreads) warp_cnt[i] = 0;
   __syncthreads();
-  // exclusive scans over the slots of (count, padded count, tile pairs): warp 0, 32 slots per shuffle scan
+  // (b) exclusive scans over the slots (warp 0): row offsets, tile-padded offsets, tile pairs
   if (warp == 0) {
     int off = 0, pad = 0, pairs = 0;
     for (int s0 = 0; s0 < n_res; s0 += 32) {
@@ -211,53 +219,36 @@ __global__ void perm_scan_kernel(int32_t* __restrict__ blk_hist, int n_blk, int 
         const int vc = __shfl_up_sync(0xffffffffu, ic, o), vp = __shfl_up_sync(0xffffffffu, ip, o), vq = __shfl_up_sync(0xffffffffu, iq, o);
         if (lane >= o) { ic += vc; ip += vp; iq += vq; }
       }
-      if (s < n_res) {
-        offsets[s] = off + ic - c;
-        pad_offsets[s] = pad + ip - pc;
-        pad_end64[s] = pad + ip - pc + (c + 63) / 64 * 64;
-        s_pad[s] = pad + ip - pc;
-        s_pair[s] = pairs + iq - qc;
-      }
+      if (s < n_res) { s_off[s] = off + ic - c; s_pad[s] = pad + ip - pc; s_pair[s] = pairs + iq - qc; }
       off += __shfl_sync(0xffffffffu, ic, 31);
       pad += __shfl_sync(0xffffffffu, ip, 31);
       pairs += __shfl_sync(0xffffffffu, iq, 31);
     }
-    if (lane == 0) {
-      offsets[n_res] = off;
-      pad_offsets[n_res] = pad;
-      s_pad[n_res] = pad;
-      s_pair[n_res] = pairs;
-      n_mtiles[0] = pad / kTileM;
-      n_mtiles[1] = pad;
-      n_mtiles[2] = pairs;
+    if (lane == 0) { s_off[n_res] = off; s_pad[n_res] = pad; s_pair[n_res] = pairs; }
+  }
+  __syncthreads();
+  if (blockIdx.x == 0) {   // publish
+    for (int s = threadIdx.x; s < n_res; s += kPermThreads) {
+      counts[s] = s_cnt[s];
+      offsets[s] = s_off[s];
+      pad_offsets[s] = s_pad[s];
+      pad_end64[s] = s_pad[s] + (s_cnt[s] + 63) / 64 * 64;
+    }
+    if (threadIdx.x == 0) {
+      offsets[n_res] = s_off[n_res];
+      pad_offsets[n_res] = s_pad[n_res];
+      n_mtiles[0] = s_pad[n_res] / kTileM;
+      n_mtiles[1] = s_pad[n_res];
+      n_mtiles[2] = s_pair[n_res];
+    }
+    for (int s = warp; s < n_res; s += n_warps) {
+      const int t0 = s_pad[s] / kTileM, t1 = s_pad[s + 1] / kTileM;
+      for (int i = t0 + lane; i < t1; i += 32) tile_slot[i] = s;
+      for (int i = lane; i < s_pair[s + 1] - s_pair[s]; i += 32)
+        pair_info[s_pair[s] + i] = 2 * (t0 + 2 * i) + (t0 + 2 * i + 1 < t1 ? 1 : 0);
     }
   }
-  __syncthreads();
-  // row tile -> slot and the pair schedule: one warp per slot
-  for (int s = warp; s < n_res; s += n_warps) {
-    const int t0 = s_pad[s] / kTileM, t1 = s_pad[s + 1] / kTileM;
-    for (int i = t0 + lane; i < t1; i += 32) tile_slot[i] = s;
-    for (int i = lane; i < s_pair[s + 1] - s_pair[s]; i += 32)
-      pair_info[s_pair[s] + i] = 2 * (t0 + 2 * i) + (t0 + 2 * i + 1 < t1 ? 1 : 0);
-  }
-}
-
-constexpr int kPermThreads = 256;
-__global__ void __launch_bounds__(kPermThreads)
-perm_scatter_kernel(const int32_t* __restrict__ topk_idx, const float* __restrict__ gate, const int32_t* __restrict__ slot_of,
-                    const int32_t* __restrict__ blk_base, const int32_t* __restrict__ offsets,
-                    const int32_t* __restrict__ pad_offsets, long n_pairs, int pairs_per_blk, int k, int n_res,
-                    int32_t* __restrict__ row_token, int32_t* __restrict__ pair_row, int32_t* __restrict__ prow_token,
-                    float* __restrict__ prow_gate, int32_t* __restrict__ prow_pair, int32_t* __restrict__ pair_prow) {
-  extern __shared__ int32_t sm[];
-  pdl_launch_dependents();
-  pdl_wait();
-  int32_t* running = sm;                 // [n_res] kept pairs of this block seen so far, per slot
-  int32_t* warp_cnt = sm + n_res;        // [8][n_res]
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  for (int i = threadIdx.x; i < n_res; i += kPermThreads) running[i] = blk_base[(size_t)blockIdx.x * n_res + i];
-  for (int i = threadIdx.x; i < 8 * n_res; i += kPermThreads) warp_cnt[i] = 0;
-  __syncthreads();
+  // (c) stable scatter of this block's pairs
   const long p0 = (long)blockIdx.x * pairs_per_blk;
   for (int it = 0; it < (pairs_per_blk + kPermThreads - 1) / kPermThreads; ++it) {
     const int ip = it * kPermThreads + threadIdx.x;
@@ -272,7 +263,7 @@ perm_scatter_kernel(const int32_t* __restrict__ topk_idx, const float* __restric
       if (s >= 0) {
         int rank = running[s] + rank_in_warp;
         for (int w = 0; w < warp; ++w) rank += warp_cnt[w * n_res + s];
-        int r = offsets[s] + rank, pr = pad_offsets[s] + rank;
+        int r = s_off[s] + rank, pr = s_pad[s] + rank;
         int t = (int)(p / k);
         row_token[r] = t;
         pair_row[p] = r;
@@ -353,13 +344,11 @@ int launch_route(const fomoe_config& c, const void* x, const float* w_router, co
     perm_hist_kernel<<<ws.n_blk, 256, sizeof(int32_t) * nr, st>>>(out.topk_idx, ws.slot_of, n_pairs, pairs_per_blk, n_res, ws.blk_hist);
     FOMOE_LAUNCH_OK("perm_hist_kernel");
   }
-  FOMOE_CUDA_OK(launch_pdl(perm_scan_kernel, 1, 1024, 0, st, ws.blk_hist, ws.n_blk, n_res, out.counts, out.offsets, ws.pad_offsets,
-                           ws.pad_end64, ws.n_mtiles, ws.tile_slot, ws.pair_info));
-  FOMOE_LAUNCH_OK("perm_scan_kernel");
-  FOMOE_CUDA_OK(launch_pdl(perm_scatter_kernel, ws.n_blk, kPermThreads, sizeof(int32_t) * 9 * nr, st, out.topk_idx, out.gate, ws.slot_of,
-                           ws.blk_hist, out.offsets, ws.pad_offsets, n_pairs, pairs_per_blk, c.top_k, n_res, out.row_token, out.pair_row,
-                           ws.prow_token, ws.prow_gate, ws.prow_pair, ws.pair_prow));
-  FOMOE_LAUNCH_OK("perm_scatter_kernel");
+  FOMOE_CUDA_OK(launch_pdl(perm_scan_scatter_kernel, ws.n_blk, kPermThreads, sizeof(int32_t) * 9 * nr, st, out.topk_idx, out.gate, ws.slot_of,
+                           ws.blk_hist, ws.n_blk, n_pairs, pairs_per_blk, c.top_k, n_res, out.counts, out.offsets, ws.pad_offsets, ws.pad_end64,
+                           ws.n_mtiles, ws.tile_slot, ws.pair_info, out.row_token, out.pair_row, ws.prow_token, ws.prow_gate, ws.prow_pair,
+                           ws.pair_prow));
+  FOMOE_LAUNCH_OK("perm_scan_scatter_kernel");
   return FOMOE_OK;
 }
 
