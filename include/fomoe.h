@@ -11,7 +11,7 @@
  *   - Pointers are DEVICE pointers unless the parameter is documented as "host".  The `cfg` structs and
  *     `fomoe_route_state` themselves live on the host; the pointers inside them are device pointers.
  *   - Every buffer is caller-owned.  The library never allocates device memory, frees or keeps a pointer after return.
- *     (Its only own state: one internal non-blocking stream and two events per host thread, created on first use by
+ *     (Its only own state: one internal non-blocking stream and two events per (host thread, device), created on first use by
  *     fomoe_moe_bwd, which forks the router's backward onto it and joins before returning work to `stream`; the fork /
  *     join are event dependencies, so a step stays capturable in a CUDA graph.  FOMOE_SIDE_STREAM=0 disables it.)
  *     Workspace sizes come from fomoe_workspace_bytes().  All device pointers must be 16-byte aligned.
@@ -37,7 +37,7 @@
 extern "C" {
 #endif
 
-#define FOMOE_ABI_VERSION 3
+#define FOMOE_ABI_VERSION 4
 
 #if defined(__GNUC__)
 #define FOMOE_API __attribute__((visibility("default")))
@@ -248,6 +248,39 @@ FOMOE_API int fomoe_moe_step_host(const fomoe_config* cfg, const void* x_host, c
                         float* dw_router, void* dw_gate, void* dw_up, void* dw_down,
                         void* d_sh_gate, void* d_sh_up, void* d_sh_down,
                         void* saved_acts, void* scratch, void* stream, void* copy_stream);
+
+/*
+ * DEBUG: validates the CONTENT of resident_ids ([n_res] int32, device): every id in [0,E), strictly ascending (so no
+ * duplicates).  fomoe_route does not check this because checking needs a device->host copy; THIS call synchronises `stream`.
+ * Returns FOMOE_ERR_BADARG (text via fomoe_last_cuda_error()) for a set fomoe_route must not be given: an out-of-range id
+ * would index the slot map out of bounds.
+ */
+FOMOE_API int fomoe_debug_validate_resident(const int32_t* resident_ids, int32_t n_res, int32_t E, void* stream);
+
+/*
+ * Routing diagnostics from the output of fomoe_route ("routing entropy, load coefficients of variation, and
+ * overflow rates"; under imbalance use "the actual frequency of the token assignments to ghost experts against
+ * the total number of assignments").  The layer is dropless, so there is no overflow rate; the realised kept / ghost
+ * fractions take its place.  Asynchronous on `stream`, no host sync.
+ *   load  [E + 2] int32 device workspace; on return load[e] = assignments (t,j) to expert e over ALL E experts
+ *   stats [FOMOE_N_STATS] fp32 device:
+ *     FOMOE_STAT_KEPT_FRACTION     P / (T k)            (the realised sigma_st of PAPER.md:200 Eq. 2)
+ *     FOMOE_STAT_GHOST_FRACTION    1 - P / (T k)
+ *     FOMOE_STAT_ZERO_KEPT_TOKENS  fraction of tokens none of whose k experts is resident
+ *     FOMOE_STAT_LOAD_CV           std(load) / mean(load) over the E experts (population std)
+ *     FOMOE_STAT_ROUTING_ENTROPY   -sum_e f_e ln f_e, f_e = load[e] / (T k)   (nats; ln E when perfectly balanced)
+ *     FOMOE_STAT_MAX_LOAD / FOMOE_STAT_MIN_LOAD
+ */
+#define FOMOE_STAT_KEPT_FRACTION 0
+#define FOMOE_STAT_GHOST_FRACTION 1
+#define FOMOE_STAT_ZERO_KEPT_TOKENS 2
+#define FOMOE_STAT_LOAD_CV 3
+#define FOMOE_STAT_ROUTING_ENTROPY 4
+#define FOMOE_STAT_MAX_LOAD 5
+#define FOMOE_STAT_MIN_LOAD 6
+#define FOMOE_N_STATS 8
+FOMOE_API int fomoe_routing_stats(const fomoe_config* cfg, const fomoe_route_state* route, int32_t n_res, int32_t* load, float* stats,
+                        void* stream);
 
 /* Number of kernels the last call on this thread launched (bench.py's gpu_launches). */
 FOMOE_API int fomoe_last_launch_count(void);

@@ -27,7 +27,9 @@ FOMOE_ROUTE_SKIP_TOKEN, FOMOE_ROUTE_FORCED_LOCAL = 0, 1
 EXPORTS = ("fomoe_workspace_bytes", "fomoe_route", "fomoe_moe_fwd", "fomoe_moe_bwd", "fomoe_pack_resident_deltas",
            "fomoe_adamw_resident", "fomoe_outer_nesterov", "fomoe_periln_workspace_bytes", "fomoe_periln_fwd", "fomoe_periln_bwd",
            "fomoe_moe_step_host", "fomoe_last_launch_count", "fomoe_last_cuda_error", "fomoe_abi_version",
-           "fomoe_set_force_simt", "fomoe_profile_enable", "fomoe_profile_collect")
+           "fomoe_set_force_simt", "fomoe_profile_enable", "fomoe_profile_collect", "fomoe_debug_validate_resident",
+           "fomoe_routing_stats")
+STAT_NAMES = ("kept_fraction", "ghost_fraction", "zero_kept_tokens", "load_cv", "routing_entropy", "max_load", "min_load")
 
 
 class fomoe_config(C.Structure):
@@ -58,7 +60,7 @@ def lib() -> C.CDLL:
         for name in EXPORTS:
             getattr(_lib, name).restype = C.c_int
         _lib.fomoe_last_cuda_error.restype = C.c_char_p
-        if _lib.fomoe_abi_version() != 3:
+        if _lib.fomoe_abi_version() != 4:
             raise FomoeError("libfomoe.so ABI version mismatch")
     return _lib
 
@@ -229,6 +231,19 @@ def fomoe_moe_step_host(cfg, x_host, dy_host, y_host, dx_host, x_dev, dy_dev, y_
         _p(router_bias), _p(resident_ids), C.c_int32(n_res), C.byref(rs), _p(w_gate), _p(w_up), _p(w_down), _p(sg), _p(su), _p(sd),
         _p(dw_router), _p(dw_gate), _p(dw_up), _p(dw_down), _p(dsg), _p(dsu), _p(dsd), _p(saved_acts), _p(scratch),
         _stream(stream), _stream(copy_stream if copy_stream is not None else stream)), "fomoe_moe_step_host")
+
+
+def fomoe_debug_validate_resident(resident_ids, E: int, stream=None) -> None:
+    """Synchronising content check of the resident set; raises FomoeError (BADARG) on out-of-range / duplicate / unsorted ids."""
+    _check(lib().fomoe_debug_validate_resident(_p(resident_ids), C.c_int32(int(resident_ids.numel())), C.c_int32(E), _stream(stream)),
+           "fomoe_debug_validate_resident")
+
+
+def fomoe_routing_stats(cfg, route: RouteState, n_res: int, load: torch.Tensor, stats: torch.Tensor, stream=None) -> None:
+    """load: int32 [E + 2], stats: fp32 [8] device tensors (see include/fomoe.h)."""
+    rs = route.c_struct()
+    _check(lib().fomoe_routing_stats(C.byref(cfg), C.byref(rs), C.c_int32(n_res), _p(load), _p(stats), _stream(stream)),
+           "fomoe_routing_stats")
 
 
 def fomoe_last_launch_count() -> int:

@@ -3,6 +3,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <atomic>
 #include <vector>
 
 #include "common.cuh"
@@ -11,7 +12,7 @@ namespace fomoe {
 
 static thread_local char g_err[512] = "";
 static thread_local int g_launches = 0;
-static int g_force_simt = 0;
+static std::atomic<int> g_force_simt{0};
 
 // optional per-kernel timing: one event after every launch (+ a marker at each entry point); kernel i's time is the
 // interval since the previous event on the same stream
@@ -40,11 +41,12 @@ int set_cuda_error(cudaError_t e, const char* where) {
 // router's backward chain (gate_bwd, dz W_r^T, x^T dz) beside the expert GEMMs.  Fork / join through events, so the pattern
 // is capturable in a CUDA graph.  FOMOE_SIDE_STREAM=0 in the environment turns it off.
 struct SideStream {
-  int dev = -1;
   cudaStream_t s = nullptr;
   cudaEvent_t fork = nullptr, join = nullptr;
+  bool ok = false;
 };
-static thread_local SideStream g_side;
+constexpr int kMaxDevices = 64;
+static thread_local SideStream g_side[kMaxDevices];   // one per (host thread, device): a device switch creates, never leaks
 static bool side_enabled() {
   static const bool on = [] { const char* e = getenv("FOMOE_SIDE_STREAM"); return !(e && e[0] == '0'); }();
   return on;
@@ -52,16 +54,15 @@ static bool side_enabled() {
 static SideStream* side_stream() {
   if (!side_enabled() || g_prof_on) return nullptr;   // per-kernel timing needs one serial stream
   int dev = -1;
-  if (cudaGetDevice(&dev) != cudaSuccess) return nullptr;
-  if (g_side.dev != dev) {
-    g_side = SideStream{};
-    if (cudaStreamCreateWithFlags(&g_side.s, cudaStreamNonBlocking) != cudaSuccess) return nullptr;
-    if (cudaEventCreateWithFlags(&g_side.fork, cudaEventDisableTiming) != cudaSuccess ||
-        cudaEventCreateWithFlags(&g_side.join, cudaEventDisableTiming) != cudaSuccess)
-      return nullptr;
-    g_side.dev = dev;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return nullptr;
+  SideStream& sd = g_side[dev];
+  if (!sd.ok) {
+    if (!sd.s && cudaStreamCreateWithFlags(&sd.s, cudaStreamNonBlocking) != cudaSuccess) return nullptr;
+    if (!sd.fork && cudaEventCreateWithFlags(&sd.fork, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+    if (!sd.join && cudaEventCreateWithFlags(&sd.join, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+    sd.ok = true;
   }
-  return &g_side;
+  return &sd;
 }
 
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -100,7 +101,7 @@ extern "C" {
 int fomoe_abi_version(void) { return FOMOE_ABI_VERSION; }
 const char* fomoe_last_cuda_error(void) { return g_err; }
 int fomoe_last_launch_count(void) { return g_launches; }
-int fomoe_set_force_simt(int on) { int p = g_force_simt; g_force_simt = on ? 1 : 0; return p; }
+int fomoe_set_force_simt(int on) { return g_force_simt.exchange(on ? 1 : 0); }
 
 int fomoe_profile_enable(int on) {
   for (auto& r : g_prof) cudaEventDestroy(r.ev);
@@ -222,21 +223,28 @@ int fomoe_moe_bwd(const fomoe_config* cfg, const void* dy, const void* x, const 
     return tc_router ? umma_router_bwd(*cfg, x, w_router, route_umma_supported(*cfg) ? rws.wr_bf : nullptr, sws, dw_router, rst)
                      : simt_router_bwd(*cfg, x, w_router, sws, dw_router, rst);
   };
+  // everything between the fork and the join: whatever it returns, the side stream is joined back into `st` afterwards (an
+  // error return must not leave a forked stream dangling, least of all inside a stream capture)
+  auto forked_region = [&]() -> int {
+    int r = FOMOE_OK;
+    if (side) {
+      r = router_bwd();
+      if (r != FOMOE_OK) return r;
+    }
+    // B2-B4 (+ shared experts)
+    r = use_umma(*cfg) ? umma_ffn_bwd(*cfg, n_res, x, dy, rws, aws, sws, w, dw_gate, dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, st)
+                       : simt_ffn_bwd(*cfg, n_res, x, dy, rws, aws, sws, w, dw_gate, dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, st);
+    if (r != FOMOE_OK) return r;
+    return side ? FOMOE_OK : router_bwd();
+  };
+  rc = forked_region();
   if (side) {
-    rc = router_bwd();
-    if (rc != FOMOE_OK) return rc;
-    FOMOE_CUDA_OK(cudaEventRecord(side->join, side->s));
+    cudaError_t e1 = cudaEventRecord(side->join, side->s);
+    cudaError_t e2 = cudaStreamWaitEvent(st, side->join, 0);
+    if (rc == FOMOE_OK && e1 != cudaSuccess) return set_cuda_error(e1, "cudaEventRecord(join)");
+    if (rc == FOMOE_OK && e2 != cudaSuccess) return set_cuda_error(e2, "cudaStreamWaitEvent(join)");
   }
-  // B2-B4 (+ shared experts)
-  rc = use_umma(*cfg) ? umma_ffn_bwd(*cfg, n_res, x, dy, rws, aws, sws, w, dw_gate, dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, st)
-                      : simt_ffn_bwd(*cfg, n_res, x, dy, rws, aws, sws, w, dw_gate, dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, st);
   if (rc != FOMOE_OK) return rc;
-  if (side) {
-    FOMOE_CUDA_OK(cudaStreamWaitEvent(st, side->join, 0));
-  } else {
-    rc = router_bwd();
-    if (rc != FOMOE_OK) return rc;
-  }
   // B5
   return launch_dx_sum(*cfg, rws, sws.dxp, cfg->n_shared > 0 ? sws.dx_sh : nullptr, tc_router ? nullptr : sws.dx_r,
                        tc_router ? (const void*)sws.dx_r : nullptr, dx, st);
@@ -258,6 +266,20 @@ int fomoe_pack_resident_deltas(const float* const w_now[3], const float* const w
   if (elems_gate % 4 || elems_up % 4 || elems_down % 4) return FOMOE_ERR_UNSUPPORTED;
   note_api_entry("@fomoe_pack_resident_deltas", (cudaStream_t)stream);
   return launch_pack(w_now, w_start, n_res, elems_gate, elems_up, elems_down, pack_slots, n_pack, payload, (cudaStream_t)stream);
+}
+
+int fomoe_debug_validate_resident(const int32_t* resident_ids, int32_t n_res, int32_t E, void* stream) {
+  if (n_res < 0 || E <= 0 || n_res > E || (n_res > 0 && !resident_ids)) return FOMOE_ERR_BADARG;
+  return validate_resident(resident_ids, n_res, E, (cudaStream_t)stream, g_err, sizeof(g_err));
+}
+
+int fomoe_routing_stats(const fomoe_config* cfg, const fomoe_route_state* route, int32_t n_res, int32_t* load, float* stats,
+                        void* stream) {
+  g_launches = 0;
+  int rc = check_cfg(cfg, n_res);
+  if (rc != FOMOE_OK) return rc;
+  if (!route || !load || !stats || !route->offsets || (cfg->T > 0 && (!route->topk_idx || !route->pair_row))) return FOMOE_ERR_BADARG;
+  return launch_routing_stats(*cfg, *route, n_res, load, stats, (cudaStream_t)stream);
 }
 
 int fomoe_periln_workspace_bytes(int32_t T, int32_t d_model, size_t* partials) {
@@ -338,40 +360,48 @@ int fomoe_moe_step_host(const fomoe_config* cfg, const void* x_host, const void*
   cudaStream_t st = (cudaStream_t)stream, cs = (cudaStream_t)copy_stream;
   const size_t bytes = (size_t)cfg->T * cfg->d_model * (cfg->dtype == FOMOE_BF16 ? 2 : 4);
   int launches = 0;
-  cudaEvent_t ev_start, ev_dy, ev_y;
-  FOMOE_CUDA_OK(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
-  FOMOE_CUDA_OK(cudaEventCreateWithFlags(&ev_dy, cudaEventDisableTiming));
-  FOMOE_CUDA_OK(cudaEventCreateWithFlags(&ev_y, cudaEventDisableTiming));
+  struct Events {   // destroyed on every exit path
+    cudaEvent_t start = nullptr, dy = nullptr, y = nullptr;
+    ~Events() {
+      if (start) cudaEventDestroy(start);
+      if (dy) cudaEventDestroy(dy);
+      if (y) cudaEventDestroy(y);
+    }
+  } ev;
+  FOMOE_CUDA_OK(cudaEventCreateWithFlags(&ev.start, cudaEventDisableTiming));
+  FOMOE_CUDA_OK(cudaEventCreateWithFlags(&ev.dy, cudaEventDisableTiming));
+  FOMOE_CUDA_OK(cudaEventCreateWithFlags(&ev.y, cudaEventDisableTiming));
   // copy stream starts after everything already queued on the compute stream (previous step's consumers)
-  FOMOE_CUDA_OK(cudaEventRecord(ev_start, st));
-  FOMOE_CUDA_OK(cudaStreamWaitEvent(cs, ev_start, 0));
+  FOMOE_CUDA_OK(cudaEventRecord(ev.start, st));
+  FOMOE_CUDA_OK(cudaStreamWaitEvent(cs, ev.start, 0));
   FOMOE_CUDA_OK(cudaMemcpyAsync(x_dev, x_host, bytes, cudaMemcpyHostToDevice, st));
   FOMOE_CUDA_OK(cudaMemcpyAsync(dy_dev, dy_host, bytes, cudaMemcpyHostToDevice, cs));  // overlaps route + forward
-  FOMOE_CUDA_OK(cudaEventRecord(ev_dy, cs));
-  rc = fomoe_route(cfg, x_dev, w_router, router_bias, resident_ids, n_res, route, st);
-  launches += g_launches;
-  if (rc == FOMOE_OK) {
-    rc = fomoe_moe_fwd(cfg, x_dev, route, n_res, w_gate, w_up, w_down, sh_gate, sh_up, sh_down, y_dev, saved_acts, scratch, st);
+  FOMOE_CUDA_OK(cudaEventRecord(ev.dy, cs));
+  // whatever happens below, `st` waits for the copy stream before this call returns (no dangling fork)
+  auto body = [&]() -> int {
+    int r = fomoe_route(cfg, x_dev, w_router, router_bias, resident_ids, n_res, route, st);
     launches += g_launches;
-  }
-  if (rc == FOMOE_OK) {
-    FOMOE_CUDA_OK(cudaEventRecord(ev_y, st));
-    FOMOE_CUDA_OK(cudaStreamWaitEvent(cs, ev_y, 0));
+    if (r != FOMOE_OK) return r;
+    r = fomoe_moe_fwd(cfg, x_dev, route, n_res, w_gate, w_up, w_down, sh_gate, sh_up, sh_down, y_dev, saved_acts, scratch, st);
+    launches += g_launches;
+    if (r != FOMOE_OK) return r;
+    FOMOE_CUDA_OK(cudaEventRecord(ev.y, st));
+    FOMOE_CUDA_OK(cudaStreamWaitEvent(cs, ev.y, 0));
     FOMOE_CUDA_OK(cudaMemcpyAsync(y_host, y_dev, bytes, cudaMemcpyDeviceToHost, cs));  // overlaps backward
-    FOMOE_CUDA_OK(cudaStreamWaitEvent(st, ev_dy, 0));
-    rc = fomoe_moe_bwd(cfg, dy_dev, x_dev, route, n_res, w_router, w_gate, w_up, w_down, sh_gate, sh_up, sh_down, saved_acts, dx_dev,
-                       dw_router, dw_gate, dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, scratch, st);
+    FOMOE_CUDA_OK(cudaStreamWaitEvent(st, ev.dy, 0));
+    r = fomoe_moe_bwd(cfg, dy_dev, x_dev, route, n_res, w_router, w_gate, w_up, w_down, sh_gate, sh_up, sh_down, saved_acts, dx_dev,
+                      dw_router, dw_gate, dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, scratch, st);
     launches += g_launches;
-  }
-  if (rc == FOMOE_OK) {
+    if (r != FOMOE_OK) return r;
     FOMOE_CUDA_OK(cudaMemcpyAsync(dx_host, dx_dev, bytes, cudaMemcpyDeviceToHost, st));
-    // join: the step is complete on `stream` only when the y download is
-    FOMOE_CUDA_OK(cudaEventRecord(ev_y, cs));
-    FOMOE_CUDA_OK(cudaStreamWaitEvent(st, ev_y, 0));
-  }
-  cudaEventDestroy(ev_start);
-  cudaEventDestroy(ev_dy);
-  cudaEventDestroy(ev_y);
+    return FOMOE_OK;
+  };
+  rc = body();
+  // join: the step is complete on `stream` only when the copy stream's work (dy upload, y download) is
+  cudaError_t e1 = cudaEventRecord(ev.y, cs);
+  cudaError_t e2 = cudaStreamWaitEvent(st, ev.y, 0);
+  if (rc == FOMOE_OK && e1 != cudaSuccess) rc = set_cuda_error(e1, "cudaEventRecord(copy join)");
+  if (rc == FOMOE_OK && e2 != cudaSuccess) rc = set_cuda_error(e2, "cudaStreamWaitEvent(copy join)");
   g_launches = launches;
   return rc;
 }

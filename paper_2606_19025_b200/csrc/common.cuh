@@ -53,6 +53,30 @@ inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, siz
   return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 
+// ---- per-device facts (a process may drive several GPUs; host threads may race: the values written are idempotent) ----
+constexpr int kMaxDev = 64;
+inline int current_device() {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDev) dev = 0;
+  return dev;
+}
+inline int num_sms() {   // SM count of the CURRENT device
+  static int n[kMaxDev] = {};
+  const int dev = current_device();
+  if (n[dev] == 0) {
+    int v = 148;
+    cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
+    n[dev] = v;
+  }
+  return n[dev];
+}
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is per device: one flag per (kernel instantiation, device)
+struct PerDeviceOnce {
+  bool done[kMaxDev] = {};
+  bool need() const { return !done[current_device()]; }
+  void set() { done[current_device()] = true; }
+};
+
 inline __host__ __device__ int ceil_div(int a, int b) { return (a + b - 1) / b; }
 inline __host__ __device__ size_t align_up(size_t a, size_t b) { return (a + b - 1) / b * b; }
 
@@ -159,7 +183,7 @@ struct ScratchWs {
   void* dsu;       // [T, n_sh*F_sh]
   void* dx_sh;     // [T, d]
   float* dwr_part; // [kRouterSplit, d, Ez] fp32 split-K partials of dW_r
-  float* wg_tail;  // [74 * 2, 128, 256] fp32 K pieces of the tail tiles of the shared-expert weight gradients (umma_gemm.cu)
+  float* wg_tail;  // [SMs / 2 tail tiles * 2 CTAs, 128, 256] fp32 K pieces of the tail tiles of the shared-expert weight gradients (umma_gemm.cu)
   void* dz_bf;     // [T, Ez] bf16 dz, Ez = E rounded up to 64 (tensor-core router backward)
   void* wr_bf;     // [d, Ez] bf16 W_r
   int Ez;
@@ -187,7 +211,7 @@ inline ScratchWs carve_scratch_ws(const fomoe_config& c, int R_cap, void* base) 
   w.dx_sh = take(es * (size_t)c.T * c.d_model);
   w.Ez = (c.E + 63) / 64 * 64;
   w.dwr_part = (float*)take(sizeof(float) * (size_t)kRouterSplit * c.d_model * w.Ez);
-  w.wg_tail = (float*)take(c.n_shared > 0 ? sizeof(float) * (size_t)80 * 2 * 128 * 256 : 0);
+  w.wg_tail = (float*)take(c.n_shared > 0 ? sizeof(float) * (size_t)(num_sms() / 2 + 1) * 2 * 128 * 256 : 0);   // < SMs / 2 tail tiles, each cut into pieces that together fill the pairs
   w.dz_bf = take(sizeof(__nv_bfloat16) * (size_t)c.T * w.Ez);
   w.wr_bf = take(sizeof(__nv_bfloat16) * (size_t)c.d_model * w.Ez);
   w.bytes = off;
@@ -242,6 +266,10 @@ int umma_route(const fomoe_config& c, const void* x, const void* wr_split, int N
 // wr_bf: W_r already rounded to bf16 [d, Ez] by the tensor-core router's preparation kernel, or nullptr (converted here)
 int umma_router_bwd(const fomoe_config& c, const void* x, const float* w_router, const void* wr_bf, const ScratchWs& sws,
                     float* dw_router, cudaStream_t st);
+
+// diagnostics (diag.cu)
+int launch_routing_stats(const fomoe_config& c, const fomoe_route_state& r, int n_res, int32_t* load, float* stats, cudaStream_t st);
+int validate_resident(const int32_t* resident_ids, int n_res, int E, cudaStream_t st, char* msg, size_t msg_len);
 
 int launch_pack(const float* const w_now[3], const float* const w_start[3], int n_res, int64_t eg, int64_t eu, int64_t ed,
                 const int32_t* pack_slots, int n_pack, float* payload, cudaStream_t st);

@@ -119,7 +119,7 @@ int launch_adamw(float* const w[3], const void* const g[3], float* const m[3], f
   a.inv_bc1 = (float)(1.0 / (1.0 - pow((double)b1, (double)step)));
   a.inv_bc2 = (float)(1.0 / (1.0 - pow((double)b2, (double)step)));
   long gx = (nmax / 4 + kOptThreads - 1) / kOptThreads;
-  if (gx > 148L * 8) gx = 148L * 8;
+  if (gx > (long)num_sms() * 8) gx = (long)num_sms() * 8;
   dim3 grid((unsigned)gx, 3);
   if (dtype == FOMOE_BF16) adamw_kernel<true><<<grid, kOptThreads, 0, st>>>(a);
   else adamw_kernel<false><<<grid, kOptThreads, 0, st>>>(a);
@@ -141,7 +141,7 @@ int launch_outer_nesterov(float* const w_start[3], float* const w_now[3], float*
   }
   a.block = off; a.lr = lr; a.mu = mu;
   if (nmax == 0) return FOMOE_OK;
-  long gx = (nmax / 4 + kOptThreads - 1) / kOptThreads, want = (148L * 16 + 3L * n_pack - 1) / (3L * n_pack);
+  long gx = (nmax / 4 + kOptThreads - 1) / kOptThreads, want = ((long)num_sms() * 16 + 3L * n_pack - 1) / (3L * n_pack);
   if (gx > want) gx = want;
   if (gx < 1) gx = 1;
   dim3 grid((unsigned)gx, (unsigned)n_pack, 3);

@@ -95,7 +95,7 @@ int launch_pack(const float* const w_now[3], const float* const w_start[3], int 
   const long per_block = (long)kPackThreads * kPackUnroll;
   long gx = (maxvec + per_block - 1) / per_block;
   // ~16 CTAs per SM in total keeps enough bytes in flight
-  long want = (148L * 16 + (long)n_pack * 3 - 1) / ((long)n_pack * 3);
+  long want = ((long)num_sms() * 16 + (long)n_pack * 3 - 1) / ((long)n_pack * 3);
   if (gx > want) gx = want;
   if (gx < 1) gx = 1;
   dim3 grid((unsigned)gx, (unsigned)n_pack, 3);

@@ -321,7 +321,7 @@ periln_reduce_kernel(const float* __restrict__ partials, int n_blk, int d, float
 
 }  // namespace
 
-int periln_blocks(int T) { int g = 148 * 8; if (g > T) g = T; return g < 1 ? 1 : g; }
+int periln_blocks(int T) { int g = num_sms() * 8; if (g > T) g = T; return g < 1 ? 1 : g; }
 
 // threads per CTA and vectors per thread needed to hold one row in registers; nv = 0: use the shared-memory kernels
 template <typename T> static void reg_shape(int d, int& threads, int& nv) {
@@ -341,7 +341,7 @@ static int periln_fwd_t(int Tn, int d, const void* x, const float* gamma, const 
                         void* out, float* stats, cudaStream_t st) {
   int threads, nv;
   reg_shape<T>(d, threads, nv);
-  const int grid = Tn < 148 * 16 ? Tn : 148 * 16;
+  const int grid = Tn < num_sms() * 16 ? Tn : num_sms() * 16;
 #define LN_FWD(NV) periln_fwd_reg_kernel<T, NV><<<grid, threads, 0, st>>>((const T*)x, gamma, beta, (const T*)residual, alpha, eps, Tn, d, (T*)out, stats)
   if (nv == 1) LN_FWD(1);
   else if (nv == 2) LN_FWD(2);

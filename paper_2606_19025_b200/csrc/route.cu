@@ -128,6 +128,9 @@ route_kernel(const XT* __restrict__ x, const float* __restrict__ w_r, const floa
         int oe = __shfl_xor_sync(0xffffffffu, be, o);
         if (ov > bv || (ov == bv && oe < be)) { bv = ov; be = oe; }
       }
+      // fewer than k logits compare greater than -inf (NaN / inf activations, a -inf bias): no candidate left.  Keep the id in
+      // range so that nothing downstream indexes with the sentinel; such a pair carries the probability of that expert
+      if (be >= E) be = E - 1;
       // owner lane marks it taken and publishes p
       float pe = 0.f;
 #pragma unroll

@@ -44,7 +44,7 @@ constexpr int kRowThreads = 128;
 // CTAs of a row kernel: 16 per SM when the tensor is small (each CTA then loops over a few rows and the launch stays cheap),
 // 64 per SM from ~24 M elements on (more rows in flight per SM: +5-10 % of HBM bandwidth on C3 / C5, measured)
 static int row_grid(long rows, int d = 0) {
-  const long cap = (rows * (long)d >= 24L * 1000 * 1000) ? 148L * 64 : 148L * 16;
+  const long cap = (rows * (long)d >= 24L * 1000 * 1000) ? (long)num_sms() * 64 : (long)num_sms() * 16;
   long g = rows < cap ? rows : cap;
   return (int)(g < 1 ? 1 : g);
 }

@@ -382,6 +382,12 @@ __device__ __forceinline__ void route_tile_epilogue(const UmmaParams& p, RouteSm
         }
       }
     }
+    // fewer than k logits compare greater than -inf (NaN / inf activations, a -inf bias): the list still holds the sentinel id.
+    // Keep every id in range so that neither the slot lookup below nor the permutation kernels index with it
+    if (half == 0) {
+#pragma unroll
+      for (int j = 0; j < KMAX; ++j) ti[j] = min(ti[j], E - 1);
+    }
     // pass 2 (softmax): denominator, summed as (half 0) + (half 1) by both warps
     float inv_s = 1.f;
     if (softmax) {
@@ -888,10 +894,10 @@ wgrad_tail_fixup_kernel(const float* __restrict__ part, int tail_first, int ks, 
 // ---------------------------------------------------------------------------------------------------------
 template <int MODE, int KMAX = 0>
 int launch(const TmaMaps& maps, const UmmaParams& p, cudaStream_t st, const char* name) {
-  static bool attr_set = false;
-  if (!attr_set) {
+  static PerDeviceOnce attr;
+  if (attr.need()) {
     FOMOE_CUDA_OK(cudaFuncSetAttribute(umma_grouped_kernel<MODE, KMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes_of(MODE)));
-    attr_set = true;
+    attr.set();
   }
   FOMOE_CUDA_OK(launch_pdl(umma_grouped_kernel<MODE, KMAX>, num_sms() & ~1, kThreads, smem_bytes_of(MODE), st, maps, p));
   FOMOE_LAUNCH_OK(name);

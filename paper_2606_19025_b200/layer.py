@@ -112,6 +112,17 @@ class SkipTokenMoE:
         return out
 
 
+    def routing_stats(self, stream=None) -> dict:
+        """Routing diagnostics of the last route() (fomoe_routing_stats): device kernel, read back here."""
+        load = torch.empty(self.w.E + 2, dtype=torch.int32, device=self.device)
+        stats = torch.empty(8, dtype=torch.float32, device=self.device)
+        B.fomoe_routing_stats(self.cfg, self.route_state, self.n_res, load, stats, stream)
+        vals = stats.cpu().tolist()
+        out = dict(zip(B.STAT_NAMES, vals))
+        out["load"] = load[:self.w.E].cpu().numpy()
+        return out
+
+
 def pack_resident_deltas(w_now, w_start, pack_slots: Optional[torch.Tensor] = None, payload: Optional[torch.Tensor] = None,
                          stream=None) -> torch.Tensor:
     """fp32 payload [n_pack, elems_gate + elems_up + elems_down] = w_start - w_now per packed slot (fomoe_pack_resident_deltas)."""

@@ -36,7 +36,7 @@ def margin_clean(p: Problem, oracle64, max_attempts=20) -> int:
     total = 0
     for attempt in range(max_attempts):
         r = oracle64.route(p.x, p.w_router, p.resident, w.k, w.gate_fn, w.gate_rule, w.temperature, p.bias, w.route_mode)
-        bad = np.nonzero(margins(r["logits"], w.k) < 2 * MARGIN)[0]
+        bad = np.nonzero(margins(r["logits"], w.k) <= MARGIN)[0]   # the bar itself: margins must EXCEED 1e-4, nothing wider
         if len(bad) == 0:
             return total
         p.x[bad] = W.redraw_x_rows(w, bad, attempt)

@@ -167,6 +167,28 @@ def test_no_resident_expert_gives_shared_only_or_zero(oracle64):
     assert np.all(y0 == 0) and np.all(b0["dx"] == 0)
 
 
+def test_shared_part_is_additive(oracle64):
+    """Shared experts sit outside the router with gate 1: the layer is (routed part) + (shared part), so
+    y, dx and the gradients split exactly.  tests/test_parity_fullsize_gpu.py uses this to pay for the shared FFN of the
+    C4 sweep once; the routed-only and shared-only runs are pinned by the brute force / closed form above."""
+    prob = refs.tiny_problem(15, T=9, d=6, E=5, k=2, F=4, n_res=3, n_sh=2, F_sh=3)
+    r, y, b = run_oracle(oracle64, prob)
+    routed = dict(prob, shared=None)
+    _, y_r, b_r = run_oracle(oracle64, routed)
+    only = dict(prob, resident=np.zeros(0, np.int32))
+    wg, wu, wd = refs.resident_stacks(prob)
+    r0 = oracle64.route(prob["x"], prob["w_r"], only["resident"], prob["k"])
+    y_s = oracle64.moe_fwd(prob["x"], r0, only["resident"], wg[:0], wu[:0], wd[:0], prob["shared"])
+    b_s = oracle64.moe_bwd(prob["x"], prob["dy"], prob["w_r"], r0, only["resident"], wg[:0], wu[:0], wd[:0], prob["shared"])
+    np.testing.assert_allclose(y, y_r + y_s, rtol=1e-12, atol=1e-14)
+    np.testing.assert_allclose(b["dx"], b_r["dx"] + b_s["dx"], rtol=1e-12, atol=1e-14)
+    for key in ("d_sh_gate", "d_sh_up", "d_sh_down"):
+        np.testing.assert_allclose(b[key], b_s[key], rtol=1e-12, atol=1e-14)
+    for key in ("dw_router", "dw_gate", "dw_up", "dw_down"):
+        np.testing.assert_allclose(b[key], b_r[key], rtol=1e-12, atol=1e-14)
+    assert not b_s["dw_router"].any()
+
+
 def test_all_resident_equals_standard_topk_moe(oracle64):
     """S = [0,E): the 'full overlap' limit is a plain top-k MoE; brute force has no residency term left."""
     prob = refs.tiny_problem(6, T=7, d=5, E=5, k=2, F=4, n_res=5)

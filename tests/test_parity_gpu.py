@@ -181,3 +181,99 @@ def test_bad_arguments_fail_loudly():
     rs = B.alloc_route_state(cfg, 4)
     with pytest.raises(B.FomoeError):
         B.fomoe_route(cfg, None, torch.zeros(64, 8, device="cuda"), None, torch.arange(4, dtype=torch.int32, device="cuda"), 4, rs)
+
+
+@pytest.mark.parametrize("dtype,E", [("f32", 8), ("bf16", 16), ("bf16", 128)])
+def test_nan_row_and_minus_inf_bias_stay_contained(oracle64, dtype, E):
+    """A diverging step (NaN activations in one token, a -inf router bias on most experts so that fewer than k logits are
+    finite) must not fault or corrupt the workspace: ids stay in [0, E), the step completes, and the rows of the other
+    tokens are what they are without the NaN token (token rows are independent: Eq. 13)."""
+    import torch
+    k = 4
+    w = W.MoEWorkload("nan", T=300, d=128, E=E, k=k, F=128, n_res=E // 2, dtype=dtype, seed=13)
+    p = H.Problem(w)
+    bias = np.zeros(E, np.float32)
+    bias[2:] = -np.inf                      # two finite logits < k = 4
+    p.bias = bias
+    layer = H.make_layer(p)
+    x_clean = layer.to_dev(p.x)
+    dy = layer.to_dev(p.dy)
+    layer.step(x_clean, dy)
+    torch.cuda.synchronize()
+    y_clean, idx_clean = layer.y.clone(), layer.route_state.topk_idx.clone()
+    xb = p.x.copy()
+    xb[7] = np.nan
+    xb[8, 3] = np.inf
+    x_bad = layer.to_dev(xb)
+    layer.step(x_bad, dy)
+    torch.cuda.synchronize()                # an illegal address would surface here
+    g = layer.routing_numpy()
+    assert g["topk_idx"].min() >= 0 and g["topk_idx"].max() < E
+    assert g["counts"].sum() == g["P"] <= w.T * k and (g["pair_row"] < g["P"]).all()
+    ok = np.ones(w.T, bool)
+    ok[[7, 8]] = False
+    okt = torch.from_numpy(ok).cuda()
+    assert torch.equal(layer.route_state.topk_idx[okt], idx_clean[okt])
+    assert torch.isfinite(layer.y[okt].float()).all()
+    assert H.rel_err(H.t2n(layer.y[okt]), H.t2n(y_clean[okt])) <= (2e-2 if dtype == "bf16" else 1e-5)
+    # and the layer still works afterwards
+    layer.step(x_clean, dy)
+    torch.cuda.synchronize()
+    assert torch.equal(layer.y, y_clean)
+
+
+def test_routing_stats_match_definitions(oracle64):
+    """fomoe_routing_stats against the numpy definitions, on a Zipf-skewed workload."""
+    from oracle import stats_oracle as SO
+    w = W.MoEWorkload("stats", T=3000, d=128, E=24, k=3, F=64, n_res=9, dtype="bf16", zipf_alpha=1.0, seed=14)
+    p = H.Problem(w)
+    H.margin_clean(p, oracle64)
+    r = oracle64.route(p.x, p.w_router, p.resident, w.k, w.gate_fn, w.gate_rule, w.temperature, p.bias)
+    want = SO.routing_stats(r["topk_idx"], p.resident, w.E)
+    layer = H.make_layer(p)
+    layer.route(layer.to_dev(p.x))
+    got = layer.routing_stats()
+    assert np.array_equal(got["load"], want["load"])
+    for key in ("kept_fraction", "ghost_fraction", "zero_kept_tokens", "load_cv", "routing_entropy", "max_load", "min_load"):
+        assert abs(got[key] - want[key]) <= 1e-5 * max(1.0, abs(want[key])), (key, got[key], want[key])
+    assert abs(got["kept_fraction"] - r["P"] / (w.T * w.k)) < 1e-6
+
+
+def test_debug_validate_resident():
+    import torch
+    from paper_2606_19025_b200 import binding as B
+    ids = lambda *a: torch.tensor(a, dtype=torch.int32, device="cuda")
+    B.fomoe_debug_validate_resident(ids(0, 3, 7), 8)
+    B.fomoe_debug_validate_resident(ids(), 8)
+    for bad, what in ((ids(0, 3, 8), "outside"), (ids(-1, 2), "outside"), (ids(1, 1, 2), "duplicate"), (ids(4, 2), "unsorted")):
+        with pytest.raises(B.FomoeError, match=what):
+            B.fomoe_debug_validate_resident(bad, 8)
+
+
+def test_step_host_matches_oracle_twice_in_a_row(oracle64):
+    """The end-to-end entry point bench.py times (fomoe_moe_step_host: uploads on two streams overlapping compute) against
+    the oracle, called twice back to back with different inputs and a separate copy stream (overlap logic)."""
+    import torch
+    w = W.MoEWorkload("e2e", T=2048, d=256, E=16, k=2, F=256, n_res=8, n_sh=1, F_sh=128, dtype="bf16", seed=15)
+    p = H.Problem(w)
+    H.margin_clean(p, oracle64)
+    layer = H.make_layer(p)
+    cs = torch.cuda.Stream()
+    td = layer.tdtype
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(td).pin_memory()
+    x1, dy1 = pin(p.x), pin(p.dy)
+    x2, dy2 = pin(p.x[::-1].copy()), pin((0.5 * p.dy[::-1]).astype(np.float32))   # token-reversed, scaled: also margin-clean
+    outs = [(torch.empty_like(x1).pin_memory(), torch.empty_like(x1).pin_memory()) for _ in range(2)]
+    xd, dyd = torch.empty((w.T, w.d), dtype=td, device="cuda"), torch.empty((w.T, w.d), dtype=td, device="cuda")
+    for (xh, dyh), (yh, dxh) in zip(((x1, dy1), (x2, dy2)), outs):
+        layer.step_host(xh, dyh, yh, dxh, xd, dyd, copy_stream=cs)     # no sync in between: the second call must order itself
+    torch.cuda.synchronize()
+    for i, ((xh, dyh), (yh, dxh)) in enumerate(zip(((x1, dy1), (x2, dy2)), outs)):
+        q = H.Problem(w)
+        q.x, q.dy = xh.float().numpy(), dyh.float().numpy()
+        r, y, b = H.oracle_all(q, oracle64)
+        assert H.rel_err(yh.float().numpy(), y) <= 2e-2, i
+        assert H.rel_err(dxh.float().numpy(), b["dx"]) <= 2e-2, i
+    # weight gradients left on the device are the second step's
+    for key, t in (("dw_router", layer.dw_router), ("dw_gate", layer.dw_gate), ("dw_down", layer.dw_down), ("d_sh_up", layer.d_shared[1])):
+        assert H.rel_err(H.t2n(t), b[key]) <= 2e-2, key

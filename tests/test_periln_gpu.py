@@ -54,26 +54,32 @@ def test_eq15_block_around_the_moe_layer(oracle64, dtype):
     dev = lambda a, dt=td: torch.from_numpy(np.ascontiguousarray(a)).cuda().to(dt)
     f32 = torch.float32
     alpha = 0.8
-    for seed in range(11, 40):      # the first seed whose normalised tokens keep every top-k margin above the bar
+    # The oracle chain consumes ITS OWN LN(x) rounded to storage; nothing the CUDA path produced enters it.  The two pre-LN
+    # outputs can differ by one storage ulp where the fp32 / fp64 results straddle a rounding boundary (a handful of bf16
+    # elements, each moving a logit by ~1e-4 |x|), so the seed is chosen -- from oracle values only -- with top-k margins
+    # above 10 x the 1e-4 bar: then both sides route identically.
+    for seed in range(11, 60):
         w = W.MoEWorkload("periln_blk", T=384, d=128, E=8, k=2, F=128, n_res=5, dtype=dtype, gate_fn=W.GATE_SIGMOID,
                           expert_fn=W.EXPERT_SILU, seed=seed)
         p = H.Problem(w)
         rng = np.random.default_rng(seed)
         x_in = st(rng.standard_normal((w.T, w.d)) * 1.7 + 0.2)
         g1, b1, g2, b2 = ((rng.standard_normal(w.d) * 0.1 + o).astype(np.float32) for o in (1.0, 0.0, 1.0, 0.0))
-        xd, g1d, b1d, g2d, b2d = dev(x_in), dev(g1, f32), dev(b1, f32), dev(g2, f32), dev(b2, f32)
-        # ---- CUDA path: pre-LN -> route/fwd -> post-LN + residual ----
-        xn = torch.empty_like(xd)
-        s1 = torch.empty((w.T, 2), dtype=f32, device="cuda")
-        s2 = torch.empty_like(s1)
-        B.fomoe_periln_fwd(xd, g1d, b1d, xn, s1)
-        torch.cuda.synchronize()
-        p.x = H.t2n(xn).astype(np.float32)          # the oracle layer consumes the same normalised tokens (storage-exact)
+        xn_ref, m1, r1 = PO.ln_fwd(x_in, g1, b1)
+        p.x = st(xn_ref.astype(np.float32))
         r, y_ref, _ = H.oracle_all(p, oracle64, bwd=False)
-        if not (H.margins(r["logits"], w.k) < 2 * H.MARGIN).any():
+        if not (H.margins(r["logits"], w.k) < 10 * H.MARGIN).any():
             break
     else:
         raise AssertionError("no seed with clean margins")
+    xd, g1d, b1d, g2d, b2d = dev(x_in), dev(g1, f32), dev(b1, f32), dev(g2, f32), dev(b2, f32)
+    # ---- CUDA path: pre-LN -> route/fwd -> post-LN + residual ----
+    xn = torch.empty_like(xd)
+    s1 = torch.empty((w.T, 2), dtype=f32, device="cuda")
+    s2 = torch.empty_like(s1)
+    B.fomoe_periln_fwd(xd, g1d, b1d, xn, s1)
+    torch.cuda.synchronize()
+    assert H.rel_err(H.t2n(xn), xn_ref) <= tol      # the pre-LN output on its own
     layer = H.make_layer(p)
     layer.route(xn)
     layer.forward(xn)
@@ -90,8 +96,6 @@ def test_eq15_block_around_the_moe_layer(oracle64, dtype):
     B.fomoe_periln_bwd(layer.dx, xd, s1, g1d, dx, dg1, db1, part, dresidual=dd)
     torch.cuda.synchronize()
     # ---- oracles chained the same way (fp64) ----
-    xn_ref, m1, r1 = PO.ln_fwd(x_in, g1, b1)
-    assert H.rel_err(H.t2n(xn), xn_ref) <= tol
     out_ref, m2, r2 = PO.periln_post_fwd(x_in, y_ref, g2, b2, alpha)
     assert H.rel_err(H.t2n(out), out_ref) <= tol
     dy_ref, dg2_ref, db2_ref = PO.periln_post_bwd(dout, y_ref, m2, r2, g2, alpha)
