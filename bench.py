@@ -216,19 +216,25 @@ def gemm_flops(mode: str, P: int, T: int, w: W.MoEWorkload, launches_per_step: f
     return float(mult) * rows * w.d * F
 
 
+L2_BYTES = 126e6   # B200 L2 (both dies); an input that fits and was just read by the previous kernel is served from it
+
+
 def hbm_bytes(name: str, P: int, T: int, w: W.MoEWorkload):
-    """Algorithmic bytes of one launch of the bandwidth-bound kernels; None for the others."""
+    """(algorithmic bytes of one launch, note) for the bandwidth-bound kernels; None for the others.
+    When the whole of x fits in L2 a kernel that re-reads it right after the router is served from L2, not HBM: those
+    bytes are then left out (counting them gave 'bandwidths' above the HBM peak) and the note says so."""
     s = 2 if w.dtype == "bf16" else 4
+    x_in_l2 = T * w.d * s <= 0.75 * L2_BYTES
     if "ROUTE" in name or name.startswith("route_kernel"):
-        return T * w.d * s + T * w.E * 4 + T * w.k * 8
+        return T * w.d * s + T * w.E * 4 + T * w.k * 8, None
     if name.startswith("gather_rows"):
-        return 2 * P * w.d * s
+        return (P * w.d * s, "x served from L2: only the write counted") if x_in_l2 else (2 * P * w.d * s, None)
     if name.startswith("combine_kernel"):
-        return (P + T * (2 if w.n_sh else 1)) * w.d * s
+        return (P + T * (2 if w.n_sh else 1)) * w.d * s, None
     if name.startswith("combine_bwd"):
-        return 3 * P * w.d * s
+        return 3 * P * w.d * s, None
     if name.startswith("dx_sum"):
-        return (P + T * (2 + (1 if w.n_sh else 0))) * w.d * s
+        return (P + T * (2 + (1 if w.n_sh else 0))) * w.d * s, None
     return None
 
 
@@ -316,6 +322,13 @@ def run_gpu(args, w, n_res):
         "clocks": clocks, "gpu_launches": launches[0] * args.steps,
         "kept_pairs": P, "kept_fraction": P / max(1, w.T * w.k), "ms_min": min(ms_list),
     }
+    try:   # routing diagnostics: realised kept fraction, load CV, entropy, zero-kept-token fraction
+        rs = layer.routing_stats()
+        out["routing_stats"] = {k: (float(v) if not hasattr(v, "tolist") else None) for k, v in rs.items() if k != "load"}
+        ld = rs["load"]
+        out["routing_stats"]["load_min_max_all_experts"] = [int(ld.min()), int(ld.max())]
+    except Exception as e:
+        out["routing_stats"] = {"error": str(e)}
     fl_pair = 18.0 if w.expert_fn == W.EXPERT_SWIGLU else 12.0   # flops per (row, d, F): 3 (2) GEMMs forward, twice that backward
     flops_step = fl_pair * P * w.d * w.F + fl_pair * w.T * w.n_sh * w.d * w.F_sh
     out["tflops"] = flops_step / (ms / 1e3) / 1e12
@@ -343,9 +356,12 @@ def run_gpu(args, w, n_res):
         kernels = []
         for name, (tt, n) in sorted(agg.items(), key=lambda kv: -kv[1][0]):
             k = {"name": name, "launches_per_step": n / args.steps, "ms_per_launch": tt / n, "share": tt / total}
-            hb = hbm_bytes(name, P, w.T, w)
-            if hb is not None:
+            hbn = hbm_bytes(name, P, w.T, w)
+            if hbn is not None:
+                hb, note = hbn
                 k.update(bound="hbm", achieved=hb / (tt / n / 1e3) / 1e9, unit="GB/s")
+                if note:
+                    k["note"] = note
                 k["frac"] = k["achieved"] / peaks["hbm_gbs"]
                 k["frac_of_nominal_8000"] = k["achieved"] / 8000.0
             elif name.startswith("umma_grouped_kernel"):
@@ -354,27 +370,34 @@ def run_gpu(args, w, n_res):
                 k["frac"] = k["achieved"] / tc_peak
             kernels.append(k)
         out["kernels"] = kernels
-        traffic = None
-        tf = ROOT / "profiles" / "r1g_traffic.csv"   # DRAM bytes per launch from the committed ncu --set full captures
+        # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed `ncu --set full` capture of
+        # THIS revision's kernels (profiles/r2_traffic.md names the command); keyed by workload and by the name the library emits
         traffic_rows = {}
+        tf = ROOT / "profiles" / "r2_traffic.csv"
         if tf.exists():
             for line in tf.read_text().splitlines()[1:]:
+                if not line.strip():
+                    continue
                 wl, rest = line.split(",", 1)          # kernel names contain commas: workload,kernel,bytes,launches
                 kname, nbytes, _ = rest.rsplit(",", 2)
                 traffic_rows[(wl, kname)] = float(nbytes)
-        gemms = [k for k in kernels if k.get("bound") == "tensor" and "router" not in k["name"]]
+        gemms = [k for k in kernels if k.get("bound") == "tensor" and "router" not in k["name"] and "ROUTE" not in k["name"]]
         if gemms:
-            dom = gemms[0]
-            traffic = traffic_rows.get((w.name, dom["name"]))
-            out["roofline"] = {"kernel": dom["name"], "bound": "tensor", "achieved": dom["achieved"],
-                               "peak": tc_peak, "unit": "TFLOP/s", "frac": dom["frac"], "traffic": traffic,
-                               "peak_source": peak_src + ", " + tc_peak_name,
-                               "frac_of_nominal_2250": dom["achieved"] / 2250.0, "share_of_step": dom["share"],
-                               "kernel_timing": "second pass of the same steps with one CUDA event after every launch"}
+            def roof(kk):
+                return {"kernel": kk["name"], "bound": "tensor", "achieved": kk["achieved"], "peak": tc_peak, "unit": "TFLOP/s",
+                        "frac": kk["frac"], "traffic": traffic_rows.get((w.name, kk["name"])),
+                        "peak_source": peak_src + ", " + tc_peak_name, "frac_of_nominal_2250": kk["achieved"] / 2250.0,
+                        "share_of_step": kk["share"], "ms_per_launch": kk["ms_per_launch"],
+                        "kernel_timing": "second pass of the same steps with one CUDA event after every launch"}
+            out["roofline"] = roof(gemms[0])                                   # the GEMM with the largest share of the step
+            out["roofline_worst"] = roof(min(gemms, key=lambda kk: kk["frac"]))  # the GEMM furthest below the peak
             gt = sum(k["ms_per_launch"] * k["launches_per_step"] for k in gemms)
             out["gemm_family"] = {"tflops": flops_step / (gt / 1e3) / 1e12, "share_of_step": gt * args.steps / total,
                                   "frac_of_peak": flops_step / (gt / 1e3) / 1e12 / tc_peak,
                                   "frac_of_nominal_2250": flops_step / (gt / 1e3) / 1e12 / 2250.0}
+        hbms = [k for k in kernels if k.get("bound") == "hbm"]
+        if hbms:
+            out["hbm_kernels"] = {k["name"]: round(k["frac"], 3) for k in hbms}
 
         # ---- end to end through the C ABI with HOST buffers (uploads x, dy; downloads y, dx every step) ----
         xh, dyh = x.cpu().pin_memory(), dy.cpu().pin_memory()
@@ -447,21 +470,44 @@ def run_gpu(args, w, n_res):
             out["periln"] = {"error": str(e)}
         del now, start, payload
 
-        # ---- skip-token speed-up against the same kernels with every expert resident ----
+        # ---- skip-token speed-up against the same kernels with every expert resident: both arms replay a CUDA graph, both
+        # are timed by the same loop, and both report the clocks sampled inside their own timed region ----
         if not args.no_all_resident and n_res < w.E:
-            del layer
+            del layer, step
             torch.cuda.empty_cache()
             full = build_layer(w.E)
-            ms_full = timed_steps(lambda: full.step(x, dy), args.steps, args.warmup)
+            full_step = full.step
+            if not args.no_graph:
+                full.step(x, dy)
+                full_step = full.capture_step(x, dy)
+            else:
+                full_step = lambda: full.step(x, dy)  # noqa: E731
+            s2 = ClockSampler(local)
+            s2.start()
+            ms_full = timed_steps(full_step, args.steps, args.warmup)
+            clocks_full = s2.stop(tuple(window))
             mf = sum(ms_full) / len(ms_full)
-            out["skip_token"] = {"ms_all_resident": mf, "speedup_vs_all_resident": mf / ms,
-                                 "ideal_flop_ratio": (w.k * fl_pair * w.d * w.F * w.T + fl_pair * w.T * w.n_sh * w.d * w.F_sh) / flops_step}
-            del full
+            ideal = (w.k * fl_pair * w.d * w.F * w.T + fl_pair * w.T * w.n_sh * w.d * w.F_sh) / flops_step
+            sk = {"ms_all_resident": mf, "speedup_vs_all_resident": mf / ms, "ideal_flop_ratio": ideal,
+                  "launch_all_resident": "eager" if args.no_graph else "CUDA graph (same as the skip arm)",
+                  "sm_mhz_skip_arm": clocks.get("sm_mhz"), "sm_mhz_all_resident": clocks_full.get("sm_mhz"),
+                  "reasons_all_resident": clocks_full.get("reasons")}
+            sk["tflops_all_resident"] = (w.k * fl_pair * w.d * w.F * w.T + fl_pair * w.T * w.n_sh * w.d * w.F_sh) / (mf / 1e3) / 1e12
+            sk["tflops_skip_arm"] = out["tflops"]
+            if mf / ms > ideal:   # a speed-up above the FLOP ratio means the all-resident arm ran less efficiently: say why
+                a, b = clocks.get("sm_mhz"), clocks_full.get("sm_mhz")
+                sk["above_ideal_because"] = (
+                    f"the longer all-resident step ran at a lower SM clock ({b} MHz against {a} MHz for the skip arm, power cap); "
+                    f"clock-normalised speed-up {mf / ms * (b / a):.2f}x" if a and b and b < 0.98 * a else
+                    f"not a clock effect ({b} vs {a} MHz): the all-resident arm reached {sk['tflops_all_resident']:.0f} TFLOP/s "
+                    f"against {out['tflops']:.0f} for the skip arm on the same kernels")
+            out["skip_token"] = sk
+            del full, full_step
 
         # ---- Fig. 11 analogue: step time against the number of ghost (non-resident) experts ----
         if args.ghost_sweep:
             try:
-                del layer
+                del layer, step
             except NameError:
                 pass
             torch.cuda.empty_cache()
@@ -501,7 +547,8 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C2", choices=sorted(W.CONFIGS))
+    ap.add_argument("--workload", default="C5", choices=sorted(W.CONFIGS),
+                    help="C5 (BASELINE.json configs[4]) is the largest single-GPU configuration: the headline")
     ap.add_argument("--n-res", type=int, default=None)
     ap.add_argument("--ref-tokens", type=int, default=16384, help="upper bound on the tokens per step of the CPU oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -510,6 +557,11 @@ def main():
     ap.add_argument("--no-graph", action="store_true", help="launch kernels eagerly instead of replaying a CUDA graph")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # not launched by torchrun: start one process per GPU ourselves (the driver's launch line, see the module docstring)
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+               "--master-port", str(29500 + os.getpid() % 2000), str(Path(__file__).resolve()), *sys.argv[1:]]
+        raise SystemExit(subprocess.call(cmd))
     w = W.config(args.workload)
     n_res = w.n_res if args.n_res is None else args.n_res
     if args.impl == "reference":

@@ -56,22 +56,25 @@ def test_eq15_block_around_the_moe_layer(oracle64, dtype):
     alpha = 0.8
     # The oracle chain consumes ITS OWN LN(x) rounded to storage; nothing the CUDA path produced enters it.  The two pre-LN
     # outputs can differ by one storage ulp where the fp32 / fp64 results straddle a rounding boundary (a handful of bf16
-    # elements, each moving a logit by ~1e-4 |x|), so the seed is chosen -- from oracle values only -- with top-k margins
-    # above 10 x the 1e-4 bar: then both sides route identically.
-    for seed in range(11, 60):
-        w = W.MoEWorkload("periln_blk", T=384, d=128, E=8, k=2, F=128, n_res=5, dtype=dtype, gate_fn=W.GATE_SIGMOID,
-                          expert_fn=W.EXPERT_SILU, seed=seed)
-        p = H.Problem(w)
-        rng = np.random.default_rng(seed)
-        x_in = st(rng.standard_normal((w.T, w.d)) * 1.7 + 0.2)
-        g1, b1, g2, b2 = ((rng.standard_normal(w.d) * 0.1 + o).astype(np.float32) for o in (1.0, 0.0, 1.0, 0.0))
+    # elements, each moving a logit by ~1e-4 |x|), so the tokens whose top-k margins -- computed from oracle values only --
+    # are below 10 x the 1e-4 bar are redrawn until none is left: then both sides route identically.
+    seed = 11
+    w = W.MoEWorkload("periln_blk", T=384, d=128, E=8, k=2, F=128, n_res=5, dtype=dtype, gate_fn=W.GATE_SIGMOID,
+                      expert_fn=W.EXPERT_SILU, seed=seed)
+    p = H.Problem(w)
+    rng = np.random.default_rng(seed)
+    x_in = st(rng.standard_normal((w.T, w.d)) * 1.7 + 0.2)
+    g1, b1, g2, b2 = ((rng.standard_normal(w.d) * 0.1 + o).astype(np.float32) for o in (1.0, 0.0, 1.0, 0.0))
+    for _ in range(64):
         xn_ref, m1, r1 = PO.ln_fwd(x_in, g1, b1)
         p.x = st(xn_ref.astype(np.float32))
         r, y_ref, _ = H.oracle_all(p, oracle64, bwd=False)
-        if not (H.margins(r["logits"], w.k) < 10 * H.MARGIN).any():
+        bad = np.nonzero(H.margins(r["logits"], w.k) < 10 * H.MARGIN)[0]
+        if len(bad) == 0:
             break
+        x_in[bad] = st(rng.standard_normal((len(bad), w.d)) * 1.7 + 0.2)
     else:
-        raise AssertionError("no seed with clean margins")
+        raise AssertionError("margin cleaning did not converge")
     xd, g1d, b1d, g2d, b2d = dev(x_in), dev(g1, f32), dev(b1, f32), dev(g2, f32), dev(b2, f32)
     # ---- CUDA path: pre-LN -> route/fwd -> post-LN + residual ----
     xn = torch.empty_like(xd)
