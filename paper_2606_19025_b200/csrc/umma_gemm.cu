@@ -44,7 +44,7 @@ constexpr int kEpiWarps = 8;    // two warps per TMEM lane quarter; they take al
 constexpr int kStgTile = 2048;
 constexpr int kDhDepth = 3;  // DH epilogue: chunks of (a, u) kept in flight per warp with cp.async
 enum Mode { FWD1 = 0, FWD2 = 1, DH = 2, DX = 3, WGRAD = 4, ROUTE = 5, FWD1S = 6 };
-constexpr int kRouteStg = 40960;  // ROUTE epilogue scratch: slot map, per-stage histograms, top-k merge lists (k <= 32)
+constexpr int kRouteStg = 57344;  // ROUTE epilogue scratch: slot map, per-stage histograms, top-k candidate / merge lists (k <= 32)
 // DH and FWD1 trade TMA stages for epilogue staging: DH streams a and u back in through a cp.async ring
 __host__ __device__ constexpr int stages_of(int mode) { return mode == DH ? 4 : (mode == FWD1 || mode == FWD1S || mode == ROUTE) ? 5 : 6; }
 __host__ __device__ constexpr int stg_tiles_per_warp(int mode) { return mode == DH ? 2 * kDhDepth : mode == FWD1 ? 3 : mode == FWD1S ? 2 : 1; }
@@ -288,15 +288,274 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16]) {
 }
 __device__ __forceinline__ void bar_sync_named(int id, int threads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory"); }
 
+constexpr int kNetK = 16;     // largest top-k list the sorting-network epilogue handles (k <= 16); k = 17..32 takes the insertion epilogue
 struct RouteSmem {            // lives in the kernel's staging area (kRouteStg bytes)
   int32_t slot[128];          // resident slot of expert e, -1 = ghost
+  float zb[128];              // additive logit term of expert e: router bias (or 0); -inf = no such column (e >= E, or a ghost
+                              // expert under forced-local routing)
   int32_t hist[kAccStages][128];
-  float lv[kMaxK][128];       // half 1 -> half 0: top-k values / ids of row r
-  int32_t li[kMaxK][128];
   float mx[2][128];           // partial max of each half
   float sum[2][128];          // partial softmax denominators
+  union {
+    struct {                  // insertion epilogue (k > kNetK)
+      float lv[kMaxK][128];   // half 1 -> half 0: top-k values / ids of row r
+      int32_t li[kMaxK][128];
+    } ins;
+    struct {                  // sorting-network epilogue
+      uint2 hand[kNetK][128];          // half 1 -> half 0: sorted (value, id) list of row r
+      uint2 cand[kNetK + 1][256];      // per-thread candidate lists (thread-private), written in id order
+    } net;
+  };
 };
 static_assert(sizeof(RouteSmem) <= kRouteStg, "route epilogue scratch");
+
+// ---- sorting networks on registers (all indices are compile-time: nothing spills) ----
+// Descending bitonic networks.  Values only: a compare-exchange is one FMNMX pair; a NaN operand is dropped by fmaxf / fminf
+// (the other operand is duplicated), which can only RAISE the outputs.
+template <int N> struct NetV {
+  static __device__ __forceinline__ void ce(float& a, float& b) { const float hi = fmaxf(a, b), lo = fminf(a, b); a = hi; b = lo; }
+  static __device__ __forceinline__ void merge(float (&v)[N]) {   // bitonic sequence -> descending
+#pragma unroll
+    for (int j = N >> 1; j > 0; j >>= 1)
+#pragma unroll
+      for (int i = 0; i < N; ++i)
+        if ((i ^ j) > i) ce(v[i], v[i ^ j]);
+  }
+  static __device__ __forceinline__ void sort(float (&v)[N]) {
+#pragma unroll
+    for (int k = 2; k <= N; k <<= 1)
+#pragma unroll
+      for (int j = k >> 1; j > 0; j >>= 1)
+#pragma unroll
+        for (int i = 0; i < N; ++i)
+          if ((i ^ j) > i) { if ((i & k) == 0) ce(v[i], v[i ^ j]); else ce(v[i ^ j], v[i]); }
+  }
+};
+// (value, id) pairs in the order of PAPER.md:519 Eq. 14 as read in DESIGN.md R5: larger logit first, ties -> lower expert id
+template <int N> struct NetKV {
+  static __device__ __forceinline__ void ce(float& av, int& ai, float& bv, int& bi) {   // afterwards a comes before b
+    const bool sw = bv > av || (bv == av && bi < ai);
+    const float v = sw ? bv : av, w = sw ? av : bv;
+    const int i = sw ? bi : ai, j = sw ? ai : bi;
+    av = v; bv = w; ai = i; bi = j;
+  }
+  static __device__ __forceinline__ void merge(float (&v)[N], int (&id)[N]) {
+#pragma unroll
+    for (int j = N >> 1; j > 0; j >>= 1)
+#pragma unroll
+      for (int i = 0; i < N; ++i)
+        if ((i ^ j) > i) ce(v[i], id[i], v[i ^ j], id[i ^ j]);
+  }
+  static __device__ __forceinline__ void sort(float (&v)[N], int (&id)[N]) {
+#pragma unroll
+    for (int k = 2; k <= N; k <<= 1)
+#pragma unroll
+      for (int j = k >> 1; j > 0; j >>= 1)
+#pragma unroll
+        for (int i = 0; i < N; ++i)
+          if ((i ^ j) > i) { if ((i & k) == 0) ce(v[i], id[i], v[i ^ j], id[i ^ j]); else ce(v[i ^ j], id[i ^ j], v[i], id[i]); }
+  }
+};
+__device__ __forceinline__ void sts64(uint32_t addr, uint32_t a, uint32_t b) {
+  asm volatile("st.shared.v2.b32 [%0], {%1, %2};" ::"r"(addr), "r"(a), "r"(b) : "memory");
+}
+__device__ __forceinline__ uint2 lds64(uint32_t addr) {
+  uint2 v;
+  asm volatile("ld.shared.v2.b32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ void stg256(float* p, const float* v) {   // 32-byte store: one whole sector per lane
+  asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]), "f"(v[4]),
+               "f"(v[5]), "f"(v[6]), "f"(v[7]) : "memory");
+}
+
+// Sorting-network ROUTE epilogue (k <= kNetK).  A thread owns one token row and, of its experts, the 16-wide chunks half,
+// half + 2, ...  Selection without data-dependent branches (a per-lane insertion list makes every lane pay for every
+// insertion of any lane, in one long dependent chain), in three rolled passes over the thread's chunks -- each pass re-reads
+// the chunk from tensor memory and recombines it with the SAME instruction sequence, so the values are bit-identical (small
+// code: the unrolled single-pass form overflowed the instruction cache and spilled):
+//   A. top-KMAX VALUES by bitonic networks of FMNMX (groups of KMAX sorted, merged into the running list);
+//   B. the KMAX-th value is the threshold: logits above it, and the first ones equal to it in id order, are the candidates
+//      -- written with predicated stores to a thread-private list in shared memory (exactly the top KMAX, ties -> lower id);
+//      the same pass sums exp(z - local max) for the softmax;
+//      then the <= KMAX candidates are sorted with their ids and the two halves' lists merged by half 0;
+//   C. probabilities.
+template <int KMAX>
+__device__ __forceinline__ void route_tile_epilogue_net(const UmmaParams& p, RouteSmem* rs, uint32_t taddr, int q, int half, int lane, int as,
+                                                        int row0, bool live) {
+  const RouteEpi& r = p.r;
+  const int E = r.E, Epad = r.Epad;
+  const bool three = r.pieces == 3, softmax = r.gate_fn == FOMOE_GATE_SOFTMAX;
+  const int rl = q * 32 + lane;        // row within the CTA's 128
+  const int t = row0 + rl;
+  const bool row_ok = live && t < p.dense_rows;
+  if (live) {
+    auto load_z = [&](int c0, float (&z)[16]) {   // logits of 16 experts from c0: identical arithmetic in every pass
+      float md[16], lo[16];
+      tmem_ld16(taddr + c0, z);
+      tmem_ld16(taddr + Epad + c0, md);
+      if (three) tmem_ld16(taddr + 2 * Epad + c0, lo);
+      float zb[16];
+#pragma unroll
+      for (int v = 0; v < 4; ++v) *reinterpret_cast<float4*>(&zb[4 * v]) = *reinterpret_cast<const float4*>(&rs->zb[c0 + 4 * v]);
+      tmem_ld_wait();
+#pragma unroll
+      for (int i = 0; i < 16; ++i) {
+        float sacc = __fadd_rn(z[i], md[i]);
+        if (three) sacc = __fadd_rn(sacc, lo[i]);
+        z[i] = __fmaf_rn(sacc, r.inv_tau, zb[i]);   // (padding columns of the accumulator are exactly 0: 0 * inv_tau - inf = -inf)
+      }
+    };
+    // A. top-KMAX values, descending
+    float tv[KMAX];
+#pragma unroll
+    for (int j = 0; j < KMAX; ++j) tv[j] = -INFINITY;
+#pragma unroll 1
+    for (int c0 = 16 * half; c0 < Epad; c0 += 32) {
+      float z[16];
+      load_z(c0, z);
+#pragma unroll
+      for (int g = 0; g < 16 / KMAX; ++g) {
+        float sv[KMAX];
+#pragma unroll
+        for (int j = 0; j < KMAX; ++j) sv[j] = z[g * KMAX + j];
+        NetV<KMAX>::sort(sv);
+#pragma unroll
+        for (int j = 0; j < KMAX; ++j) tv[j] = fmaxf(tv[j], sv[KMAX - 1 - j]);   // the top half of the 2 KMAX values, bitonic
+        NetV<KMAX>::merge(tv);
+      }
+    }
+    const float mxl = tv[0];
+    const float mxe = mxl == -INFINITY ? 0.f : mxl;   // (no finite logit in this half: every exponential below is exp(-inf) = 0)
+    rs->mx[half][rl] = mxl;
+    // B. candidates: > threshold, and the first `need` ones == threshold; softmax partial sum against the local max
+    const float thr = tv[KMAX - 1];
+    int need = KMAX;
+#pragma unroll
+    for (int j = 0; j < KMAX - 1; ++j) need -= tv[j] > thr ? 1 : 0;
+    const uint32_t cand0 = smem_u32(&rs->net.cand[0][half * 128 + rl]);
+    constexpr uint32_t kCandStride = 256 * sizeof(uint2);
+#pragma unroll
+    for (int j = 0; j < KMAX; ++j) sts64(cand0 + j * kCandStride, __float_as_uint(-INFINITY), (uint32_t)kMaxE);
+    float sml = 0.f;
+    {
+      uint32_t ca = cand0;
+      int eqc = 0;
+#pragma unroll 1
+      for (int c0 = 16 * half; c0 < Epad; c0 += 32) {
+        float z[16];
+        load_z(c0, z);
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+          const float v = z[i];
+          const bool eq = v == thr && eqc < need;
+          if (v > thr || eq) { sts64(ca, __float_as_uint(v), (uint32_t)(c0 + i)); ca += kCandStride; }
+          eqc += eq ? 1 : 0;
+        }
+        if (softmax) {
+#pragma unroll
+          for (int i = 0; i < 16; ++i) sml += __expf(z[i] - mxe);   // (exp(-inf) = 0 for the columns that do not exist)
+        }
+      }
+    }
+    rs->sum[half][rl] = sml;
+    float cv[KMAX];
+    int ci[KMAX];
+#pragma unroll
+    for (int j = 0; j < KMAX; ++j) {
+      const uint2 e = lds64(cand0 + j * kCandStride);
+      cv[j] = __uint_as_float(e.x);
+      ci[j] = (int)e.y;
+    }
+    NetKV<KMAX>::sort(cv, ci);
+    if (half == 1) {
+#pragma unroll
+      for (int j = 0; j < KMAX; ++j) rs->net.hand[j][rl] = make_uint2(__float_as_uint(cv[j]), (uint32_t)ci[j]);
+    }
+    bar_sync_named(1 + q, 64);
+    const float mx0 = rs->mx[0][rl], mx1 = rs->mx[1][rl];
+    const float mx = fmaxf(mx0, mx1);
+    float inv_s = 1.f;
+    if (softmax) {   // denominators of the two halves, rescaled to the common max (a half without experts: max -inf, sum 0)
+      const float s0 = rs->sum[0][rl], s1 = rs->sum[1][rl];
+      inv_s = 1.0f / ((mx0 == mx || s0 == 0.f ? s0 : s0 * __expf(mx0 - mx)) + (mx1 == mx || s1 == 0.f ? s1 : s1 * __expf(mx1 - mx)));
+    }
+    if (half == 0) {   // top KMAX of the two sorted lists: pairwise "earlier of a[j], b[KMAX-1-j]" is bitonic, then merge
+#pragma unroll
+      for (int j = 0; j < KMAX; ++j) {
+        const uint2 e = rs->net.hand[KMAX - 1 - j][rl];
+        const float bv = __uint_as_float(e.x);
+        const int bi = (int)e.y;
+        const bool sw = bv > cv[j] || (bv == cv[j] && bi < ci[j]);
+        cv[j] = sw ? bv : cv[j];
+        ci[j] = sw ? bi : ci[j];
+      }
+      NetKV<KMAX>::merge(cv, ci);
+      // fewer than k logits compare greater than -inf (NaN / inf activations, a -inf bias): the list still holds the sentinel id.
+      // Keep every id in range so that neither the slot lookup below nor the permutation kernels index with it
+#pragma unroll
+      for (int j = 0; j < KMAX; ++j) ci[j] = min(ci[j], E - 1);
+    }
+    auto prob_of = [&](float zz) { return softmax ? __expf(zz - mx) * inv_s : __fdividef(1.0f, 1.0f + __expf(-zz)); };
+    // C. probabilities of this warp's chunks
+#pragma unroll 1
+    for (int c0 = 16 * half; c0 < Epad; c0 += 32) {
+      float z[16];
+      load_z(c0, z);
+#pragma unroll
+      for (int i = 0; i < 16; ++i) z[i] = prob_of(z[i]);
+      if (row_ok) {
+        float* dst = r.probs + (size_t)t * E + c0;
+        if ((E & 7) == 0) {
+          if (c0 < E) stg256(dst, &z[0]);
+          if (c0 + 8 < E) stg256(dst + 8, &z[8]);
+        } else {
+#pragma unroll
+          for (int i = 0; i < 16; ++i)
+            if (c0 + i < E) dst[i] = z[i];
+        }
+      }
+    }
+    // residency mask, gate rule, outputs, per-slot histogram of the block
+    if (half == 0 && row_ok) {
+      float pj[KMAX];
+      int sl[KMAX];
+      float s_all = 0.f, s_kept = 0.f;
+#pragma unroll
+      for (int j = 0; j < KMAX; ++j) {
+        pj[j] = 0.f;
+        sl[j] = -1;
+        if (j < r.k) {
+          pj[j] = prob_of(cv[j]);
+          sl[j] = rs->slot[ci[j]];
+          s_all += pj[j];
+          if (sl[j] >= 0) s_kept += pj[j];
+        }
+      }
+#pragma unroll
+      for (int j = 0; j < KMAX; ++j) {
+        if (j < r.k) {
+          float g = 0.f;
+          if (sl[j] >= 0) {
+            g = r.gate_rule == FOMOE_DROP_ONLY ? pj[j] : r.gate_rule == FOMOE_RENORM_TOPK ? pj[j] / s_all : pj[j] / s_kept;
+            atomicAdd(&rs->hist[as][sl[j]], 1);
+          }
+          r.topk_idx[(size_t)t * r.k + j] = ci[j];
+          r.gate[(size_t)t * r.k + j] = g;
+        }
+      }
+    }
+  }
+  // all 8 epilogue warps: the block's histogram is complete; flush and clear it (next use of hist[as] is two tiles later)
+  bar_sync_named(5, kEpiWarps * 32);
+  if (live) {
+    const int tid = (half * 4 + q) * 32 + lane;
+    for (int i = tid; i < r.n_res; i += kEpiWarps * 32) {
+      r.blk_hist[(size_t)(row0 / BM) * r.n_res + i] = rs->hist[as][i];
+      rs->hist[as][i] = 0;
+    }
+  }
+}
 
 template <int KMAX>
 __device__ __forceinline__ void route_tile_epilogue(const UmmaParams& p, RouteSmem* rs, uint32_t taddr, int q, int half, int lane, int as,
@@ -359,15 +618,15 @@ __device__ __forceinline__ void route_tile_epilogue(const UmmaParams& p, RouteSm
     rs->mx[half][rl] = mx;
     if (half == 1) {
 #pragma unroll
-      for (int j = 0; j < KMAX; ++j) { rs->lv[j][rl] = tv[j]; rs->li[j][rl] = ti[j]; }
+      for (int j = 0; j < KMAX; ++j) { rs->ins.lv[j][rl] = tv[j]; rs->ins.li[j][rl] = ti[j]; }
     }
     bar_sync_named(1 + q, 64);
     mx = fmaxf(rs->mx[0][rl], rs->mx[1][rl]);
     if (half == 0) {   // merge the partner's list: insert its entries (descending) with the (value, lower id) order
 #pragma unroll 1
       for (int jj = 0; jj < KMAX; ++jj) {
-        float cv = rs->lv[jj][rl];
-        int ci = rs->li[jj][rl];
+        float cv = rs->ins.lv[jj][rl];
+        int ci = rs->ins.li[jj][rl];
         bool ins = false;
 #pragma unroll
         for (int j = 0; j < KMAX; ++j) {
@@ -620,7 +879,11 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
       RouteSmem* rs = reinterpret_cast<RouteSmem*>(stg_base);
       {  // slot map and cleared histograms, visible to all epilogue warps before the first tile
         const int tid = threadIdx.x - 128;
-        for (int i = tid; i < p.r.E; i += kEpiWarps * 32) rs->slot[i] = p.r.slot_of[i];
+        for (int i = tid; i < 128; i += kEpiWarps * 32) {
+          const int sl = i < p.r.E ? p.r.slot_of[i] : -1;
+          rs->slot[i] = sl;
+          rs->zb[i] = (i >= p.r.E || (p.r.forced_local && sl < 0)) ? -INFINITY : (p.r.bias ? p.r.bias[i] : 0.f);
+        }
         for (int i = tid; i < kAccStages * 128; i += kEpiWarps * 32) (&rs->hist[0][0])[i] = 0;
         bar_sync_named(5, kEpiWarps * 32);
       }
@@ -631,7 +894,8 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
         const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * BN;
         mbar_wait(smem_u32(&tfull_bar[as]), aphase);
         tc_fence_after();
-        route_tile_epilogue<(KMAX > 0 ? KMAX : 2)>(p, rs, taddr, q, half, lane, as, t.row0, t.live);
+        if constexpr (KMAX > kNetK) route_tile_epilogue<KMAX>(p, rs, taddr, q, half, lane, as, t.row0, t.live);
+        else route_tile_epilogue_net<(KMAX > 0 ? KMAX : 2)>(p, rs, taddr, q, half, lane, as, t.row0, t.live);
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive_cluster(tempty_leader + 8 * as);
