@@ -449,23 +449,50 @@ def run_gpu(args, w, n_res):
             del grads, m1, v1, wc
         except Exception as e:   # never let the side measurements take the headline down
             out["optim"] = {"error": str(e)}
-        # ---- Peri-LN either side of the block (Eq. 15): two streaming row kernels ----
+        # ---- Peri-LN either side of the block (Eq. 15): the stand-alone streaming kernels
+        # against the HBM roofline, and the whole block x + alpha LN(MoE(LN(x))) fused (post-LN inside the combine, pre-LN backward
+        # inside the dx scatter-sum) and unfused, in units of one pass over [T, d] beyond the MoE step ----
         try:
             gam, bet = torch.ones(w.d, device="cuda"), torch.zeros(w.d, device="cuda")
-            stats = torch.empty((w.T, 2), dtype=torch.float32, device="cuda")
-            lo, ldx = torch.empty_like(x), torch.empty_like(x)
+            stats, stats2 = (torch.empty((w.T, 2), dtype=torch.float32, device="cuda") for _ in range(2))
+            lo, ldx, xn, dyy = (torch.empty_like(x) for _ in range(4))
             dgm, dbt = torch.empty(w.d, device="cuda"), torch.empty(w.d, device="cuda")
             part = torch.empty(B.fomoe_periln_workspace_bytes(w.T, w.d), dtype=torch.uint8, device="cuda")
             es = x.element_size()
-            ft = timed_steps(lambda: B.fomoe_periln_fwd(x, gam, bet, lo, stats, residual=dy, alpha=0.8), max(args.steps, 10), 3)
-            bt = timed_steps(lambda: B.fomoe_periln_bwd(dy, x, stats, gam, ldx, dgm, dbt, part, dresidual=dy, alpha=0.8), max(args.steps, 10), 3)
+            n10 = max(args.steps, 10)
+            ft = timed_steps(lambda: B.fomoe_periln_fwd(x, gam, bet, lo, stats, residual=dy, alpha=0.8), n10, 3)
+            bt = timed_steps(lambda: B.fomoe_periln_bwd(dy, x, stats, gam, ldx, dgm, dbt, part, dresidual=dy, alpha=0.8), n10, 3)
             fms, bms = sum(ft) / len(ft), sum(bt) / len(bt)
             fby, bby = 3.0 * w.T * w.d * es, 4.0 * w.T * w.d * es       # post-LN + residual: read y, x, write out; bwd: read dout, x, dres, write dx
-            out["periln"] = {"post_fwd": {"bound": "hbm", "achieved": fby / (fms / 1e3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                                          "frac": fby / (fms / 1e3) / 1e9 / peaks["hbm_gbs"], "ms": fms, "bytes": fby},
-                             "pre_bwd": {"bound": "hbm", "achieved": bby / (bms / 1e3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                                         "frac": bby / (bms / 1e3) / 1e9 / peaks["hbm_gbs"], "ms": bms, "bytes": bby}}
-            del lo, ldx, part
+            pl = {"post_fwd": {"bound": "hbm", "achieved": fby / (fms / 1e3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                               "frac": fby / (fms / 1e3) / 1e9 / peaks["hbm_gbs"], "ms": fms, "bytes": fby},
+                  "pre_bwd": {"bound": "hbm", "achieved": bby / (bms / 1e3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                              "frac": bby / (bms / 1e3) / 1e9 / peaks["hbm_gbs"], "ms": bms, "bytes": bby}}
+
+            def block(fused):
+                B.fomoe_periln_fwd(x, gam, bet, xn, stats)                                  # pre-LN
+                layer.route(xn)
+                if fused:
+                    layer.forward_periln(xn, gam, bet, x, lo, stats2, alpha=0.8)            # MoE + post-LN + residual
+                else:
+                    layer.forward(xn)
+                    B.fomoe_periln_fwd(layer.y, gam, bet, lo, stats2, residual=x, alpha=0.8)
+                B.fomoe_periln_bwd(dy, layer.y, stats2, gam, dyy, dgm, dbt, part, alpha=0.8)  # post-LN backward -> dy of the layer
+                if fused:
+                    layer.backward_periln(dyy, xn, x, stats, gam, dy, dgm, dbt, part)       # MoE backward + pre-LN backward + residual
+                else:
+                    layer.backward(dyy, xn)
+                    B.fomoe_periln_bwd(layer.dx, x, stats, gam, ldx, dgm, dbt, part, dresidual=dy)
+            if B.fomoe_periln_fused_supported(layer.cfg):
+                pass_ms = 2.0 * w.T * w.d * es / (peaks["hbm_gbs"] * 1e9) * 1e3    # read + write of [T, d] at the measured copy rate
+                step_ms = sum(timed_steps(step_eager, n10, 3)) / n10
+                tf_ = sum(timed_steps(lambda: block(True), n10, 3)) / n10
+                tu_ = sum(timed_steps(lambda: block(False), n10, 3)) / n10
+                pl["block"] = {"ms_moe_step_eager": step_ms, "ms_block_fused": tf_, "ms_block_unfused": tu_,
+                               "extra_passes_fused": (tf_ - step_ms) / pass_ms, "extra_passes_unfused": (tu_ - step_ms) / pass_ms,
+                               "pass_ms": pass_ms, "launch": "eager (all three arms)"}
+            out["periln"] = pl
+            del lo, ldx, xn, dyy, part
         except Exception as e:
             out["periln"] = {"error": str(e)}
         del now, start, payload

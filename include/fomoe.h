@@ -37,7 +37,7 @@
 extern "C" {
 #endif
 
-#define FOMOE_ABI_VERSION 4
+#define FOMOE_ABI_VERSION 5
 
 #if defined(__GNUC__)
 #define FOMOE_API __attribute__((visibility("default")))
@@ -203,6 +203,47 @@ FOMOE_API int fomoe_periln_fwd(int32_t T, int32_t d_model, int32_t dtype, const 
 FOMOE_API int fomoe_periln_bwd(int32_t T, int32_t d_model, int32_t dtype, const void* dout, const void* x, const float* stats,
                      const float* gamma, float alpha, const void* dresidual, void* dx, float* dgamma, float* dbeta, float* partials,
                      void* stream);
+
+/*
+ * The same block with the LayerNorms FUSED into the layer's own row kernels ("post-LN + depth multiplier +
+ * residual fused into combine"; Eq. 15, 601):
+ *   fomoe_moe_fwd_periln = fomoe_moe_fwd, whose combine also writes  out = residual + alpha LN(y)  and stats (y is still written: the
+ *       post-LN backward reads it).  Bit-identical to fomoe_moe_fwd followed by fomoe_periln_fwd(y, gamma, beta, eps, residual, alpha).
+ *   fomoe_moe_bwd_periln = fomoe_moe_bwd, whose final scatter-sum applies the PRE-LN backward to the gradient it has just summed:
+ *       dx = dresidual + LN-backward(dxn; x_raw, stats, gamma), dgamma / dbeta overwritten; dxn (the gradient w.r.t. the layer's
+ *       input tokens) is never stored.  Bit-identical to fomoe_moe_bwd followed by fomoe_periln_bwd(dxn, x_raw, stats, gamma, 1,
+ *       dresidual).  `x` stays the layer's input (the pre-LN OUTPUT); x_raw is the block input the pre-LN normalised.
+ * All pointers device, caller-owned; gamma, beta, dgamma, dbeta fp32 [d_model]; stats fp32 [T,2]; partials as for
+ * fomoe_periln_bwd.  d_model must fit the register-resident row shape (a multiple of 8 (bf16) / 4 (fp32), <= 8192 (bf16) /
+ * 4096 (fp32)): otherwise FOMOE_ERR_UNSUPPORTED and the caller runs the unfused calls.
+ */
+typedef struct {
+  const float* gamma;   /* [d_model] */
+  const float* beta;    /* [d_model] */
+  float eps;
+  float alpha;          /* depth multiplier on the normalised block output */
+  const void* residual; /* [T,d_model] block input x_l */
+  void* out;            /* [T,d_model] x_{l+1} */
+  float* stats;         /* [T,2] (mean, rstd) of y, for the post-LN backward */
+} fomoe_periln_post;
+typedef struct {
+  const void* x_raw;     /* [T,d_model] block input x_l (what the pre-LN normalised) */
+  const float* stats;    /* [T,2] written by the pre-LN forward */
+  const float* gamma;    /* [d_model] pre-LN gain */
+  const void* dresidual; /* [T,d_model] or NULL: gradient arriving through the residual branch */
+  float* dgamma;         /* [d_model] out */
+  float* dbeta;          /* [d_model] out */
+  float* partials;       /* fomoe_periln_workspace_bytes(T, d_model) bytes */
+} fomoe_periln_pre_bwd;
+FOMOE_API int fomoe_moe_fwd_periln(const fomoe_config* cfg, const void* x, const fomoe_route_state* route, int32_t n_res,
+                  const void* w_gate, const void* w_up, const void* w_down,
+                  const void* sh_gate, const void* sh_up, const void* sh_down,
+                  void* y, void* saved_acts, void* scratch, const fomoe_periln_post* ln, void* stream);
+FOMOE_API int fomoe_moe_bwd_periln(const fomoe_config* cfg, const void* dy, const void* x, const fomoe_route_state* route, int32_t n_res,
+                  const float* w_router, const void* w_gate, const void* w_up, const void* w_down,
+                  const void* sh_gate, const void* sh_up, const void* sh_down, const void* saved_acts,
+                  void* dx, float* dw_router, void* dw_gate, void* dw_up, void* dw_down,
+                  void* d_sh_gate, void* d_sh_up, void* d_sh_down, void* scratch, const fomoe_periln_pre_bwd* ln, void* stream);
 
 /*
  * Fused local AdamW over the resident experts ("workers execute AdamW locally on their

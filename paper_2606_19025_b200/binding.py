@@ -28,7 +28,7 @@ EXPORTS = ("fomoe_workspace_bytes", "fomoe_route", "fomoe_moe_fwd", "fomoe_moe_b
            "fomoe_adamw_resident", "fomoe_outer_nesterov", "fomoe_periln_workspace_bytes", "fomoe_periln_fwd", "fomoe_periln_bwd",
            "fomoe_moe_step_host", "fomoe_last_launch_count", "fomoe_last_cuda_error", "fomoe_abi_version",
            "fomoe_set_force_simt", "fomoe_profile_enable", "fomoe_profile_collect", "fomoe_debug_validate_resident",
-           "fomoe_routing_stats")
+           "fomoe_routing_stats", "fomoe_moe_fwd_periln", "fomoe_moe_bwd_periln")
 STAT_NAMES = ("kept_fraction", "ghost_fraction", "zero_kept_tokens", "load_cv", "routing_entropy", "max_load", "min_load")
 
 
@@ -41,6 +41,16 @@ class fomoe_config(C.Structure):
 class fomoe_route_state(C.Structure):
     _fields_ = [("topk_idx", C.c_void_p), ("gate", C.c_void_p), ("probs", C.c_void_p), ("counts", C.c_void_p),
                 ("offsets", C.c_void_p), ("row_token", C.c_void_p), ("pair_row", C.c_void_p), ("internal", C.c_void_p)]
+
+
+class fomoe_periln_post(C.Structure):
+    _fields_ = [("gamma", C.c_void_p), ("beta", C.c_void_p), ("eps", C.c_float), ("alpha", C.c_float), ("residual", C.c_void_p),
+                ("out", C.c_void_p), ("stats", C.c_void_p)]
+
+
+class fomoe_periln_pre_bwd(C.Structure):
+    _fields_ = [("x_raw", C.c_void_p), ("stats", C.c_void_p), ("gamma", C.c_void_p), ("dresidual", C.c_void_p), ("dgamma", C.c_void_p),
+                ("dbeta", C.c_void_p), ("partials", C.c_void_p)]
 
 
 class FomoeError(RuntimeError):
@@ -60,7 +70,7 @@ def lib() -> C.CDLL:
         for name in EXPORTS:
             getattr(_lib, name).restype = C.c_int
         _lib.fomoe_last_cuda_error.restype = C.c_char_p
-        if _lib.fomoe_abi_version() != 4:
+        if _lib.fomoe_abi_version() != 5:
             raise FomoeError("libfomoe.so ABI version mismatch")
     return _lib
 
@@ -145,6 +155,39 @@ def fomoe_moe_bwd(cfg, dy, x, route: RouteState, n_res, w_router, w_gate, w_up, 
     _check(lib().fomoe_moe_bwd(C.byref(cfg), _p(dy), _p(x), C.byref(rs), C.c_int32(n_res), _p(w_router), _p(w_gate), _p(w_up),
                                _p(w_down), _p(sg), _p(su), _p(sd), _p(saved_acts), _p(dx), _p(dw_router), _p(dw_gate), _p(dw_up),
                                _p(dw_down), _p(dsg), _p(dsu), _p(dsd), _p(scratch), _stream(stream)), "fomoe_moe_bwd")
+
+
+def fomoe_periln_fused_supported(cfg) -> bool:
+    """Whether d_model fits the register-resident row shape of the fused Peri-LN forms (host-side shape rule of fomoe.h)."""
+    vn = 8 if cfg.dtype == FOMOE_BF16 else 4
+    return cfg.d_model % vn == 0 and cfg.d_model // vn <= 1024
+
+
+def _dp(t: Optional[torch.Tensor]):
+    return None if t is None else t.data_ptr()
+
+
+def fomoe_moe_fwd_periln(cfg, x, route: RouteState, n_res, w_gate, w_up, w_down, shared, y, saved_acts, scratch, gamma, beta, residual,
+                         out, stats, alpha=1.0, eps=1e-5, stream=None) -> None:
+    """fomoe_moe_fwd whose combine also applies the post-LN, the depth multiplier and the residual (Eq. 15)."""
+    rs = route.c_struct()
+    sg, su, sd = shared if shared is not None else (None, None, None)
+    ln = fomoe_periln_post(_dp(gamma), _dp(beta), eps, alpha, _dp(residual), _dp(out), _dp(stats))
+    _check(lib().fomoe_moe_fwd_periln(C.byref(cfg), _p(x), C.byref(rs), C.c_int32(n_res), _p(w_gate), _p(w_up), _p(w_down), _p(sg), _p(su),
+                                      _p(sd), _p(y), _p(saved_acts), _p(scratch), C.byref(ln), _stream(stream)), "fomoe_moe_fwd_periln")
+
+
+def fomoe_moe_bwd_periln(cfg, dy, x, route: RouteState, n_res, w_router, w_gate, w_up, w_down, shared, saved_acts, dx, dw_router, dw_gate,
+                         dw_up, dw_down, d_shared, scratch, x_raw, stats, gamma, dresidual, dgamma, dbeta, partials, stream=None) -> None:
+    """fomoe_moe_bwd whose scatter-sum also applies the pre-LN backward and adds the residual-branch gradient."""
+    rs = route.c_struct()
+    sg, su, sd = shared if shared is not None else (None, None, None)
+    dsg, dsu, dsd = d_shared if d_shared is not None else (None, None, None)
+    ln = fomoe_periln_pre_bwd(_dp(x_raw), _dp(stats), _dp(gamma), _dp(dresidual), _dp(dgamma), _dp(dbeta), _dp(partials))
+    _check(lib().fomoe_moe_bwd_periln(C.byref(cfg), _p(dy), _p(x), C.byref(rs), C.c_int32(n_res), _p(w_router), _p(w_gate), _p(w_up),
+                                      _p(w_down), _p(sg), _p(su), _p(sd), _p(saved_acts), _p(dx), _p(dw_router), _p(dw_gate), _p(dw_up),
+                                      _p(dw_down), _p(dsg), _p(dsu), _p(dsd), _p(scratch), C.byref(ln), _stream(stream)),
+           "fomoe_moe_bwd_periln")
 
 
 def fomoe_pack_resident_deltas(w_now, w_start, pack_slots, payload, stream=None) -> None:

@@ -149,9 +149,9 @@ int fomoe_route(const fomoe_config* cfg, const void* x, const float* w_router, c
   return launch_route(*cfg, x, w_router, router_bias, resident_ids, n_res, *out, ws, (cudaStream_t)stream);
 }
 
-int fomoe_moe_fwd(const fomoe_config* cfg, const void* x, const fomoe_route_state* route, int32_t n_res, const void* w_gate,
-                  const void* w_up, const void* w_down, const void* sh_gate, const void* sh_up, const void* sh_down, void* y,
-                  void* saved_acts, void* scratch, void* stream) {
+static int moe_fwd_impl(const fomoe_config* cfg, const void* x, const fomoe_route_state* route, int32_t n_res, const void* w_gate,
+                        const void* w_up, const void* w_down, const void* sh_gate, const void* sh_up, const void* sh_down, void* y,
+                        void* saved_acts, void* scratch, const fomoe_periln_post* ln, void* stream) {
   g_launches = 0;
   int rc = check_cfg(cfg, n_res);
   if (rc != FOMOE_OK) return rc;
@@ -175,13 +175,31 @@ int fomoe_moe_fwd(const fomoe_config* cfg, const void* x, const fomoe_route_stat
   }
   rc = use_umma(*cfg) ? umma_ffn_fwd(*cfg, n_res, x, rws, aws, sws, w, st) : simt_ffn_fwd(*cfg, n_res, x, rws, aws, sws, w, st);
   if (rc != FOMOE_OK) return rc;
+  if (ln) return launch_combine_periln(*cfg, *route, rws, aws.o, cfg->n_shared > 0 ? sws.y_sh : nullptr, y, *ln, st);
   return launch_combine(*cfg, *route, rws, aws.o, cfg->n_shared > 0 ? sws.y_sh : nullptr, y, st);
 }
 
-int fomoe_moe_bwd(const fomoe_config* cfg, const void* dy, const void* x, const fomoe_route_state* route, int32_t n_res,
-                  const float* w_router, const void* w_gate, const void* w_up, const void* w_down, const void* sh_gate,
-                  const void* sh_up, const void* sh_down, const void* saved_acts, void* dx, float* dw_router, void* dw_gate,
-                  void* dw_up, void* dw_down, void* d_sh_gate, void* d_sh_up, void* d_sh_down, void* scratch, void* stream) {
+int fomoe_moe_fwd(const fomoe_config* cfg, const void* x, const fomoe_route_state* route, int32_t n_res, const void* w_gate,
+                  const void* w_up, const void* w_down, const void* sh_gate, const void* sh_up, const void* sh_down, void* y,
+                  void* saved_acts, void* scratch, void* stream) {
+  return moe_fwd_impl(cfg, x, route, n_res, w_gate, w_up, w_down, sh_gate, sh_up, sh_down, y, saved_acts, scratch, nullptr, stream);
+}
+
+int fomoe_moe_fwd_periln(const fomoe_config* cfg, const void* x, const fomoe_route_state* route, int32_t n_res, const void* w_gate,
+                         const void* w_up, const void* w_down, const void* sh_gate, const void* sh_up, const void* sh_down, void* y,
+                         void* saved_acts, void* scratch, const fomoe_periln_post* ln, void* stream) {
+  if (!cfg || !ln || !ln->gamma || !ln->beta || !(ln->eps >= 0.f)) return FOMOE_ERR_BADARG;
+  if (cfg->T > 0 && (!ln->residual || !ln->out || !ln->stats)) return FOMOE_ERR_BADARG;
+  if (!aligned16(ln->residual) || !aligned16(ln->out) || !aligned16(ln->gamma) || !aligned16(ln->beta)) return FOMOE_ERR_BADARG;
+  if (cfg->d_model > 0 && (cfg->dtype == FOMOE_F32 || cfg->dtype == FOMOE_BF16) && !periln_fused_supported(*cfg)) return FOMOE_ERR_UNSUPPORTED;
+  return moe_fwd_impl(cfg, x, route, n_res, w_gate, w_up, w_down, sh_gate, sh_up, sh_down, y, saved_acts, scratch, ln, stream);
+}
+
+static int moe_bwd_impl(const fomoe_config* cfg, const void* dy, const void* x, const fomoe_route_state* route, int32_t n_res,
+                        const float* w_router, const void* w_gate, const void* w_up, const void* w_down, const void* sh_gate,
+                        const void* sh_up, const void* sh_down, const void* saved_acts, void* dx, float* dw_router, void* dw_gate,
+                        void* dw_up, void* dw_down, void* d_sh_gate, void* d_sh_up, void* d_sh_down, void* scratch,
+                        const fomoe_periln_pre_bwd* ln, void* stream) {
   g_launches = 0;
   int rc = check_cfg(cfg, n_res);
   if (rc != FOMOE_OK) return rc;
@@ -245,9 +263,32 @@ int fomoe_moe_bwd(const fomoe_config* cfg, const void* dy, const void* x, const 
     if (rc == FOMOE_OK && e2 != cudaSuccess) return set_cuda_error(e2, "cudaStreamWaitEvent(join)");
   }
   if (rc != FOMOE_OK) return rc;
-  // B5
+  // B5 (with the pre-LN backward folded in when asked for)
+  if (ln) return launch_dx_sum_periln(*cfg, rws, sws.dxp, cfg->n_shared > 0 ? sws.dx_sh : nullptr, tc_router ? nullptr : sws.dx_r,
+                                      tc_router ? (const void*)sws.dx_r : nullptr, *ln, dx, st);
   return launch_dx_sum(*cfg, rws, sws.dxp, cfg->n_shared > 0 ? sws.dx_sh : nullptr, tc_router ? nullptr : sws.dx_r,
                        tc_router ? (const void*)sws.dx_r : nullptr, dx, st);
+}
+
+int fomoe_moe_bwd(const fomoe_config* cfg, const void* dy, const void* x, const fomoe_route_state* route, int32_t n_res,
+                  const float* w_router, const void* w_gate, const void* w_up, const void* w_down, const void* sh_gate,
+                  const void* sh_up, const void* sh_down, const void* saved_acts, void* dx, float* dw_router, void* dw_gate,
+                  void* dw_up, void* dw_down, void* d_sh_gate, void* d_sh_up, void* d_sh_down, void* scratch, void* stream) {
+  return moe_bwd_impl(cfg, dy, x, route, n_res, w_router, w_gate, w_up, w_down, sh_gate, sh_up, sh_down, saved_acts, dx, dw_router, dw_gate,
+                      dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, scratch, nullptr, stream);
+}
+
+int fomoe_moe_bwd_periln(const fomoe_config* cfg, const void* dy, const void* x, const fomoe_route_state* route, int32_t n_res,
+                         const float* w_router, const void* w_gate, const void* w_up, const void* w_down, const void* sh_gate,
+                         const void* sh_up, const void* sh_down, const void* saved_acts, void* dx, float* dw_router, void* dw_gate,
+                         void* dw_up, void* dw_down, void* d_sh_gate, void* d_sh_up, void* d_sh_down, void* scratch,
+                         const fomoe_periln_pre_bwd* ln, void* stream) {
+  if (!cfg || !ln || !ln->gamma || !ln->dgamma || !ln->dbeta || !ln->partials) return FOMOE_ERR_BADARG;
+  if (cfg->T > 0 && (!ln->x_raw || !ln->stats)) return FOMOE_ERR_BADARG;
+  if (!aligned16(ln->x_raw) || !aligned16(ln->dresidual) || !aligned16(ln->gamma)) return FOMOE_ERR_BADARG;
+  if (cfg->d_model > 0 && (cfg->dtype == FOMOE_F32 || cfg->dtype == FOMOE_BF16) && !periln_fused_supported(*cfg)) return FOMOE_ERR_UNSUPPORTED;
+  return moe_bwd_impl(cfg, dy, x, route, n_res, w_router, w_gate, w_up, w_down, sh_gate, sh_up, sh_down, saved_acts, dx, dw_router, dw_gate,
+                      dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, scratch, ln, stream);
 }
 
 int fomoe_pack_resident_deltas(const float* const w_now[3], const float* const w_start[3], int32_t n_res, int64_t elems_gate,

@@ -281,6 +281,13 @@ int launch_periln_fwd(int T, int d, int dtype, const void* x, const float* gamma
 int launch_periln_bwd(int T, int d, int dtype, const void* dout, const void* x, const float* stats, const float* gamma, float alpha,
                       const void* dresidual, void* dx, float* dgamma, float* dbeta, float* partials, cudaStream_t st);
 
+// fused forms (periln.cu): combine + post-LN + residual, dx scatter-sum + pre-LN backward + residual
+bool periln_fused_supported(const fomoe_config& c);
+int launch_combine_periln(const fomoe_config& c, const fomoe_route_state& r, const RouteWs& ws, const void* o, const void* y_sh, void* y,
+                          const fomoe_periln_post& ln, cudaStream_t st);
+int launch_dx_sum_periln(const fomoe_config& c, const RouteWs& ws, const void* dxp, const void* dx_sh, const float* dx_r, const void* dx_r_t,
+                         const fomoe_periln_pre_bwd& ln, void* dx, cudaStream_t st);
+
 // optimizer steps around the pack (optim.cu)
 int launch_adamw(float* const w[3], const void* const g[3], float* const m[3], float* const v[3], void* const wc[3], int dtype,
                  int n_res, const int64_t elems[3], int step, float lr, float b1, float b2, float eps, float wd, cudaStream_t st);

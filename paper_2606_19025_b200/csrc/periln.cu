@@ -25,6 +25,26 @@ __device__ __forceinline__ float block_sum(float v, float* red) {
   return s;
 }
 
+// The element formulas, with every rounding spelled out (no compiler-chosen FMA contraction): the stand-alone kernels and the
+// forms fused into combine / dx_sum (below) must produce the same bits.
+__device__ __forceinline__ float ln_out(float centred, float rstd, float g, float b, float alpha, bool has_res, float res) {
+  const float t = __fmaf_rn(g, __fmul_rn(centred, rstd), b);
+  return has_res ? __fmaf_rn(alpha, t, res) : __fmul_rn(alpha, t);
+}
+__device__ __forceinline__ float ln_dx(float rstd, float dxhat, float m1, float xhat, float m2, bool has_res, float res) {
+  const float t = __fmul_rn(rstd, __fmaf_rn(-xhat, m2, __fsub_rn(dxhat, m1)));
+  return has_res ? __fadd_rn(t, res) : t;
+}
+// accumulates one element into (dgamma, dbeta, sum dxhat, sum dxhat xhat); returns dxhat = go * gamma
+__device__ __forceinline__ float ln_bwd_acc(float go, float xhat, float g, float& ag, float& ab, float& s1, float& s2) {
+  ag = __fmaf_rn(go, xhat, ag);
+  ab = __fadd_rn(ab, go);
+  const float dxh = __fmul_rn(go, g);
+  s1 = __fadd_rn(s1, dxh);
+  s2 = __fmaf_rn(dxh, xhat, s2);
+  return dxh;
+}
+
 // 16-byte vector access: VN elements of T as fp32 (bf16: 8, fp32: 4)
 template <typename T> struct VecN { static constexpr int n = 16 / sizeof(T); };
 template <typename T> __device__ __forceinline__ void ldv(const T* p, float (&v)[VecN<T>::n]);
@@ -81,16 +101,12 @@ periln_fwd_kernel(const T* __restrict__ x, const float* __restrict__ gamma, cons
         float v[VN], r[VN];
         if (residual) ldv<T>(residual + (size_t)t * d + c, r);
 #pragma unroll
-        for (int i = 0; i < VN; ++i) {
-          v[i] = alpha * (gamma[c + i] * ((row[c + i] - mean) * rstd) + beta[c + i]);
-          if (residual) v[i] += r[i];
-        }
+        for (int i = 0; i < VN; ++i) v[i] = ln_out(row[c + i] - mean, rstd, gamma[c + i], beta[c + i], alpha, residual != nullptr, residual ? r[i] : 0.f);
         stv<T>(out + (size_t)t * d + c, v);
       }
     } else {
       for (int c = threadIdx.x; c < d; c += kLnThreads) {
-        float v = alpha * (gamma[c] * ((row[c] - mean) * rstd) + beta[c]);
-        if (residual) v += to_f32(residual[(size_t)t * d + c]);
+        const float v = ln_out(row[c] - mean, rstd, gamma[c], beta[c], alpha, residual != nullptr, residual ? to_f32(residual[(size_t)t * d + c]) : 0.f);
         out[(size_t)t * d + c] = from_f32<T>(v);
       }
     }
@@ -119,22 +135,17 @@ periln_bwd_kernel(const T* __restrict__ dout, const T* __restrict__ x, const flo
         ldv<T>(x + (size_t)t * d + c, xv);
 #pragma unroll
         for (int i = 0; i < VN; ++i) {
-          const float g = alpha * go[i], h = (xv[i] - mean) * rstd, dh = g * gamma[c + i];
-          xh[c + i] = h; dxh[c + i] = dh;
-          ag[c + i] += g * h;
-          ab[c + i] += g;
-          s1 += dh; s2 += dh * h;
+          const float g = __fmul_rn(alpha, go[i]), h = __fmul_rn(xv[i] - mean, rstd);
+          xh[c + i] = h;
+          dxh[c + i] = ln_bwd_acc(g, h, gamma[c + i], ag[c + i], ab[c + i], s1, s2);
         }
       }
     } else {
       for (int c = threadIdx.x; c < d; c += kLnThreads) {
-        const float go = alpha * to_f32(dout[(size_t)t * d + c]);
-        const float h = (to_f32(x[(size_t)t * d + c]) - mean) * rstd;
-        const float dh = go * gamma[c];
-        xh[c] = h; dxh[c] = dh;
-        ag[c] += go * h;               // each column is owned by one thread: no atomics, fixed token order
-        ab[c] += go;
-        s1 += dh; s2 += dh * h;
+        const float go = __fmul_rn(alpha, to_f32(dout[(size_t)t * d + c]));
+        const float h = __fmul_rn(to_f32(x[(size_t)t * d + c]) - mean, rstd);
+        xh[c] = h;
+        dxh[c] = ln_bwd_acc(go, h, gamma[c], ag[c], ab[c], s1, s2);   // each column is owned by one thread: no atomics, fixed token order
       }
     }
     const float m1 = block_sum(s1, red) / (float)d;
@@ -144,16 +155,12 @@ periln_bwd_kernel(const T* __restrict__ dout, const T* __restrict__ x, const flo
         float v[VN], r[VN];
         if (dresidual) ldv<T>(dresidual + (size_t)t * d + c, r);
 #pragma unroll
-        for (int i = 0; i < VN; ++i) {
-          v[i] = rstd * (dxh[c + i] - m1 - xh[c + i] * m2);
-          if (dresidual) v[i] += r[i];
-        }
+        for (int i = 0; i < VN; ++i) v[i] = ln_dx(rstd, dxh[c + i], m1, xh[c + i], m2, dresidual != nullptr, dresidual ? r[i] : 0.f);
         stv<T>(dx + (size_t)t * d + c, v);
       }
     } else {
       for (int c = threadIdx.x; c < d; c += kLnThreads) {
-        float v = rstd * (dxh[c] - m1 - xh[c] * m2);
-        if (dresidual) v += to_f32(dresidual[(size_t)t * d + c]);
+        const float v = ln_dx(rstd, dxh[c], m1, xh[c], m2, dresidual != nullptr, dresidual ? to_f32(dresidual[(size_t)t * d + c]) : 0.f);
         dx[(size_t)t * d + c] = from_f32<T>(v);
       }
     }
@@ -167,19 +174,21 @@ periln_bwd_kernel(const T* __restrict__ dout, const T* __restrict__ x, const flo
 
 // ---- register-resident variants (d a multiple of the vector width, at most NV vectors per thread): the row never touches
 // shared memory, gamma and the dgamma / dbeta accumulators live in registers across the CTA's tokens ----
+// gamma / beta are re-read per token (16-byte loads, L1-resident) instead of living in registers: the register count decides how
+// many rows an SM keeps in flight, and these kernels are bound by exactly that
+template <typename T, int VN> __device__ __forceinline__ void ld_param(const float* p, float (&v)[VN]) {
+  ldv<float>(p, *reinterpret_cast<float(*)[4]>(&v[0]));
+  if constexpr (VN == 8) ldv<float>(p + 4, *reinterpret_cast<float(*)[4]>(&v[4]));
+}
+
 template <typename T, int NV>
-__global__ void __launch_bounds__(kLnThreads)
+__global__ void __launch_bounds__(kLnThreads, 4)
 periln_fwd_reg_kernel(const T* __restrict__ x, const float* __restrict__ gamma, const float* __restrict__ beta, const T* __restrict__ residual,
                       float alpha, float eps, int T_, int d, T* __restrict__ out, float* __restrict__ stats) {
   constexpr int VN = VecN<T>::n;
   __shared__ float red[kLnThreads / 32];
-  float g[NV][VN], b[NV][VN];
-#pragma unroll
-  for (int j = 0; j < NV; ++j) {
-    const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
-#pragma unroll
-    for (int i = 0; i < VN; ++i) { g[j][i] = c < d ? gamma[c + i] : 0.f; b[j][i] = c < d ? beta[c + i] : 0.f; }
-  }
+  pdl_launch_dependents();
+  pdl_wait();
   for (int t = blockIdx.x; t < T_; t += gridDim.x) {
     const size_t base = (size_t)t * d;
     float v[NV][VN], r[NV][VN];
@@ -190,6 +199,12 @@ periln_fwd_reg_kernel(const T* __restrict__ x, const float* __restrict__ gamma, 
       if (c < d) {
         ldv<T>(x + base + c, v[j]);
         if (residual) ldv<T>(residual + base + c, r[j]);
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
+      if (c < d) {
 #pragma unroll
         for (int i = 0; i < VN; ++i) s += v[j][i];
       }
@@ -210,11 +225,11 @@ periln_fwd_reg_kernel(const T* __restrict__ x, const float* __restrict__ gamma, 
     for (int j = 0; j < NV; ++j) {
       const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
       if (c < d) {
+        float g[VN], b[VN];
+        ld_param<T, VN>(gamma + c, g);
+        ld_param<T, VN>(beta + c, b);
 #pragma unroll
-        for (int i = 0; i < VN; ++i) {
-          v[j][i] = alpha * (g[j][i] * (v[j][i] * rstd) + b[j][i]);
-          if (residual) v[j][i] += r[j][i];
-        }
+        for (int i = 0; i < VN; ++i) v[j][i] = ln_out(v[j][i], rstd, g[i], b[i], alpha, residual != nullptr, residual ? r[j][i] : 0.f);
         stv<T>(out + base + c, v[j]);
       }
     }
@@ -227,6 +242,8 @@ periln_bwd_reg_kernel(const T* __restrict__ dout, const T* __restrict__ x, const
                       float alpha, const T* __restrict__ dresidual, int T_, int d, T* __restrict__ dx, float* __restrict__ partials) {
   constexpr int VN = VecN<T>::n;
   __shared__ float red[kLnThreads / 32];
+  pdl_launch_dependents();
+  pdl_wait();
   float g[NV][VN], ag[NV][VN], ab[NV][VN];
 #pragma unroll
   for (int j = 0; j < NV; ++j) {
@@ -246,15 +263,17 @@ periln_bwd_reg_kernel(const T* __restrict__ dout, const T* __restrict__ x, const
         ldv<T>(dout + base + c, dh[j]);
         ldv<T>(x + base + c, h[j]);
         if (dresidual) ldv<T>(dresidual + base + c, r[j]);
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
+      if (c < d) {
 #pragma unroll
         for (int i = 0; i < VN; ++i) {
-          const float go = alpha * dh[j][i];
-          h[j][i] = (h[j][i] - mean) * rstd;
-          ag[j][i] += go * h[j][i];          // fixed token order per CTA
-          ab[j][i] += go;
-          dh[j][i] = go * g[j][i];
-          s1 += dh[j][i];
-          s2 += dh[j][i] * h[j][i];
+          const float go = __fmul_rn(alpha, dh[j][i]);
+          h[j][i] = __fmul_rn(h[j][i] - mean, rstd);
+          dh[j][i] = ln_bwd_acc(go, h[j][i], g[j][i], ag[j][i], ab[j][i], s1, s2);   // fixed token order per CTA
         }
       }
     }
@@ -265,10 +284,7 @@ periln_bwd_reg_kernel(const T* __restrict__ dout, const T* __restrict__ x, const
       const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
       if (c < d) {
 #pragma unroll
-        for (int i = 0; i < VN; ++i) {
-          dh[j][i] = rstd * (dh[j][i] - m1 - h[j][i] * m2);
-          if (dresidual) dh[j][i] += r[j][i];
-        }
+        for (int i = 0; i < VN; ++i) dh[j][i] = ln_dx(rstd, dh[j][i], m1, h[j][i], m2, dresidual != nullptr, dresidual ? r[j][i] : 0.f);
         stv<T>(dx + base + c, dh[j]);
       }
     }
@@ -276,6 +292,198 @@ periln_bwd_reg_kernel(const T* __restrict__ dout, const T* __restrict__ x, const
 #pragma unroll
   for (int j = 0; j < NV; ++j) {
     const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
+    if (c < d) {
+#pragma unroll
+      for (int i = 0; i < VN; ++i) {
+        partials[((size_t)blockIdx.x * 2) * d + c + i] = ag[j][i];
+        partials[((size_t)blockIdx.x * 2 + 1) * d + c + i] = ab[j][i];
+      }
+    }
+  }
+}
+
+// ---- fused into the MoE layer's own row kernels (SURVEY.md §8(f) row 3 as written: "post-LN + depth multiplier + residual
+// fused into combine"; the pre-LN backward + residual into the dx scatter-sum).  A CTA holds a whole token row in registers
+// either way, so the LayerNorm statistics cost two block reductions and no extra pass over [T, d].  The sums run in exactly
+// the order of combine_kernel / dx_sum_kernel (rows.cu) and the LayerNorm is applied to the value ROUNDED to the storage type,
+// so the fused path is bit-identical to combine -> fomoe_periln_fwd and dx_sum -> fomoe_periln_bwd. ----
+
+// y[t] = sum_j gate[t,j] o[pair_prow[t,j]] (+ y_sh[t])  (saved: the post-LN backward needs it);
+// out[t] = residual[t] + alpha (gamma xhat(y[t]) + beta); stats[t] = (mean, rstd)
+template <typename T, int NV, int THREADS>
+__global__ void __launch_bounds__(THREADS, NV <= 2 ? 1024 / THREADS : 1)
+combine_periln_kernel(const T* __restrict__ o, const T* __restrict__ y_sh, const float* __restrict__ gate, const int32_t* __restrict__ pair_prow,
+                      int T_, int d, int k, T* __restrict__ y, const float* __restrict__ gamma, const float* __restrict__ beta,
+                      const T* __restrict__ residual, float alpha, float eps, T* __restrict__ out, float* __restrict__ stats) {
+  constexpr int VN = VecN<T>::n;
+  __shared__ float red[THREADS / 32];
+  pdl_launch_dependents();
+  pdl_wait();
+  for (int t = blockIdx.x; t < T_; t += gridDim.x) {
+    const size_t base = (size_t)t * d;
+    float v[NV][VN];
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * THREADS + threadIdx.x) * VN;
+      if (c < d && y_sh) ldv<T>(y_sh + base + c, v[j]);
+      else {
+#pragma unroll
+        for (int i = 0; i < VN; ++i) v[j][i] = 0.f;
+      }
+    }
+    for (int jj = 0; jj < k; ++jj) {          // ascending j: the order of combine_kernel
+      const int r = pair_prow[(size_t)t * k + jj];
+      if (r < 0) continue;
+      const float g = gate[(size_t)t * k + jj];
+#pragma unroll
+      for (int j = 0; j < NV; ++j) {
+        const int c = (j * THREADS + threadIdx.x) * VN;
+        if (c < d) {
+          float a[VN];
+          ldv<T>(o + (size_t)r * d + c, a);
+#pragma unroll
+          for (int i = 0; i < VN; ++i) v[j][i] = fmaf(g, a[i], v[j][i]);
+        }
+      }
+    }
+    float rres[NV][VN];                        // residual row: requested before the reductions
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * THREADS + threadIdx.x) * VN;
+      if (c < d) ldv<T>(residual + base + c, rres[j]);
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * THREADS + threadIdx.x) * VN;
+      if (c < d) {
+        stv<T>(y + base + c, v[j]);
+#pragma unroll
+        for (int i = 0; i < VN; ++i) { v[j][i] = to_f32(from_f32<T>(v[j][i])); s += v[j][i]; }   // LayerNorm of what was stored
+      }
+    }
+    const float mean = block_sum(s, red) / (float)d;
+    float q = 0.f;
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * THREADS + threadIdx.x) * VN;
+      if (c < d) {
+#pragma unroll
+        for (int i = 0; i < VN; ++i) { v[j][i] -= mean; q += v[j][i] * v[j][i]; }
+      }
+    }
+    const float rstd = rsqrtf(block_sum(q, red) / (float)d + eps);
+    if (threadIdx.x == 0) { stats[2 * (size_t)t] = mean; stats[2 * (size_t)t + 1] = rstd; }
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * THREADS + threadIdx.x) * VN;
+      if (c < d) {
+        float gm[VN], bt[VN];
+        ldv<float>(gamma + c, *reinterpret_cast<float(*)[4]>(&gm[0]));
+        ldv<float>(beta + c, *reinterpret_cast<float(*)[4]>(&bt[0]));
+        if constexpr (VN == 8) {
+          ldv<float>(gamma + c + 4, *reinterpret_cast<float(*)[4]>(&gm[4]));
+          ldv<float>(beta + c + 4, *reinterpret_cast<float(*)[4]>(&bt[4]));
+        }
+#pragma unroll
+        for (int i = 0; i < VN; ++i) v[j][i] = ln_out(v[j][i], rstd, gm[i], bt[i], alpha, true, rres[j][i]);
+        stv<T>(out + base + c, v[j]);
+      }
+    }
+  }
+}
+
+// dxn[t] = sum_j dxp[pair_prow[t,j]] + dx_sh[t] + dx_r[t]  (gradient w.r.t. the pre-LN output; never stored);
+// dx[t] = dresidual[t] + LN backward of dxn[t] at (x_raw[t], stats[t], gamma); per-CTA partial dgamma / dbeta
+template <typename T, int NV, int THREADS>
+__global__ void __launch_bounds__(THREADS, NV <= 2 ? 512 / THREADS : 1)
+dx_sum_periln_kernel(const T* __restrict__ dxp, const T* __restrict__ dx_sh, const float* __restrict__ dx_r, const T* __restrict__ dx_r_t,
+                     const int32_t* __restrict__ pair_prow, int T_, int d, int k, const T* __restrict__ x_raw, const float* __restrict__ stats,
+                     const float* __restrict__ gamma, const T* __restrict__ dresidual, T* __restrict__ dx, float* __restrict__ partials) {
+  constexpr int VN = VecN<T>::n;
+  __shared__ float red[THREADS / 32];
+  pdl_launch_dependents();
+  pdl_wait();
+  float ag[NV][VN], ab[NV][VN];
+#pragma unroll
+  for (int j = 0; j < NV; ++j)
+#pragma unroll
+    for (int i = 0; i < VN; ++i) { ag[j][i] = 0.f; ab[j][i] = 0.f; }
+  for (int t = blockIdx.x; t < T_; t += gridDim.x) {
+    const size_t base = (size_t)t * d;
+    float dh[NV][VN], h[NV][VN];
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * THREADS + threadIdx.x) * VN;
+      if (c < d && dx_sh) ldv<T>(dx_sh + base + c, dh[j]);
+      else {
+#pragma unroll
+        for (int i = 0; i < VN; ++i) dh[j][i] = 0.f;
+      }
+      if (c < d) ldv<T>(x_raw + base + c, h[j]);
+    }
+    float rres[NV][VN];                        // residual-branch gradient: requested early, used last
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * THREADS + threadIdx.x) * VN;
+      if (c < d && dresidual) ldv<T>(dresidual + base + c, rres[j]);
+    }
+    for (int jj = 0; jj < k; ++jj) {          // the order of dx_sum_kernel
+      const int r = pair_prow[(size_t)t * k + jj];
+      if (r < 0) continue;
+#pragma unroll
+      for (int j = 0; j < NV; ++j) {
+        const int c = (j * THREADS + threadIdx.x) * VN;
+        if (c < d) {
+          float a[VN];
+          ldv<T>(dxp + (size_t)r * d + c, a);
+#pragma unroll
+          for (int i = 0; i < VN; ++i) dh[j][i] += a[i];
+        }
+      }
+    }
+    const float mean = stats[2 * (size_t)t], rstd = stats[2 * (size_t)t + 1];
+    float s1 = 0.f, s2 = 0.f;
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * THREADS + threadIdx.x) * VN;
+      if (c < d) {
+        if (dx_r) {
+#pragma unroll
+          for (int i = 0; i < VN; ++i) dh[j][i] += dx_r[base + c + i];
+        }
+        if (dx_r_t) {
+          float a[VN];
+          ldv<T>(dx_r_t + base + c, a);
+#pragma unroll
+          for (int i = 0; i < VN; ++i) dh[j][i] += a[i];
+        }
+        float gm[VN];
+        ldv<float>(gamma + c, *reinterpret_cast<float(*)[4]>(&gm[0]));
+        if constexpr (VN == 8) ldv<float>(gamma + c + 4, *reinterpret_cast<float(*)[4]>(&gm[4]));
+#pragma unroll
+        for (int i = 0; i < VN; ++i) {
+          const float go = to_f32(from_f32<T>(dh[j][i]));      // what dx_sum_kernel would have stored (alpha = 1)
+          h[j][i] = __fmul_rn(h[j][i] - mean, rstd);
+          dh[j][i] = ln_bwd_acc(go, h[j][i], gm[i], ag[j][i], ab[j][i], s1, s2);   // fixed token order per CTA
+        }
+      }
+    }
+    const float m1 = block_sum(s1, red) / (float)d;
+    const float m2 = block_sum(s2, red) / (float)d;
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * THREADS + threadIdx.x) * VN;
+      if (c < d) {
+#pragma unroll
+        for (int i = 0; i < VN; ++i) dh[j][i] = ln_dx(rstd, dh[j][i], m1, h[j][i], m2, dresidual != nullptr, dresidual ? rres[j][i] : 0.f);
+        stv<T>(dx + base + c, dh[j]);
+      }
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < NV; ++j) {
+    const int c = (j * THREADS + threadIdx.x) * VN;
     if (c < d) {
 #pragma unroll
       for (int i = 0; i < VN; ++i) {
@@ -342,7 +550,7 @@ static int periln_fwd_t(int Tn, int d, const void* x, const float* gamma, const 
   int threads, nv;
   reg_shape<T>(d, threads, nv);
   const int grid = Tn < num_sms() * 16 ? Tn : num_sms() * 16;
-#define LN_FWD(NV) periln_fwd_reg_kernel<T, NV><<<grid, threads, 0, st>>>((const T*)x, gamma, beta, (const T*)residual, alpha, eps, Tn, d, (T*)out, stats)
+#define LN_FWD(NV) FOMOE_CUDA_OK(launch_pdl(periln_fwd_reg_kernel<T, NV>, grid, threads, 0, st, (const T*)x, gamma, beta, (const T*)residual, alpha, eps, Tn, d, (T*)out, stats))
   if (nv == 1) LN_FWD(1);
   else if (nv == 2) LN_FWD(2);
   else if (nv == 4) LN_FWD(4);
@@ -368,7 +576,7 @@ static int periln_bwd_t(int Tn, int d, int nb, const void* dout, const void* x, 
                         const void* dresidual, void* dx, float* partials, cudaStream_t st) {
   int threads, nv;
   reg_shape<T>(d, threads, nv);
-#define LN_BWD(NV) periln_bwd_reg_kernel<T, NV><<<nb, threads, 0, st>>>((const T*)dout, (const T*)x, stats, gamma, alpha, (const T*)dresidual, Tn, d, (T*)dx, partials)
+#define LN_BWD(NV) FOMOE_CUDA_OK(launch_pdl(periln_bwd_reg_kernel<T, NV>, nb, threads, 0, st, (const T*)dout, (const T*)x, stats, gamma, alpha, (const T*)dresidual, Tn, d, (T*)dx, partials))
   if (nv == 1) LN_BWD(1);
   else if (nv == 2) LN_BWD(2);
   else if (nv == 4) LN_BWD(4);
@@ -391,6 +599,62 @@ int launch_periln_bwd(int T, int d, int dtype, const void* dout, const void* x, 
     if (rc != FOMOE_OK) return rc;
   }
   periln_reduce_kernel<<<ceil_div(d, 32), 1024, 0, st>>>(partials, T > 0 ? nb : 0, d, dgamma, dbeta);
+  FOMOE_LAUNCH_OK("periln_reduce_kernel");
+  return FOMOE_OK;
+}
+
+// ---- launchers of the fused forms; return FOMOE_ERR_UNSUPPORTED when the row does not fit the register-resident shape
+// (the caller then runs the unfused sequence) ----
+bool periln_fused_supported(const fomoe_config& c) {
+  int threads, nv;
+  if (c.dtype == FOMOE_BF16) reg_shape<__nv_bfloat16>(c.d_model, threads, nv); else reg_shape<float>(c.d_model, threads, nv);
+  return nv != 0;
+}
+
+template <typename T>
+static int combine_periln_t(const fomoe_config& c, const fomoe_route_state& r, const RouteWs& ws, const void* o, const void* y_sh, void* y,
+                            const fomoe_periln_post& ln, cudaStream_t st) {
+  int threads, nv;
+  reg_shape<T>(c.d_model, threads, nv);
+  const int grid = c.T < num_sms() * 16 ? c.T : num_sms() * 16;
+#define CB(NV, TH) FOMOE_CUDA_OK(launch_pdl(combine_periln_kernel<T, NV, TH>, grid, TH, 0, st, (const T*)o, (const T*)y_sh, (const float*)r.gate, \
+    (const int32_t*)ws.pair_prow, c.T, c.d_model, c.top_k, (T*)y, ln.gamma, ln.beta, (const T*)ln.residual, ln.alpha, ln.eps, (T*)ln.out, ln.stats))
+  if (threads == 128) { if (nv == 1) CB(1, 128); else if (nv == 2) CB(2, 128); else return FOMOE_ERR_UNSUPPORTED; }
+  else { if (nv == 2) CB(2, 256); else if (nv == 4) CB(4, 256); else return FOMOE_ERR_UNSUPPORTED; }
+#undef CB
+  FOMOE_LAUNCH_OK("combine_periln_kernel");
+  return FOMOE_OK;
+}
+
+int launch_combine_periln(const fomoe_config& c, const fomoe_route_state& r, const RouteWs& ws, const void* o, const void* y_sh, void* y,
+                          const fomoe_periln_post& ln, cudaStream_t st) {
+  if (c.T == 0) return FOMOE_OK;
+  return c.dtype == FOMOE_BF16 ? combine_periln_t<__nv_bfloat16>(c, r, ws, o, y_sh, y, ln, st) : combine_periln_t<float>(c, r, ws, o, y_sh, y, ln, st);
+}
+
+template <typename T>
+static int dx_sum_periln_t(const fomoe_config& c, const RouteWs& ws, const void* dxp, const void* dx_sh, const float* dx_r, const void* dx_r_t,
+                           const fomoe_periln_pre_bwd& ln, void* dx, int nb, cudaStream_t st) {
+  int threads, nv;
+  reg_shape<T>(c.d_model, threads, nv);
+#define DB(NV, TH) FOMOE_CUDA_OK(launch_pdl(dx_sum_periln_kernel<T, NV, TH>, nb, TH, 0, st, (const T*)dxp, (const T*)dx_sh, dx_r, (const T*)dx_r_t, \
+    (const int32_t*)ws.pair_prow, c.T, c.d_model, c.top_k, (const T*)ln.x_raw, ln.stats, ln.gamma, (const T*)ln.dresidual, (T*)dx, ln.partials))
+  if (threads == 128) { if (nv == 1) DB(1, 128); else if (nv == 2) DB(2, 128); else return FOMOE_ERR_UNSUPPORTED; }
+  else { if (nv == 2) DB(2, 256); else if (nv == 4) DB(4, 256); else return FOMOE_ERR_UNSUPPORTED; }
+#undef DB
+  FOMOE_LAUNCH_OK("dx_sum_periln_kernel");
+  return FOMOE_OK;
+}
+
+int launch_dx_sum_periln(const fomoe_config& c, const RouteWs& ws, const void* dxp, const void* dx_sh, const float* dx_r, const void* dx_r_t,
+                         const fomoe_periln_pre_bwd& ln, void* dx, cudaStream_t st) {
+  const int nb = periln_blocks(c.T);
+  if (c.T > 0) {
+    int rc = c.dtype == FOMOE_BF16 ? dx_sum_periln_t<__nv_bfloat16>(c, ws, dxp, dx_sh, dx_r, dx_r_t, ln, dx, nb, st)
+                                   : dx_sum_periln_t<float>(c, ws, dxp, dx_sh, dx_r, dx_r_t, ln, dx, nb, st);
+    if (rc != FOMOE_OK) return rc;
+  }
+  periln_reduce_kernel<<<ceil_div(c.d_model, 32), 1024, 0, st>>>(ln.partials, c.T > 0 ? nb : 0, c.d_model, ln.dgamma, ln.dbeta);
   FOMOE_LAUNCH_OK("periln_reduce_kernel");
   return FOMOE_OK;
 }

@@ -71,6 +71,21 @@ class SkipTokenMoE:
         self.launches = B.fomoe_last_launch_count()
         return self.dx
 
+    def forward_periln(self, xn: torch.Tensor, gamma, beta, residual, out, stats, alpha=1.0, eps=1e-5, stream=None) -> torch.Tensor:
+        """Forward on the pre-LN output xn; the combine also writes out = residual + alpha LN(y) (Eq. 15)."""
+        B.fomoe_moe_fwd_periln(self.cfg, xn, self.route_state, self.n_res, self.w_gate, self.w_up, self.w_down, self.shared, self.y,
+                               self.saved_acts, self.scratch, gamma, beta, residual, out, stats, alpha, eps, stream)
+        self.launches = B.fomoe_last_launch_count()
+        return out
+
+    def backward_periln(self, dy: torch.Tensor, xn: torch.Tensor, x_raw, stats, gamma, dresidual, dgamma, dbeta, partials, stream=None):
+        """Backward whose final scatter-sum applies the pre-LN backward: self.dx = gradient w.r.t. the BLOCK input."""
+        B.fomoe_moe_bwd_periln(self.cfg, dy, xn, self.route_state, self.n_res, self.w_router, self.w_gate, self.w_up, self.w_down,
+                               self.shared, self.saved_acts, self.dx, self.dw_router, self.dw_gate, self.dw_up, self.dw_down, self.d_shared,
+                               self.scratch, x_raw, stats, gamma, dresidual, dgamma, dbeta, partials, stream)
+        self.launches = B.fomoe_last_launch_count()
+        return self.dx
+
     def step(self, x: torch.Tensor, dy: torch.Tensor, stream=None) -> int:
         """route + forward + backward on device-resident inputs; returns the number of kernels launched."""
         n = 0

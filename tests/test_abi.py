@@ -25,7 +25,7 @@ def test_exports_match_header(B):
     lib = C.CDLL(str(B.LIB_PATH))
     for name in declared:
         assert hasattr(lib, name), name
-    assert lib.fomoe_abi_version() == 4
+    assert lib.fomoe_abi_version() == 5
 
 
 def test_workspace_sizes_and_argument_checks(B):

@@ -43,9 +43,11 @@ def test_periln_fwd_bwd(dtype, T, d):
     assert torch.equal(dg, dg1)
 
 
+@pytest.mark.parametrize("fused", [False, True])
 @pytest.mark.parametrize("dtype", ["f32", "bf16"])
-def test_eq15_block_around_the_moe_layer(oracle64, dtype):
-    """out = x + alpha LN2(MoE(LN1(x))) and its backward, CUDA path vs the two oracles chained the same way."""
+def test_eq15_block_around_the_moe_layer(oracle64, dtype, fused):
+    """out = x + alpha LN2(MoE(LN1(x))) and its backward, CUDA path vs the two oracles chained the same way.  fused: the post-LN
+    runs inside the combine and the pre-LN backward inside the dx scatter-sum (fomoe_moe_fwd_periln / fomoe_moe_bwd_periln)."""
     import torch
     from paper_2606_19025_b200 import binding as B
     tol = 2e-2 if dtype == "bf16" else 1e-4
@@ -85,9 +87,12 @@ def test_eq15_block_around_the_moe_layer(oracle64, dtype):
     assert H.rel_err(H.t2n(xn), xn_ref) <= tol      # the pre-LN output on its own
     layer = H.make_layer(p)
     layer.route(xn)
-    layer.forward(xn)
     out = torch.empty_like(xd)
-    B.fomoe_periln_fwd(layer.y, g2d, b2d, out, s2, residual=xd, alpha=alpha)
+    if fused:
+        layer.forward_periln(xn, g2d, b2d, xd, out, s2, alpha=alpha)
+    else:
+        layer.forward(xn)
+        B.fomoe_periln_fwd(layer.y, g2d, b2d, out, s2, residual=xd, alpha=alpha)
     # ---- backward ----
     dout = st(rng.standard_normal((w.T, w.d)))
     dd = dev(dout)
@@ -95,8 +100,11 @@ def test_eq15_block_around_the_moe_layer(oracle64, dtype):
     dy, dx = torch.empty_like(xd), torch.empty_like(xd)
     dg2, db2, dg1, db1 = (torch.empty(w.d, device="cuda") for _ in range(4))
     B.fomoe_periln_bwd(dd, layer.y, s2, g2d, dy, dg2, db2, part, alpha=alpha)
-    layer.backward(dy, xn)
-    B.fomoe_periln_bwd(layer.dx, xd, s1, g1d, dx, dg1, db1, part, dresidual=dd)
+    if fused:
+        dx = layer.backward_periln(dy, xn, xd, s1, g1d, dd, dg1, db1, part)
+    else:
+        layer.backward(dy, xn)
+        B.fomoe_periln_bwd(layer.dx, xd, s1, g1d, dx, dg1, db1, part, dresidual=dd)
     torch.cuda.synchronize()
     # ---- oracles chained the same way (fp64) ----
     out_ref, m2, r2 = PO.periln_post_fwd(x_in, y_ref, g2, b2, alpha)
@@ -110,3 +118,67 @@ def test_eq15_block_around_the_moe_layer(oracle64, dtype):
                 dw_up=H.rel_err(H.t2n(layer.dw_up), b["dw_up"]), dw_router=H.rel_err(H.t2n(layer.dw_router), b["dw_router"]))
     print("eq15", dtype, errs)
     assert all(v <= tol for v in errs.values()), errs
+
+
+@pytest.mark.parametrize("dtype,d,n_sh", [("bf16", 128, 0), ("bf16", 1024, 1), ("f32", 200, 0), ("bf16", 4096, 0), ("f32", 2048, 1)])
+def test_fused_periln_is_the_unfused_sequence_bit_for_bit(dtype, d, n_sh):
+    """fomoe_moe_fwd_periln / fomoe_moe_bwd_periln (post-LN + alpha + residual inside the combine, pre-LN backward + residual
+    inside the dx scatter-sum, Eq. 15) against fomoe_moe_fwd -> fomoe_periln_fwd and
+    fomoe_moe_bwd -> fomoe_periln_bwd on the same inputs: every output identical, bit for bit (the unfused calls are the ones
+    the oracle parity tests cover)."""
+    import torch
+    from paper_2606_19025_b200 import binding as B
+    td = torch.bfloat16 if dtype == "bf16" else torch.float32
+    f32 = torch.float32
+    w = W.MoEWorkload("periln_fused", T=700, d=d, E=16, k=3, F=128, n_res=7, n_sh=n_sh, F_sh=64 if n_sh else 0, dtype=dtype, seed=21)
+    p = H.Problem(w)
+    rng = np.random.default_rng(5)
+    st = lambda a: W.bf16_round(a) if dtype == "bf16" else a.astype(np.float32)
+    dev = lambda a, dt=td: torch.from_numpy(np.ascontiguousarray(a)).cuda().to(dt)
+    x_in, dout = dev(st(rng.standard_normal((w.T, d)) * 1.3 + 0.1)), dev(st(rng.standard_normal((w.T, d))))
+    g1, b1, g2, b2 = (dev((rng.standard_normal(d) * 0.1 + o).astype(np.float32), f32) for o in (1.0, 0.0, 1.0, 0.0))
+    alpha = 0.7
+    layer = H.make_layer(p)
+    xn, s1 = torch.empty_like(x_in), torch.empty((w.T, 2), dtype=f32, device="cuda")
+    B.fomoe_periln_fwd(x_in, g1, b1, xn, s1)
+    layer.route(xn)
+    part = torch.empty(B.fomoe_periln_workspace_bytes(w.T, d), dtype=torch.uint8, device="cuda")
+    # ---- unfused ----
+    layer.forward(xn)
+    out_u, s2_u = torch.empty_like(x_in), torch.empty_like(s1)
+    B.fomoe_periln_fwd(layer.y, g2, b2, out_u, s2_u, residual=x_in, alpha=alpha)
+    y_u = layer.y.clone()
+    dy = torch.empty_like(x_in)
+    dg2, db2 = torch.empty(d, device="cuda"), torch.empty(d, device="cuda")
+    B.fomoe_periln_bwd(dout, layer.y, s2_u, g2, dy, dg2, db2, part, alpha=alpha)
+    layer.backward(dy, xn)
+    dx_u, dg1_u, db1_u = torch.empty_like(x_in), torch.empty(d, device="cuda"), torch.empty(d, device="cuda")
+    B.fomoe_periln_bwd(layer.dx, x_in, s1, g1, dx_u, dg1_u, db1_u, part, dresidual=dout)
+    dwu_u = layer.dw_up.clone()
+    torch.cuda.synchronize()
+    # ---- fused ----
+    layer.y.zero_()
+    out_f, s2_f = torch.empty_like(x_in), torch.empty_like(s1)
+    layer.forward_periln(xn, g2, b2, x_in, out_f, s2_f, alpha=alpha)
+    dg1_f, db1_f = torch.empty(d, device="cuda"), torch.empty(d, device="cuda")
+    layer.backward_periln(dy, xn, x_in, s1, g1, dout, dg1_f, db1_f, part)
+    torch.cuda.synchronize()
+    assert torch.equal(layer.y, y_u) and torch.equal(out_f, out_u) and torch.equal(s2_f, s2_u)
+    assert torch.equal(layer.dx, dx_u) and torch.equal(dg1_f, dg1_u) and torch.equal(db1_f, db1_u)
+    assert torch.equal(layer.dw_up, dwu_u)
+    assert torch.isfinite(out_f.float()).all() and torch.isfinite(layer.dx.float()).all()
+
+
+def test_fused_periln_unsupported_row_shape():
+    """A row that does not fit the register-resident shape is refused, not silently mis-computed."""
+    import torch
+    from paper_2606_19025_b200 import binding as B
+    w = W.MoEWorkload("periln_odd", T=64, d=36, E=8, k=2, F=32, n_res=4, dtype="bf16", seed=3)
+    p = H.Problem(w)
+    layer = H.make_layer(p)
+    x = layer.to_dev(p.x)
+    layer.route(x)
+    g = torch.ones(w.d, device="cuda")
+    out, st = torch.empty_like(x), torch.empty((w.T, 2), device="cuda")
+    with pytest.raises(B.FomoeError, match="UNSUPPORTED"):
+        layer.forward_periln(x, g, g, x, out, st)
