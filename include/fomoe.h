@@ -274,11 +274,20 @@ FOMOE_API int fomoe_outer_nesterov(float* const w_start[3], float* const w_now[3
                          int64_t elems_down, const int32_t* pack_slots, int32_t n_pack, float lr, float mu, void* stream);
 
 /*
- * One whole step from HOST buffers (the end-to-end path bench.py times): copies x_host (and dy_host) to the device,
+ * One whole step from HOST buffers (the end-to-end path bench.py times): copies x_host and dy_host to the device,
  * runs fomoe_route + fomoe_moe_fwd + fomoe_moe_bwd, copies y and dx back.  x_host, dy_host, y_host, dx_host:
  * HOST pointers, [T,d] cfg->dtype, ideally pinned.  x_dev, dy_dev, y_dev, dx_dev: device staging buffers [T,d].
- * copy_stream: a second stream used to overlap the dy upload and the y download with compute (may equal stream).
- * Everything else as in the three calls above.  Returns after enqueueing; the caller synchronises `stream`.
+ * Three engines work side by side: uploads on `copy_stream` (may equal `stream`), kernels on `stream`, downloads on a
+ * stream the library owns (per host thread and device).  Inside one call the dy upload overlaps route + forward and the y
+ * download overlaps the backward.  ACROSS calls, the library orders every use of a staging buffer after the previous call's
+ * use of the same ADDRESS (it keeps one event per address seen; it never dereferences or frees them): a caller that alternates
+ * two (x_dev, dy_dev) pairs gets the next step's uploads, this step's kernels and the previous step's dx download running
+ * at the same time -- the step is then bound by the slower of PCIe and compute instead of their sum.
+ * defer_join = 0: before returning, `stream` is made to wait for the downloads: y_host and dx_host are complete when
+ *                 `stream` completes (and consecutive calls do not overlap).
+ * defer_join = 1: downloads are left running; call fomoe_moe_step_host_join(stream) (or synchronise the device) before
+ *                 reading y_host / dx_host.
+ * Everything else as in the three calls above.  Returns after enqueueing.
  */
 FOMOE_API int fomoe_moe_step_host(const fomoe_config* cfg, const void* x_host, const void* dy_host, void* y_host, void* dx_host,
                         void* x_dev, void* dy_dev, void* y_dev, void* dx_dev,
@@ -288,7 +297,9 @@ FOMOE_API int fomoe_moe_step_host(const fomoe_config* cfg, const void* x_host, c
                         const void* sh_gate, const void* sh_up, const void* sh_down,
                         float* dw_router, void* dw_gate, void* dw_up, void* dw_down,
                         void* d_sh_gate, void* d_sh_up, void* d_sh_down,
-                        void* saved_acts, void* scratch, void* stream, void* copy_stream);
+                        void* saved_acts, void* scratch, void* stream, void* copy_stream, int32_t defer_join);
+/* Makes `stream` wait for every download this host thread's fomoe_moe_step_host calls have enqueued so far (current device). */
+FOMOE_API int fomoe_moe_step_host_join(void* stream);
 
 /*
  * DEBUG: validates the CONTENT of resident_ids ([n_res] int32, device): every id in [0,E), strictly ascending (so no

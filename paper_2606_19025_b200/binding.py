@@ -26,7 +26,7 @@ FOMOE_ROUTE_SKIP_TOKEN, FOMOE_ROUTE_FORCED_LOCAL = 0, 1
 
 EXPORTS = ("fomoe_workspace_bytes", "fomoe_route", "fomoe_moe_fwd", "fomoe_moe_bwd", "fomoe_pack_resident_deltas",
            "fomoe_adamw_resident", "fomoe_outer_nesterov", "fomoe_periln_workspace_bytes", "fomoe_periln_fwd", "fomoe_periln_bwd",
-           "fomoe_moe_step_host", "fomoe_last_launch_count", "fomoe_last_cuda_error", "fomoe_abi_version",
+           "fomoe_moe_step_host", "fomoe_moe_step_host_join", "fomoe_last_launch_count", "fomoe_last_cuda_error", "fomoe_abi_version",
            "fomoe_set_force_simt", "fomoe_profile_enable", "fomoe_profile_collect", "fomoe_debug_validate_resident",
            "fomoe_routing_stats", "fomoe_moe_fwd_periln", "fomoe_moe_bwd_periln")
 STAT_NAMES = ("kept_fraction", "ghost_fraction", "zero_kept_tokens", "load_cv", "routing_entropy", "max_load", "min_load")
@@ -265,7 +265,7 @@ def fomoe_outer_nesterov(w_start, w_now, momentum, w_compute, payload_avg, pack_
 
 def fomoe_moe_step_host(cfg, x_host, dy_host, y_host, dx_host, x_dev, dy_dev, y_dev, dx_dev, w_router, router_bias, resident_ids,
                         n_res, route: RouteState, w_gate, w_up, w_down, shared, dw_router, dw_gate, dw_up, dw_down, d_shared,
-                        saved_acts, scratch, stream=None, copy_stream=None) -> None:
+                        saved_acts, scratch, stream=None, copy_stream=None, defer_join=False) -> None:
     rs = route.c_struct()
     sg, su, sd = shared if shared is not None else (None, None, None)
     dsg, dsu, dsd = d_shared if d_shared is not None else (None, None, None)
@@ -273,7 +273,12 @@ def fomoe_moe_step_host(cfg, x_host, dy_host, y_host, dx_host, x_dev, dy_dev, y_
         C.byref(cfg), _p(x_host), _p(dy_host), _p(y_host), _p(dx_host), _p(x_dev), _p(dy_dev), _p(y_dev), _p(dx_dev), _p(w_router),
         _p(router_bias), _p(resident_ids), C.c_int32(n_res), C.byref(rs), _p(w_gate), _p(w_up), _p(w_down), _p(sg), _p(su), _p(sd),
         _p(dw_router), _p(dw_gate), _p(dw_up), _p(dw_down), _p(dsg), _p(dsu), _p(dsd), _p(saved_acts), _p(scratch),
-        _stream(stream), _stream(copy_stream if copy_stream is not None else stream)), "fomoe_moe_step_host")
+        _stream(stream), _stream(copy_stream if copy_stream is not None else stream), C.c_int32(1 if defer_join else 0)),
+        "fomoe_moe_step_host")
+
+
+def fomoe_moe_step_host_join(stream=None) -> None:
+    _check(lib().fomoe_moe_step_host_join(_stream(stream)), "fomoe_moe_step_host_join")
 
 
 def fomoe_debug_validate_resident(resident_ids, E: int, stream=None) -> None:

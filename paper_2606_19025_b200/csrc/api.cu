@@ -65,6 +65,37 @@ static SideStream* side_stream() {
   return &sd;
 }
 
+// State of fomoe_moe_step_host, per (host thread, device): a download stream (device -> host copies run on their own copy
+// engine, beside the uploads and the kernels) and one event per staging-buffer ADDRESS seen, which orders a call after the
+// previous call's use of the same buffer.  Addresses are only compared, never dereferenced.
+struct HostPipe {
+  cudaStream_t dl = nullptr;
+  cudaEvent_t joined = nullptr;
+  struct Slot { const void* p; cudaEvent_t ev; };
+  std::vector<Slot> slots;
+  cudaEvent_t event_of(const void* p) {
+    for (auto& sl : slots)
+      if (sl.p == p) return sl.ev;
+    if (slots.size() >= 64) {                     // a caller cycling through many buffers: forget the oldest (its event is long done)
+      cudaEventDestroy(slots.front().ev);
+      slots.erase(slots.begin());
+    }
+    cudaEvent_t e = nullptr;
+    if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+    slots.push_back({p, e});
+    return e;
+  }
+};
+static thread_local HostPipe g_pipe[kMaxDevices];
+static HostPipe* host_pipe() {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return nullptr;
+  HostPipe& hp = g_pipe[dev];
+  if (!hp.dl && cudaStreamCreateWithFlags(&hp.dl, cudaStreamNonBlocking) != cudaSuccess) return nullptr;
+  if (!hp.joined && cudaEventCreateWithFlags(&hp.joined, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+  return &hp;
+}
+
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 static int check_cfg(const fomoe_config* c, int n_res) {
@@ -394,32 +425,42 @@ int fomoe_moe_step_host(const fomoe_config* cfg, const void* x_host, const void*
                         const int32_t* resident_ids, int32_t n_res, const fomoe_route_state* route, const void* w_gate,
                         const void* w_up, const void* w_down, const void* sh_gate, const void* sh_up, const void* sh_down,
                         float* dw_router, void* dw_gate, void* dw_up, void* dw_down, void* d_sh_gate, void* d_sh_up, void* d_sh_down,
-                        void* saved_acts, void* scratch, void* stream, void* copy_stream) {
+                        void* saved_acts, void* scratch, void* stream, void* copy_stream, int32_t defer_join) {
   int rc = check_cfg(cfg, n_res);
   if (rc != FOMOE_OK) return rc;
   if (!x_host || !dy_host || !y_host || !dx_host || !x_dev || !dy_dev || !y_dev || !dx_dev) return FOMOE_ERR_BADARG;
   cudaStream_t st = (cudaStream_t)stream, cs = (cudaStream_t)copy_stream;
   const size_t bytes = (size_t)cfg->T * cfg->d_model * (cfg->dtype == FOMOE_BF16 ? 2 : 4);
+  HostPipe* hp = host_pipe();
+  if (!hp) return set_cuda_error(cudaErrorUnknown, "fomoe_moe_step_host: download stream");
+  cudaStream_t dl = hp->dl;
+  // last use of each staging buffer by an earlier call of this thread: uploads wait for the readers of x_dev / dy_dev, the
+  // kernels that overwrite y_dev / dx_dev wait for their previous download.  (Never-recorded events are no-ops to wait on.)
+  cudaEvent_t e_x = hp->event_of(x_dev), e_dy = hp->event_of(dy_dev), e_y = hp->event_of(y_dev), e_dx = hp->event_of(dx_dev);
+  if (!e_x || !e_dy || !e_y || !e_dx) return set_cuda_error(cudaErrorUnknown, "fomoe_moe_step_host: events");
   int launches = 0;
-  struct Events {   // destroyed on every exit path
-    cudaEvent_t start = nullptr, dy = nullptr, y = nullptr;
+  struct Events {   // destroyed on every exit path (destroying a pending event is deferred by the runtime)
+    cudaEvent_t xup = nullptr, dyup = nullptr, y = nullptr, dx = nullptr;
     ~Events() {
-      if (start) cudaEventDestroy(start);
-      if (dy) cudaEventDestroy(dy);
-      if (y) cudaEventDestroy(y);
+      for (cudaEvent_t e : {xup, dyup, y, dx})
+        if (e) cudaEventDestroy(e);
     }
   } ev;
-  FOMOE_CUDA_OK(cudaEventCreateWithFlags(&ev.start, cudaEventDisableTiming));
-  FOMOE_CUDA_OK(cudaEventCreateWithFlags(&ev.dy, cudaEventDisableTiming));
+  FOMOE_CUDA_OK(cudaEventCreateWithFlags(&ev.xup, cudaEventDisableTiming));
+  FOMOE_CUDA_OK(cudaEventCreateWithFlags(&ev.dyup, cudaEventDisableTiming));
   FOMOE_CUDA_OK(cudaEventCreateWithFlags(&ev.y, cudaEventDisableTiming));
-  // copy stream starts after everything already queued on the compute stream (previous step's consumers)
-  FOMOE_CUDA_OK(cudaEventRecord(ev.start, st));
-  FOMOE_CUDA_OK(cudaStreamWaitEvent(cs, ev.start, 0));
-  FOMOE_CUDA_OK(cudaMemcpyAsync(x_dev, x_host, bytes, cudaMemcpyHostToDevice, st));
-  FOMOE_CUDA_OK(cudaMemcpyAsync(dy_dev, dy_host, bytes, cudaMemcpyHostToDevice, cs));  // overlaps route + forward
-  FOMOE_CUDA_OK(cudaEventRecord(ev.dy, cs));
-  // whatever happens below, `st` waits for the copy stream before this call returns (no dangling fork)
+  FOMOE_CUDA_OK(cudaEventCreateWithFlags(&ev.dx, cudaEventDisableTiming));
+  // uploads (copy stream): x, then dy -- the second one overlaps route + forward; with alternating staging buffers both
+  // overlap the PREVIOUS call's compute
+  FOMOE_CUDA_OK(cudaStreamWaitEvent(cs, e_x, 0));
+  FOMOE_CUDA_OK(cudaMemcpyAsync(x_dev, x_host, bytes, cudaMemcpyHostToDevice, cs));
+  FOMOE_CUDA_OK(cudaEventRecord(ev.xup, cs));
+  FOMOE_CUDA_OK(cudaStreamWaitEvent(cs, e_dy, 0));
+  FOMOE_CUDA_OK(cudaMemcpyAsync(dy_dev, dy_host, bytes, cudaMemcpyHostToDevice, cs));
+  FOMOE_CUDA_OK(cudaEventRecord(ev.dyup, cs));
   auto body = [&]() -> int {
+    FOMOE_CUDA_OK(cudaStreamWaitEvent(st, ev.xup, 0));
+    FOMOE_CUDA_OK(cudaStreamWaitEvent(st, e_y, 0));
     int r = fomoe_route(cfg, x_dev, w_router, router_bias, resident_ids, n_res, route, st);
     launches += g_launches;
     if (r != FOMOE_OK) return r;
@@ -427,24 +468,41 @@ int fomoe_moe_step_host(const fomoe_config* cfg, const void* x_host, const void*
     launches += g_launches;
     if (r != FOMOE_OK) return r;
     FOMOE_CUDA_OK(cudaEventRecord(ev.y, st));
-    FOMOE_CUDA_OK(cudaStreamWaitEvent(cs, ev.y, 0));
-    FOMOE_CUDA_OK(cudaMemcpyAsync(y_host, y_dev, bytes, cudaMemcpyDeviceToHost, cs));  // overlaps backward
-    FOMOE_CUDA_OK(cudaStreamWaitEvent(st, ev.dy, 0));
+    FOMOE_CUDA_OK(cudaStreamWaitEvent(dl, ev.y, 0));
+    FOMOE_CUDA_OK(cudaMemcpyAsync(y_host, y_dev, bytes, cudaMemcpyDeviceToHost, dl));  // overlaps the backward
+    FOMOE_CUDA_OK(cudaEventRecord(e_y, dl));
+    FOMOE_CUDA_OK(cudaStreamWaitEvent(st, ev.dyup, 0));
+    FOMOE_CUDA_OK(cudaStreamWaitEvent(st, e_dx, 0));
     r = fomoe_moe_bwd(cfg, dy_dev, x_dev, route, n_res, w_router, w_gate, w_up, w_down, sh_gate, sh_up, sh_down, saved_acts, dx_dev,
                       dw_router, dw_gate, dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, scratch, st);
     launches += g_launches;
     if (r != FOMOE_OK) return r;
-    FOMOE_CUDA_OK(cudaMemcpyAsync(dx_host, dx_dev, bytes, cudaMemcpyDeviceToHost, st));
+    FOMOE_CUDA_OK(cudaEventRecord(e_x, st));    // x_dev and dy_dev have been read for the last time
+    FOMOE_CUDA_OK(cudaEventRecord(e_dy, st));
+    FOMOE_CUDA_OK(cudaEventRecord(ev.dx, st));
+    FOMOE_CUDA_OK(cudaStreamWaitEvent(dl, ev.dx, 0));
+    FOMOE_CUDA_OK(cudaMemcpyAsync(dx_host, dx_dev, bytes, cudaMemcpyDeviceToHost, dl));  // overlaps the NEXT call's compute
+    FOMOE_CUDA_OK(cudaEventRecord(e_dx, dl));
     return FOMOE_OK;
   };
   rc = body();
-  // join: the step is complete on `stream` only when the copy stream's work (dy upload, y download) is
-  cudaError_t e1 = cudaEventRecord(ev.y, cs);
-  cudaError_t e2 = cudaStreamWaitEvent(st, ev.y, 0);
-  if (rc == FOMOE_OK && e1 != cudaSuccess) rc = set_cuda_error(e1, "cudaEventRecord(copy join)");
-  if (rc == FOMOE_OK && e2 != cudaSuccess) rc = set_cuda_error(e2, "cudaStreamWaitEvent(copy join)");
+  // whatever happened, `st` is ordered after the uploads it may not have waited for yet (no dangling work on the copy stream)
+  cudaError_t e0 = cudaStreamWaitEvent(st, ev.dyup, 0);
+  if (rc == FOMOE_OK && e0 != cudaSuccess) rc = set_cuda_error(e0, "cudaStreamWaitEvent(copy join)");
+  if (!defer_join) {
+    int jr = fomoe_moe_step_host_join(stream);
+    if (rc == FOMOE_OK) rc = jr;
+  }
   g_launches = launches;
   return rc;
+}
+
+int fomoe_moe_step_host_join(void* stream) {
+  HostPipe* hp = host_pipe();
+  if (!hp) return set_cuda_error(cudaErrorUnknown, "fomoe_moe_step_host_join: download stream");
+  FOMOE_CUDA_OK(cudaEventRecord(hp->joined, hp->dl));
+  FOMOE_CUDA_OK(cudaStreamWaitEvent((cudaStream_t)stream, hp->joined, 0));
+  return FOMOE_OK;
 }
 
 }  // extern "C"

@@ -110,14 +110,19 @@ class SkipTokenMoE:
         self.launches = n
         return g.replay
 
-    def step_host(self, x_host, dy_host, y_host, dx_host, x_dev, dy_dev, stream=None, copy_stream=None) -> int:
-        """Whole step from pinned HOST buffers through fomoe_moe_step_host (uploads x, dy; downloads y, dx)."""
+    def step_host(self, x_host, dy_host, y_host, dx_host, x_dev, dy_dev, stream=None, copy_stream=None, defer_join=False) -> int:
+        """Whole step from pinned HOST buffers through fomoe_moe_step_host (uploads x, dy; downloads y, dx).  defer_join=True
+        leaves the downloads running (call host_join() before reading y_host / dx_host): with alternating (x_dev, dy_dev) pairs
+        consecutive steps then overlap their PCIe copies with each other's compute."""
         B.fomoe_moe_step_host(self.cfg, x_host, dy_host, y_host, dx_host, x_dev, dy_dev, self.y, self.dx, self.w_router,
                               self.router_bias, self.resident, self.n_res, self.route_state, self.w_gate, self.w_up, self.w_down,
                               self.shared, self.dw_router, self.dw_gate, self.dw_up, self.dw_down, self.d_shared, self.saved_acts,
-                              self.scratch, stream, copy_stream)
+                              self.scratch, stream, copy_stream, defer_join)
         self.launches = B.fomoe_last_launch_count()
         return self.launches
+
+    def host_join(self, stream=None) -> None:
+        B.fomoe_moe_step_host_join(stream)
 
     def routing_numpy(self) -> dict:
         """Device -> host copy of the public routing outputs (tests / diagnostics only)."""

@@ -250,9 +250,11 @@ def test_debug_validate_resident():
             B.fomoe_debug_validate_resident(bad, 8)
 
 
-def test_step_host_matches_oracle_twice_in_a_row(oracle64):
-    """The end-to-end entry point bench.py times (fomoe_moe_step_host: uploads on two streams overlapping compute) against
-    the oracle, called twice back to back with different inputs and a separate copy stream (overlap logic)."""
+@pytest.mark.parametrize("pipelined", [False, True])
+def test_step_host_matches_oracle_twice_in_a_row(oracle64, pipelined):
+    """The end-to-end entry point bench.py times (fomoe_moe_step_host: uploads, kernels and downloads on three streams) against
+    the oracle, called back to back with different inputs and no synchronisation in between.  pipelined: alternating staging
+    buffers and deferred join (the form bench.py times: consecutive steps overlap), four calls, then ONE join + stream sync."""
     import torch
     w = W.MoEWorkload("e2e", T=2048, d=256, E=16, k=2, F=256, n_res=8, n_sh=1, F_sh=128, dtype="bf16", seed=15)
     p = H.Problem(w)
@@ -265,9 +267,19 @@ def test_step_host_matches_oracle_twice_in_a_row(oracle64):
     x2, dy2 = pin(p.x[::-1].copy()), pin((0.5 * p.dy[::-1]).astype(np.float32))   # token-reversed, scaled: also margin-clean
     outs = [(torch.empty_like(x1).pin_memory(), torch.empty_like(x1).pin_memory()) for _ in range(2)]
     xd, dyd = torch.empty((w.T, w.d), dtype=td, device="cuda"), torch.empty((w.T, w.d), dtype=td, device="cuda")
-    for (xh, dyh), (yh, dxh) in zip(((x1, dy1), (x2, dy2)), outs):
-        layer.step_host(xh, dyh, yh, dxh, xd, dyd, copy_stream=cs)     # no sync in between: the second call must order itself
-    torch.cuda.synchronize()
+    if pipelined:
+        stage = [(xd, dyd), (torch.empty_like(xd), torch.empty_like(dyd))]
+        scratch_out = (torch.empty_like(x1).pin_memory(), torch.empty_like(x1).pin_memory())
+        seq = [((x2, dy2), scratch_out), ((x1, dy1), outs[0]), ((x2, dy2), outs[1])]     # first call: results overwritten later
+        seq.insert(1, ((x1, dy1), scratch_out))
+        for i, ((xh, dyh), (yh, dxh)) in enumerate(seq):
+            layer.step_host(xh, dyh, yh, dxh, *stage[i % 2], copy_stream=cs, defer_join=True)
+        layer.host_join()
+        torch.cuda.current_stream().synchronize()      # the join made the compute stream wait for the downloads
+    else:
+        for (xh, dyh), (yh, dxh) in zip(((x1, dy1), (x2, dy2)), outs):
+            layer.step_host(xh, dyh, yh, dxh, xd, dyd, copy_stream=cs)     # no sync in between: the second call must order itself
+        torch.cuda.current_stream().synchronize()      # defer_join = 0: results are complete when the stream is
     for i, ((xh, dyh), (yh, dxh)) in enumerate(zip(((x1, dy1), (x2, dy2)), outs)):
         q = H.Problem(w)
         q.x, q.dy = xh.float().numpy(), dyh.float().numpy()
