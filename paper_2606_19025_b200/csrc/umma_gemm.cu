@@ -26,6 +26,7 @@
 // Row space is either the tile-padded routed rows (pairs of 128-row tiles of ONE slot; the last pair of a slot may hold a
 // single tile, then CTA 1 computes rows nobody stores) or dense rows (shared experts).
 #include <cuda.h>
+#include <stdlib.h>
 
 #include "common.cuh"
 #include "umma_ptx.cuh"
@@ -47,7 +48,7 @@ enum Mode { FWD1 = 0, FWD2 = 1, DH = 2, DX = 3, WGRAD = 4, ROUTE = 5, FWD1S = 6 
 constexpr int kRouteStg = 57344;  // ROUTE epilogue scratch: slot map, per-stage histograms, top-k candidate / merge lists (k <= 32)
 // DH and FWD1 trade TMA stages for epilogue staging: DH streams a and u back in through a cp.async ring
 __host__ __device__ constexpr int stages_of(int mode) { return mode == DH ? 4 : (mode == FWD1 || mode == FWD1S || mode == ROUTE) ? 5 : 6; }
-__host__ __device__ constexpr int stg_tiles_per_warp(int mode) { return mode == DH ? 2 * kDhDepth : mode == FWD1 ? 3 : mode == FWD1S ? 2 : 1; }
+__host__ __device__ constexpr int stg_tiles_per_warp(int mode) { return mode == DH ? 2 * kDhDepth : mode == FWD1 ? 3 : 2; }   // FWD2 / DX: two tiles, alternating under the bulk stores
 __host__ __device__ constexpr int stg_bytes_of(int mode) { return mode == ROUTE ? kRouteStg : kEpiWarps * stg_tiles_per_warp(mode) * kStgTile; }
 __host__ __device__ constexpr int smem_bytes_of(int mode) {
   return stages_of(mode) * kStageBytes + stg_bytes_of(mode) + 1024 /*align*/ + 256 /*barriers*/;
@@ -55,7 +56,7 @@ __host__ __device__ constexpr int smem_bytes_of(int mode) {
 constexpr int kTmemCols = 512;
 
 struct TmaMaps {
-  CUtensorMap m[6];   // WGRAD with several jobs: (A, B) of job j at m[2j], m[2j+1]
+  CUtensorMap m[6];   // WGRAD with several jobs: (A, B) of job j at m[2j], m[2j+1].  FWD2 / DX: m[4] = the output, for the bulk-store epilogue
 };
 
 // ROUTE mode (rows F1-F4 + the per-block histogram of F5): everything the router epilogue needs
@@ -85,6 +86,7 @@ struct UmmaParams {
   int a_gcol, b_gcol;          // WGRAD dense: per-group column offset into A / B
   int ksegs;                   // DX: K segments (2: dA W_gate + dU W_up; 1: dA W_up, two-matrix expert)
   int k_chunk;                 // WGRAD dense: > 0 = split-K, group g reduces rows [g*k_chunk, (g+1)*k_chunk)
+  int tma_store;               // FWD2 / DX: the epilogue stores its 32 x 32 chunks with TMA bulk stores through maps.m[4]
   float* out_f32;              // WGRAD: if set, fp32 output [n_groups, M, N] instead of out0
   // WGRAD dense, tail split: the tiles of the last, partially filled round of the persistent schedule (tile ids >= tail_first)
   // are cut into tail_ks K ranges of tail_chunk rows each, so that round takes 1 / tail_ks of a tile time; the pieces go to
@@ -138,6 +140,19 @@ __device__ __forceinline__ void stg_put_row(uint32_t stg, int lane, const float 
     w.z = pack_bf16x2(v[q * 8 + 4], v[q * 8 + 5]);
     w.w = pack_bf16x2(v[q * 8 + 6], v[q * 8 + 7]);
     sts128(stg + stg_off(lane, q), w);
+  }
+}
+// lane = row: 32 fp32 as bf16 into a 32 x 64 B tile in the TMA SWIZZLE_64B image (16-byte piece q of row r at
+// r * 64 + ((q ^ ((r >> 1) & 3)) << 4)): what a bulk tensor store with a {32 columns, 32 rows} box reads; conflict-free
+__device__ __forceinline__ void stg_put_row_sw64(uint32_t stg, int lane, const float (&v)[32]) {
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    uint4 w;
+    w.x = pack_bf16x2(v[q * 8 + 0], v[q * 8 + 1]);
+    w.y = pack_bf16x2(v[q * 8 + 2], v[q * 8 + 3]);
+    w.z = pack_bf16x2(v[q * 8 + 4], v[q * 8 + 5]);
+    w.w = pack_bf16x2(v[q * 8 + 6], v[q * 8 + 7]);
+    sts128(stg + lane * 64 + ((q ^ ((lane >> 1) & 3)) << 4), w);
   }
 }
 // whole warp: staging tile -> global rows [0, rows_valid) x 32 columns at g (row stride ld elements); 4 lanes per row
@@ -753,6 +768,8 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
 #pragma unroll
     for (int i = 0; i < 4; ++i) prefetch_tmap(&maps.m[i]);
     if (MODE == WGRAD && p.n_jobs > 2) { prefetch_tmap(&maps.m[4]); prefetch_tmap(&maps.m[5]); }   // (zero-filled otherwise)
+    if ((MODE == FWD2 || MODE == DX) && p.tma_store) prefetch_tmap(&maps.m[4]);
+    if ((MODE == FWD1 || MODE == FWD1S) && p.tma_store) { prefetch_tmap(&maps.m[3]); prefetch_tmap(&maps.m[5]); if (MODE == FWD1) prefetch_tmap(&maps.m[4]); }
   }
   if (warp == 1 && lane == 0) {
     for (int i = 0; i < kStages; ++i) { mbar_init(smem_u32(&full_bar[i]), 1); mbar_init(smem_u32(&empty_bar[i]), 1); }
@@ -998,6 +1015,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
       cp_async_wait<0>();
     } else {
     const uint32_t stg1 = stg0 + kStgTile, stg2 = stg1 + kStgTile;  // FWD1 only
+    int st_buf = 0;                                                   // FWD2 / DX bulk stores: staging tile in turn
     int as = 0;
     uint32_t aphase = 0;
     for (long id = cluster_id; id < sched.total; id += n_clusters) {
@@ -1063,6 +1081,23 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
               u[i] = sa;
               sa_h[i] = h;
             }
+            if (p.tma_store) {   // three bulk tensor stores per chunk (maps m[3..5] = the outputs); the previous chunk's have been
+              if (lane == 0) bulk_wait_read<0>();   // reading the tiles while this chunk's sigmoids were computed
+              __syncwarp();
+              stg_put_row_sw64(stg0, lane, a);
+              stg_put_row_sw64(stg1, lane, u);
+              stg_put_row_sw64(stg2, lane, sa_h);
+              asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+              __syncwarp();
+              if (lane == 0) {
+                const int c0 = t.part * p.F + n;
+                tma_store_2d(&maps.m[3], stg0, c0, row0);
+                tma_store_2d(&maps.m[4], stg1, c0, row0);
+                tma_store_2d(&maps.m[5], stg2, c0, row0);
+                bulk_commit();
+              }
+              continue;
+            }
             stg_put_row(stg0, lane, a);
             stg_put_row(stg1, lane, u);
             stg_put_row(stg2, lane, sa_h);
@@ -1087,12 +1122,44 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
               h[i] = a[i] * sg;                          // silu(a)
               a[i] = fmaf(h[i], 1.0f - sg, sg);           // silu'(a) = s (1 + a (1 - s))
             }
+            if (p.tma_store) {   // (maps m[3], m[5] = out0, out2)
+              if (lane == 0) bulk_wait_read<0>();
+              __syncwarp();
+              stg_put_row_sw64(stg0, lane, a);
+              stg_put_row_sw64(stg1, lane, h);
+              asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+              __syncwarp();
+              if (lane == 0) {
+                const int c0 = t.part * p.F + n;
+                tma_store_2d(&maps.m[3], stg0, c0, row0);
+                tma_store_2d(&maps.m[5], stg1, c0, row0);
+                bulk_commit();
+              }
+              continue;
+            }
             stg_put_row(stg0, lane, a);
             stg_put_row(stg1, lane, h);
             __syncwarp();
             stg_to_global(stg0, p.out0 + base + n, p.ld, lane, rows_valid);
             stg_to_global(stg1, p.out2 + base + n, p.ld, lane, rows_valid);
             __syncwarp();
+          }
+        } else if (p.tma_store) {  // FWD2, DX: [rows, d] tile, one bulk tensor store per 32 x 32 chunk (rows beyond the tensor are clipped)
+#pragma unroll 1
+          for (int cc = half; cc < BN / 32 && rows_valid > 0; cc += 2) {
+            const int n = t.n_tile * BN + cc * 32;
+            if (n >= p.d) break;
+            float v[32];
+            tmem_ld32(taddr + cc * 32, v);
+            tmem_ld_wait();
+            const uint32_t stg = stg0 + st_buf * kStgTile;
+            if (lane == 0) bulk_wait_read<1>();       // the store that last read this tile (two chunks ago) has its data
+            __syncwarp();
+            stg_put_row_sw64(stg, lane, v);
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> the bulk store's async-proxy reads
+            __syncwarp();
+            if (lane == 0) { tma_store_2d(&maps.m[4], stg, n, row0); bulk_commit(); }
+            st_buf ^= 1;
           }
         } else {  // FWD2, DX: plain store of a [rows, d] tile
 #pragma unroll 1
@@ -1116,6 +1183,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
         if (++as == kAccStages) { as = 0; aphase ^= 1; }
       }
     }
+    if ((MODE == FWD2 || MODE == DX || MODE == FWD1 || MODE == FWD1S) && p.tma_store && lane == 0) bulk_wait_all();   // shared memory stays valid until the stores have read it
     }
   }
 
@@ -1170,6 +1238,31 @@ int launch(const TmaMaps& maps, const UmmaParams& p, cudaStream_t st, const char
 
 }  // namespace
 
+// FWD2 / DX output through TMA bulk stores: m[4] = [rows, d] with a {32 columns, 32 rows} box, 64-byte swizzle.  FOMOE_TMA_STORE=0
+// in the environment keeps the st.global epilogue (A/B measurements).
+static bool tma_store_enabled() {
+  static const bool on = [] { const char* e = getenv("FOMOE_TMA_STORE"); return !(e && e[0] == '0'); }();
+  return on;
+}
+static bool set_store_map(TmaMaps& m, UmmaParams& q, const void* out, uint64_t rows, int d) {
+  q.tma_store = 0;
+  if (!tma_store_enabled()) return true;
+  if (!make_map_box(&m.m[4], out, (uint64_t)d, rows, (uint64_t)d, 32, 32, CU_TENSOR_MAP_SWIZZLE_64B)) return false;
+  q.tma_store = 1;
+  return true;
+}
+
+// FWD1 / FWD1S: m[3], m[4], m[5] = out0, out1, out2 ([rows, ld]); a NULL output is skipped
+static bool set_store_maps3(TmaMaps& m, UmmaParams& q, uint64_t rows, int ld) {
+  q.tma_store = 0;
+  if (!tma_store_enabled()) return true;
+  const void* outs[3] = {q.out0, q.out1, q.out2};
+  for (int i = 0; i < 3; ++i)
+    if (outs[i] && !make_map_box(&m.m[3 + i], outs[i], (uint64_t)ld, rows, (uint64_t)ld, 32, 32, CU_TENSOR_MAP_SWIZZLE_64B)) return false;
+  q.tma_store = 1;
+  return true;
+}
+
 bool umma_supported(const fomoe_config& c) {
   if (c.dtype != FOMOE_BF16) return false;
   if (c.d_model % 64 || c.d_ff % 64) return false;
@@ -1211,6 +1304,7 @@ int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs&
       m.m[2] = m.m[3] = m.m[0];
       UmmaParams q = p;
       q.out0 = (bf16*)aws.a; q.out2 = (bf16*)aws.h;
+      MAP_OK(set_store_maps3(m, q, R, F));
       int rc = launch<FWD1S>(m, q, st, "umma_grouped_kernel<FWD1S>");
       if (rc != FOMOE_OK) return rc;
     } else {
@@ -1221,6 +1315,7 @@ int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs&
       m.m[3] = m.m[0];
       UmmaParams q = p;
       q.out0 = (bf16*)aws.a; q.out1 = (bf16*)aws.u; q.out2 = (bf16*)aws.h;
+      MAP_OK(set_store_maps3(m, q, R, F));
       int rc = launch<FWD1>(m, q, st, "umma_grouped_kernel<FWD1>");
       if (rc != FOMOE_OK) return rc;
     }
@@ -1231,6 +1326,7 @@ int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs&
       m.m[2] = m.m[3] = m.m[0];
       UmmaParams q = p;
       q.out0 = (bf16*)aws.o;
+      MAP_OK(set_store_map(m, q, aws.o, R, d));
       int rc = launch<FWD2>(m, q, st, "umma_grouped_kernel<FWD2>");
       if (rc != FOMOE_OK) return rc;
     }
@@ -1246,6 +1342,7 @@ int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs&
       m.m[2] = m.m[3] = m.m[0];
       UmmaParams q = p;
       q.out0 = (bf16*)aws.sa; q.out2 = (bf16*)aws.sh;
+      MAP_OK(set_store_maps3(m, q, c.T, ld));
       int rc = launch<FWD1S>(m, q, st, "umma_grouped_kernel<FWD1S,shared>");
       if (rc != FOMOE_OK) return rc;
     } else {
@@ -1256,6 +1353,7 @@ int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs&
       m.m[3] = m.m[0];
       UmmaParams q = p;
       q.out0 = (bf16*)aws.sa; q.out1 = (bf16*)aws.su; q.out2 = (bf16*)aws.sh;
+      MAP_OK(set_store_maps3(m, q, c.T, ld));
       int rc = launch<FWD1>(m, q, st, "umma_grouped_kernel<FWD1,shared>");
       if (rc != FOMOE_OK) return rc;
     }
@@ -1266,6 +1364,7 @@ int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs&
       m.m[2] = m.m[3] = m.m[0];
       UmmaParams q = p;
       q.out0 = (bf16*)sws.y_sh;
+      MAP_OK(set_store_map(m, q, sws.y_sh, c.T, d));
       int rc = launch<FWD2>(m, q, st, "umma_grouped_kernel<FWD2,shared>");
       if (rc != FOMOE_OK) return rc;
     }
@@ -1302,6 +1401,7 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
         UmmaParams q = p;
         q.ksegs = silu ? 1 : 2;
         q.out0 = (bf16*)sws.dxp;
+        MAP_OK(set_store_map(m, q, sws.dxp, R, d));
         int rc = launch<DX>(m, q, st, "umma_grouped_kernel<DX>");
         if (rc != FOMOE_OK) return rc;
       }
@@ -1355,6 +1455,7 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
         UmmaParams q = p;
         q.ksegs = silu ? 1 : 2;
         q.out0 = (bf16*)sws.dx_sh;
+        MAP_OK(set_store_map(m, q, sws.dx_sh, c.T, d));
         int rc = launch<DX>(m, q, st, "umma_grouped_kernel<DX,shared>");
         if (rc != FOMOE_OK) return rc;
       }
@@ -1453,6 +1554,7 @@ int umma_router_bwd(const fomoe_config& c, const void* x, const float* w_router,
     MAP_OK(make_map(&m.m[1], wr_bf, Ez, d, Ez, 128));
     m.m[2] = m.m[3] = m.m[0];
     p.out0 = (bf16*)sws.dx_r;
+    MAP_OK(set_store_map(m, p, sws.dx_r, T, d));
     int rc = launch<FWD2>(m, p, st, "umma_grouped_kernel<FWD2,router dx>");
     if (rc != FOMOE_OK) return rc;
   }
