@@ -25,7 +25,14 @@
  *     fallback: a shape the kernels do not cover returns FOMOE_ERR_UNSUPPORTED.
  *   - dtype: FOMOE_BF16 runs the expert GEMMs on tcgen05 tensor cores (bf16 in, fp32 accumulate in TMEM)
  *     when d_model % 64 == 0 and d_ff % 64 == 0 (otherwise, and for FOMOE_F32, fp32 SIMT kernels).
- *     The router always accumulates in fp32 with fp32 W_r (BASELINE.json config 2 "fp32 router").
+ *     Router precision (BASELINE.json config 2 "fp32 router"): logits accumulate in fp32.  The fp32 kernels multiply in fp32.
+ *     The bf16 tensor-core router (bf16 x, d_model % 64 == 0, E <= 128) multiplies the bf16-exact x with W_r SPLIT into bf16
+ *     pieces (hi + mid + lo, each the bf16 rounding of the running residual): 3 pieces = 24 mantissa bits of W_r for E <= 80,
+ *     2 pieces = 16 bits for 80 < E <= 128; every product is exact in fp32, the sums are fp32.  Logit error against the fp32
+ *     definition: <= ~2e-6 (3 pieces) / <= ~1.6e-5 (2 pieces, d = 4096, |x| ~ 1, |W_r| ~ 0.02): below the 1e-4 margin at which
+ *     routing indices are specified to be bit-exact.  The router BACKWARD of the bf16 path runs on bf16 operands (dz, W_r and x
+ *     rounded to bf16, fp32 accumulation): dw_router and the router's share of dx carry bf16-level relative error (~4e-3), like
+ *     every other gradient of that path.
  */
 #ifndef FOMOE_H_
 #define FOMOE_H_

@@ -6,11 +6,13 @@
 // The row is staged once in shared memory (fp32), so mean and the centred variance are computed exactly as LayerNorm
 // defines them and global memory is read once.  Bound: HBM.
 #include "common.cuh"
+#include <stdlib.h>
 
 namespace fomoe {
 namespace {
 
 constexpr int kLnThreads = 256;
+
 
 __device__ __forceinline__ float block_sum(float v, float* red) {
 #pragma unroll
@@ -23,6 +25,20 @@ __device__ __forceinline__ float block_sum(float v, float* red) {
 #pragma unroll
   for (int i = 0; i < (int)(blockDim.x >> 5); ++i) s += red[i];   // same order in every thread
   return s;
+}
+
+// two independent sums through the same tree as block_sum (so each equals what block_sum would return), one barrier pair
+__device__ __forceinline__ void block_sum2(float& a, float& b, float* red) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, o); b += __shfl_xor_sync(0xffffffffu, b, o); }
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = (int)(blockDim.x >> 5);
+  __syncthreads();
+  if (l == 0) { red[w] = a; red[nw + w] = b; }
+  __syncthreads();
+  float sa = 0.f, sb = 0.f;
+#pragma unroll
+  for (int i = 0; i < nw; ++i) { sa += red[i]; sb += red[nw + i]; }
+  a = sa; b = sb;
 }
 
 // The element formulas, with every rounding spelled out (no compiler-chosen FMA contraction): the stand-alone kernels and the
@@ -54,6 +70,17 @@ template <> __device__ __forceinline__ void ldv<float>(const float* p, float (&v
 }
 template <> __device__ __forceinline__ void ldv<__nv_bfloat16>(const __nv_bfloat16* p, float (&v)[8]) {
   const uint4 r = *reinterpret_cast<const uint4*>(p);
+  const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&r);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { const float2 f = __bfloat1622float2(h[i]); v[2 * i] = f.x; v[2 * i + 1] = f.y; }
+}
+// a 16-byte vector kept as loaded (bf16: 8 values in 4 registers) and widened when used: the register count decides how many
+// rows an SM keeps in flight
+template <typename T> __device__ __forceinline__ void unpack(const uint4& r, float (&v)[VecN<T>::n]);
+template <> __device__ __forceinline__ void unpack<float>(const uint4& r, float (&v)[4]) {
+  v[0] = __uint_as_float(r.x); v[1] = __uint_as_float(r.y); v[2] = __uint_as_float(r.z); v[3] = __uint_as_float(r.w);
+}
+template <> __device__ __forceinline__ void unpack<__nv_bfloat16>(const uint4& r, float (&v)[8]) {
   const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&r);
 #pragma unroll
   for (int i = 0; i < 4; ++i) { const float2 f = __bfloat1622float2(h[i]); v[2 * i] = f.x; v[2 * i + 1] = f.y; }
@@ -181,8 +208,10 @@ template <typename T, int VN> __device__ __forceinline__ void ld_param(const flo
   if constexpr (VN == 8) ldv<float>(p + 4, *reinterpret_cast<float(*)[4]>(&v[4]));
 }
 
-template <typename T, int NV>
-__global__ void __launch_bounds__(kLnThreads, 4)
+// The row is held as loaded (bf16: 8 values in 4 registers) and widened each time it is used: with <= 40 registers per thread
+// six CTAs are resident per SM, and the number of rows in flight per SM is what bounds this kernel.
+template <typename T, int NV, bool RES>   // RES: a residual row is read and added (post-LN); without it two more CTAs fit per SM
+__global__ void __launch_bounds__(kLnThreads, NV <= 2 ? (RES ? 5 : 6) : 2)
 periln_fwd_reg_kernel(const T* __restrict__ x, const float* __restrict__ gamma, const float* __restrict__ beta, const T* __restrict__ residual,
                       float alpha, float eps, int T_, int d, T* __restrict__ out, float* __restrict__ stats) {
   constexpr int VN = VecN<T>::n;
@@ -191,22 +220,26 @@ periln_fwd_reg_kernel(const T* __restrict__ x, const float* __restrict__ gamma, 
   pdl_wait();
   for (int t = blockIdx.x; t < T_; t += gridDim.x) {
     const size_t base = (size_t)t * d;
-    float v[NV][VN], r[NV][VN];
+    uint4 xr[NV], rr[NV];
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
+      xr[j] = make_uint4(0u, 0u, 0u, 0u);
+      rr[j] = make_uint4(0u, 0u, 0u, 0u);
+      if (c < d) {
+        xr[j] = *reinterpret_cast<const uint4*>(x + base + c);
+        if (RES) rr[j] = *reinterpret_cast<const uint4*>(residual + base + c);
+      }
+    }
     float s = 0.f;
 #pragma unroll
     for (int j = 0; j < NV; ++j) {
       const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
       if (c < d) {
-        ldv<T>(x + base + c, v[j]);
-        if (residual) ldv<T>(residual + base + c, r[j]);
-      }
-    }
+        float v[VN];
+        unpack<T>(xr[j], v);
 #pragma unroll
-    for (int j = 0; j < NV; ++j) {
-      const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
-      if (c < d) {
-#pragma unroll
-        for (int i = 0; i < VN; ++i) s += v[j][i];
+        for (int i = 0; i < VN; ++i) s += v[i];
       }
     }
     const float mean = block_sum(s, red) / (float)d;
@@ -215,8 +248,10 @@ periln_fwd_reg_kernel(const T* __restrict__ x, const float* __restrict__ gamma, 
     for (int j = 0; j < NV; ++j) {
       const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
       if (c < d) {
+        float v[VN];
+        unpack<T>(xr[j], v);
 #pragma unroll
-        for (int i = 0; i < VN; ++i) { v[j][i] -= mean; q += v[j][i] * v[j][i]; }
+        for (int i = 0; i < VN; ++i) { v[i] -= mean; q += v[i] * v[i]; }
       }
     }
     const float rstd = rsqrtf(block_sum(q, red) / (float)d + eps);
@@ -225,67 +260,100 @@ periln_fwd_reg_kernel(const T* __restrict__ x, const float* __restrict__ gamma, 
     for (int j = 0; j < NV; ++j) {
       const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
       if (c < d) {
-        float g[VN], b[VN];
+        float g[VN], b[VN], v[VN], r[VN];
         ld_param<T, VN>(gamma + c, g);
         ld_param<T, VN>(beta + c, b);
+        unpack<T>(xr[j], v);
+        unpack<T>(rr[j], r);
 #pragma unroll
-        for (int i = 0; i < VN; ++i) v[j][i] = ln_out(v[j][i], rstd, g[i], b[i], alpha, residual != nullptr, residual ? r[j][i] : 0.f);
-        stv<T>(out + base + c, v[j]);
+        for (int i = 0; i < VN; ++i) v[i] = ln_out(v[i] - mean, rstd, g[i], b[i], alpha, RES, r[i]);
+        stv<T>(out + base + c, v);
       }
     }
   }
 }
 
+// Rows held as loaded (see periln_fwd_reg_kernel).  The dgamma / dbeta accumulators live in shared memory when the row is at
+// most two vectors per thread (each thread reads and writes only its own columns: no conflicts, no atomics, fixed token
+// order), which brings the kernel from 80-127 registers to <= 64 and from 2-3 resident CTAs per SM to 4.
 template <typename T, int NV>
-__global__ void __launch_bounds__(kLnThreads)
+__global__ void __launch_bounds__(kLnThreads, NV <= 2 ? 4 : 1)
 periln_bwd_reg_kernel(const T* __restrict__ dout, const T* __restrict__ x, const float* __restrict__ stats, const float* __restrict__ gamma,
                       float alpha, const T* __restrict__ dresidual, int T_, int d, T* __restrict__ dx, float* __restrict__ partials) {
   constexpr int VN = VecN<T>::n;
-  __shared__ float red[kLnThreads / 32];
+  constexpr bool kSmemAcc = NV <= 2;
+  extern __shared__ float acc_sm[];          // kSmemAcc: [2][d] dgamma | dbeta accumulators of this CTA
+  __shared__ float red[2 * (kLnThreads / 32)];
   pdl_launch_dependents();
   pdl_wait();
-  float g[NV][VN], ag[NV][VN], ab[NV][VN];
+  float ag[kSmemAcc ? 1 : NV][VN], ab[kSmemAcc ? 1 : NV][VN];
 #pragma unroll
   for (int j = 0; j < NV; ++j) {
     const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
 #pragma unroll
-    for (int i = 0; i < VN; ++i) { g[j][i] = c < d ? gamma[c + i] : 0.f; ag[j][i] = 0.f; ab[j][i] = 0.f; }
+    for (int i = 0; i < VN; ++i) {
+      if (kSmemAcc) { if (c < d) { acc_sm[c + i] = 0.f; acc_sm[d + c + i] = 0.f; } }
+      else { ag[j][i] = 0.f; ab[j][i] = 0.f; }
+    }
   }
   for (int t = blockIdx.x; t < T_; t += gridDim.x) {
     const size_t base = (size_t)t * d;
     const float mean = stats[2 * (size_t)t], rstd = stats[2 * (size_t)t + 1];
-    float dh[NV][VN], h[NV][VN], r[NV][VN];
+    uint4 gr[NV], xr[NV], rr[NV];
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
+      gr[j] = xr[j] = rr[j] = make_uint4(0u, 0u, 0u, 0u);
+      if (c < d) {
+        gr[j] = *reinterpret_cast<const uint4*>(dout + base + c);
+        xr[j] = *reinterpret_cast<const uint4*>(x + base + c);
+        if (dresidual) rr[j] = *reinterpret_cast<const uint4*>(dresidual + base + c);
+      }
+    }
     float s1 = 0.f, s2 = 0.f;
 #pragma unroll
     for (int j = 0; j < NV; ++j) {
       const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
       if (c < d) {
-        ldv<T>(dout + base + c, dh[j]);
-        ldv<T>(x + base + c, h[j]);
-        if (dresidual) ldv<T>(dresidual + base + c, r[j]);
-      }
-    }
-#pragma unroll
-    for (int j = 0; j < NV; ++j) {
-      const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
-      if (c < d) {
+        float g[VN], go[VN], h[VN], a_g[VN], a_b[VN];
+        ld_param<T, VN>(gamma + c, g);
+        unpack<T>(gr[j], go);
+        unpack<T>(xr[j], h);
+        if (kSmemAcc) { ld_param<T, VN>(acc_sm + c, a_g); ld_param<T, VN>(acc_sm + d + c, a_b); }
 #pragma unroll
         for (int i = 0; i < VN; ++i) {
-          const float go = __fmul_rn(alpha, dh[j][i]);
-          h[j][i] = __fmul_rn(h[j][i] - mean, rstd);
-          dh[j][i] = ln_bwd_acc(go, h[j][i], g[j][i], ag[j][i], ab[j][i], s1, s2);   // fixed token order per CTA
+          const float gi = __fmul_rn(alpha, go[i]);
+          const float hi = __fmul_rn(h[i] - mean, rstd);
+          if (kSmemAcc) ln_bwd_acc(gi, hi, g[i], a_g[i], a_b[i], s1, s2);   // fixed token order per CTA
+          else ln_bwd_acc(gi, hi, g[i], ag[j][i], ab[j][i], s1, s2);
+        }
+        if (kSmemAcc) {
+#pragma unroll
+          for (int v4 = 0; v4 < VN / 4; ++v4) {
+            *reinterpret_cast<float4*>(acc_sm + c + 4 * v4) = make_float4(a_g[4 * v4], a_g[4 * v4 + 1], a_g[4 * v4 + 2], a_g[4 * v4 + 3]);
+            *reinterpret_cast<float4*>(acc_sm + d + c + 4 * v4) = make_float4(a_b[4 * v4], a_b[4 * v4 + 1], a_b[4 * v4 + 2], a_b[4 * v4 + 3]);
+          }
         }
       }
     }
-    const float m1 = block_sum(s1, red) / (float)d;
-    const float m2 = block_sum(s2, red) / (float)d;
+    block_sum2(s1, s2, red);
+    const float m1 = s1 / (float)d, m2 = s2 / (float)d;
 #pragma unroll
     for (int j = 0; j < NV; ++j) {
       const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
       if (c < d) {
+        float g[VN], go[VN], h[VN], r[VN];
+        ld_param<T, VN>(gamma + c, g);
+        unpack<T>(gr[j], go);
+        unpack<T>(xr[j], h);
+        unpack<T>(rr[j], r);
 #pragma unroll
-        for (int i = 0; i < VN; ++i) dh[j][i] = ln_dx(rstd, dh[j][i], m1, h[j][i], m2, dresidual != nullptr, dresidual ? r[j][i] : 0.f);
-        stv<T>(dx + base + c, dh[j]);
+        for (int i = 0; i < VN; ++i) {
+          const float dxh = __fmul_rn(__fmul_rn(alpha, go[i]), g[i]);          // the same roundings as in ln_bwd_acc
+          const float hi = __fmul_rn(h[i] - mean, rstd);
+          go[i] = ln_dx(rstd, dxh, m1, hi, m2, dresidual != nullptr, r[i]);
+        }
+        stv<T>(dx + base + c, go);
       }
     }
   }
@@ -295,8 +363,8 @@ periln_bwd_reg_kernel(const T* __restrict__ dout, const T* __restrict__ x, const
     if (c < d) {
 #pragma unroll
       for (int i = 0; i < VN; ++i) {
-        partials[((size_t)blockIdx.x * 2) * d + c + i] = ag[j][i];
-        partials[((size_t)blockIdx.x * 2 + 1) * d + c + i] = ab[j][i];
+        partials[((size_t)blockIdx.x * 2) * d + c + i] = kSmemAcc ? acc_sm[c + i] : ag[j][i];
+        partials[((size_t)blockIdx.x * 2 + 1) * d + c + i] = kSmemAcc ? acc_sm[d + c + i] : ab[j][i];
       }
     }
   }
@@ -396,22 +464,30 @@ combine_periln_kernel(const T* __restrict__ o, const T* __restrict__ y_sh, const
 // dxn[t] = sum_j dxp[pair_prow[t,j]] + dx_sh[t] + dx_r[t]  (gradient w.r.t. the pre-LN output; never stored);
 // dx[t] = dresidual[t] + LN backward of dxn[t] at (x_raw[t], stats[t], gamma); per-CTA partial dgamma / dbeta
 template <typename T, int NV, int THREADS>
-__global__ void __launch_bounds__(THREADS, NV <= 2 ? 512 / THREADS : 1)
+__global__ void __launch_bounds__(THREADS, NV <= 2 ? 768 / THREADS : 1)
 dx_sum_periln_kernel(const T* __restrict__ dxp, const T* __restrict__ dx_sh, const float* __restrict__ dx_r, const T* __restrict__ dx_r_t,
                      const int32_t* __restrict__ pair_prow, int T_, int d, int k, const T* __restrict__ x_raw, const float* __restrict__ stats,
                      const float* __restrict__ gamma, const T* __restrict__ dresidual, T* __restrict__ dx, float* __restrict__ partials) {
   constexpr int VN = VecN<T>::n;
-  __shared__ float red[THREADS / 32];
+  constexpr bool kSmemAcc = NV <= 2;          // (as in periln_bwd_reg_kernel: accumulators in shared memory, rows held as loaded)
+  extern __shared__ float acc_sm[];
+  __shared__ float red[2 * (THREADS / 32)];
   pdl_launch_dependents();
   pdl_wait();
-  float ag[NV][VN], ab[NV][VN];
+  float ag[kSmemAcc ? 1 : NV][VN], ab[kSmemAcc ? 1 : NV][VN];
 #pragma unroll
-  for (int j = 0; j < NV; ++j)
+  for (int j = 0; j < NV; ++j) {
+    const int c = (j * THREADS + threadIdx.x) * VN;
 #pragma unroll
-    for (int i = 0; i < VN; ++i) { ag[j][i] = 0.f; ab[j][i] = 0.f; }
+    for (int i = 0; i < VN; ++i) {
+      if (kSmemAcc) { if (c < d) { acc_sm[c + i] = 0.f; acc_sm[d + c + i] = 0.f; } }
+      else { ag[j][i] = 0.f; ab[j][i] = 0.f; }
+    }
+  }
   for (int t = blockIdx.x; t < T_; t += gridDim.x) {
     const size_t base = (size_t)t * d;
-    float dh[NV][VN], h[NV][VN];
+    float dh[NV][VN];
+    uint4 xr[NV], rr[NV];                      // block input row and residual-branch gradient: requested early, used last
 #pragma unroll
     for (int j = 0; j < NV; ++j) {
       const int c = (j * THREADS + threadIdx.x) * VN;
@@ -420,13 +496,11 @@ dx_sum_periln_kernel(const T* __restrict__ dxp, const T* __restrict__ dx_sh, con
 #pragma unroll
         for (int i = 0; i < VN; ++i) dh[j][i] = 0.f;
       }
-      if (c < d) ldv<T>(x_raw + base + c, h[j]);
-    }
-    float rres[NV][VN];                        // residual-branch gradient: requested early, used last
-#pragma unroll
-    for (int j = 0; j < NV; ++j) {
-      const int c = (j * THREADS + threadIdx.x) * VN;
-      if (c < d && dresidual) ldv<T>(dresidual + base + c, rres[j]);
+      xr[j] = rr[j] = make_uint4(0u, 0u, 0u, 0u);
+      if (c < d) {
+        xr[j] = *reinterpret_cast<const uint4*>(x_raw + base + c);
+        if (dresidual) rr[j] = *reinterpret_cast<const uint4*>(dresidual + base + c);
+      }
     }
     for (int jj = 0; jj < k; ++jj) {          // the order of dx_sum_kernel
       const int r = pair_prow[(size_t)t * k + jj];
@@ -458,25 +532,37 @@ dx_sum_periln_kernel(const T* __restrict__ dxp, const T* __restrict__ dx_sh, con
 #pragma unroll
           for (int i = 0; i < VN; ++i) dh[j][i] += a[i];
         }
-        float gm[VN];
-        ldv<float>(gamma + c, *reinterpret_cast<float(*)[4]>(&gm[0]));
-        if constexpr (VN == 8) ldv<float>(gamma + c + 4, *reinterpret_cast<float(*)[4]>(&gm[4]));
+        float gm[VN], h[VN], a_g[VN], a_b[VN];
+        ld_param<T, VN>(gamma + c, gm);
+        unpack<T>(xr[j], h);
+        if (kSmemAcc) { ld_param<T, VN>(acc_sm + c, a_g); ld_param<T, VN>(acc_sm + d + c, a_b); }
 #pragma unroll
         for (int i = 0; i < VN; ++i) {
           const float go = to_f32(from_f32<T>(dh[j][i]));      // what dx_sum_kernel would have stored (alpha = 1)
-          h[j][i] = __fmul_rn(h[j][i] - mean, rstd);
-          dh[j][i] = ln_bwd_acc(go, h[j][i], gm[i], ag[j][i], ab[j][i], s1, s2);   // fixed token order per CTA
+          const float hi = __fmul_rn(h[i] - mean, rstd);
+          if (kSmemAcc) dh[j][i] = ln_bwd_acc(go, hi, gm[i], a_g[i], a_b[i], s1, s2);   // fixed token order per CTA
+          else dh[j][i] = ln_bwd_acc(go, hi, gm[i], ag[j][i], ab[j][i], s1, s2);
+        }
+        if (kSmemAcc) {
+#pragma unroll
+          for (int v4 = 0; v4 < VN / 4; ++v4) {
+            *reinterpret_cast<float4*>(acc_sm + c + 4 * v4) = make_float4(a_g[4 * v4], a_g[4 * v4 + 1], a_g[4 * v4 + 2], a_g[4 * v4 + 3]);
+            *reinterpret_cast<float4*>(acc_sm + d + c + 4 * v4) = make_float4(a_b[4 * v4], a_b[4 * v4 + 1], a_b[4 * v4 + 2], a_b[4 * v4 + 3]);
+          }
         }
       }
     }
-    const float m1 = block_sum(s1, red) / (float)d;
-    const float m2 = block_sum(s2, red) / (float)d;
+    block_sum2(s1, s2, red);
+    const float m1 = s1 / (float)d, m2 = s2 / (float)d;
 #pragma unroll
     for (int j = 0; j < NV; ++j) {
       const int c = (j * THREADS + threadIdx.x) * VN;
       if (c < d) {
+        float h[VN], r[VN];
+        unpack<T>(xr[j], h);
+        unpack<T>(rr[j], r);
 #pragma unroll
-        for (int i = 0; i < VN; ++i) dh[j][i] = ln_dx(rstd, dh[j][i], m1, h[j][i], m2, dresidual != nullptr, dresidual ? rres[j][i] : 0.f);
+        for (int i = 0; i < VN; ++i) dh[j][i] = ln_dx(rstd, dh[j][i], m1, __fmul_rn(h[i] - mean, rstd), m2, dresidual != nullptr, r[i]);
         stv<T>(dx + base + c, dh[j]);
       }
     }
@@ -487,8 +573,8 @@ dx_sum_periln_kernel(const T* __restrict__ dxp, const T* __restrict__ dx_sh, con
     if (c < d) {
 #pragma unroll
       for (int i = 0; i < VN; ++i) {
-        partials[((size_t)blockIdx.x * 2) * d + c + i] = ag[j][i];
-        partials[((size_t)blockIdx.x * 2 + 1) * d + c + i] = ab[j][i];
+        partials[((size_t)blockIdx.x * 2) * d + c + i] = kSmemAcc ? acc_sm[c + i] : ag[j][i];
+        partials[((size_t)blockIdx.x * 2 + 1) * d + c + i] = kSmemAcc ? acc_sm[d + c + i] : ab[j][i];
       }
     }
   }
@@ -549,8 +635,15 @@ static int periln_fwd_t(int Tn, int d, const void* x, const float* gamma, const 
                         void* out, float* stats, cudaStream_t st) {
   int threads, nv;
   reg_shape<T>(d, threads, nv);
+  const int grid_reg = Tn < num_sms() * 32 ? Tn : num_sms() * 32;
   const int grid = Tn < num_sms() * 16 ? Tn : num_sms() * 16;
-#define LN_FWD(NV) FOMOE_CUDA_OK(launch_pdl(periln_fwd_reg_kernel<T, NV>, grid, threads, 0, st, (const T*)x, gamma, beta, (const T*)residual, alpha, eps, Tn, d, (T*)out, stats))
+#define LN_FWD(NV)                                                                                                                  \
+  do {                                                                                                                            \
+    if (residual) FOMOE_CUDA_OK(launch_pdl(periln_fwd_reg_kernel<T, NV, true>, grid_reg, threads, 0, st, (const T*)x, gamma, beta,      \
+                                           (const T*)residual, alpha, eps, Tn, d, (T*)out, stats));                                \
+    else FOMOE_CUDA_OK(launch_pdl(periln_fwd_reg_kernel<T, NV, false>, grid_reg, threads, 0, st, (const T*)x, gamma, beta,              \
+                                  (const T*)residual, alpha, eps, Tn, d, (T*)out, stats));                                         \
+  } while (0)
   if (nv == 1) LN_FWD(1);
   else if (nv == 2) LN_FWD(2);
   else if (nv == 4) LN_FWD(4);
@@ -576,7 +669,7 @@ static int periln_bwd_t(int Tn, int d, int nb, const void* dout, const void* x, 
                         const void* dresidual, void* dx, float* partials, cudaStream_t st) {
   int threads, nv;
   reg_shape<T>(d, threads, nv);
-#define LN_BWD(NV) FOMOE_CUDA_OK(launch_pdl(periln_bwd_reg_kernel<T, NV>, nb, threads, 0, st, (const T*)dout, (const T*)x, stats, gamma, alpha, (const T*)dresidual, Tn, d, (T*)dx, partials))
+#define LN_BWD(NV) FOMOE_CUDA_OK(launch_pdl(periln_bwd_reg_kernel<T, NV>, nb, threads, (NV <= 2 ? sizeof(float) * 2 * (size_t)d : 0), st, (const T*)dout, (const T*)x, stats, gamma, alpha, (const T*)dresidual, Tn, d, (T*)dx, partials))
   if (nv == 1) LN_BWD(1);
   else if (nv == 2) LN_BWD(2);
   else if (nv == 4) LN_BWD(4);
@@ -637,7 +730,7 @@ static int dx_sum_periln_t(const fomoe_config& c, const RouteWs& ws, const void*
                            const fomoe_periln_pre_bwd& ln, void* dx, int nb, cudaStream_t st) {
   int threads, nv;
   reg_shape<T>(c.d_model, threads, nv);
-#define DB(NV, TH) FOMOE_CUDA_OK(launch_pdl(dx_sum_periln_kernel<T, NV, TH>, nb, TH, 0, st, (const T*)dxp, (const T*)dx_sh, dx_r, (const T*)dx_r_t, \
+#define DB(NV, TH) FOMOE_CUDA_OK(launch_pdl(dx_sum_periln_kernel<T, NV, TH>, nb, TH, (NV <= 2 ? sizeof(float) * 2 * (size_t)c.d_model : 0), st, (const T*)dxp, (const T*)dx_sh, dx_r, (const T*)dx_r_t, \
     (const int32_t*)ws.pair_prow, c.T, c.d_model, c.top_k, (const T*)ln.x_raw, ln.stats, ln.gamma, (const T*)ln.dresidual, (T*)dx, ln.partials))
   if (threads == 128) { if (nv == 1) DB(1, 128); else if (nv == 2) DB(2, 128); else return FOMOE_ERR_UNSUPPORTED; }
   else { if (nv == 2) DB(2, 256); else if (nv == 4) DB(4, 256); else return FOMOE_ERR_UNSUPPORTED; }
