@@ -4,6 +4,7 @@
 #include <string.h>
 
 #include <atomic>
+#include <functional>
 #include <vector>
 
 #include "common.cuh"
@@ -249,45 +250,53 @@ static int moe_bwd_impl(const fomoe_config* cfg, const void* dy, const void* x, 
   ScratchWs sws = carve_scratch_ws(*cfg, rws.R_cap, scratch);
   FfnPtrs w{w_gate, w_up, w_down, sh_gate, sh_up, sh_down};
   note_api_entry("@fomoe_moe_bwd", st);
-  // B1: do = g dy per row, dgate = <dy, o>
+  // B1: do = g dy per row, dgate = <dy, o>.  Two-matrix expert on the tensor-core path: <dy, o> = <dh, h> / g falls out of the
+  // DH epilogue (dh = do W_down is there in fp32 and F is narrow), so B1 neither reads o nor reduces: one pass over [P, d] less
+  const bool tc_router = use_umma(*cfg) && cfg->T > 0;
+  const bool dgate_in_dh = tc_router && n_res > 0 && cfg->expert_fn == FOMOE_EXPERT_SILU;
   if (n_res > 0 && cfg->T > 0) {
-    rc = launch_combine_bwd(*cfg, dy, aws.o, rws, sws.dop, sws.dgate, st);
+    rc = dgate_in_dh ? launch_scale_rows(*cfg, dy, rws, sws.dop, st) : launch_combine_bwd(*cfg, dy, aws.o, rws, sws.dop, sws.dgate, st);
     if (rc != FOMOE_OK) return rc;
   } else {
     FOMOE_CUDA_OK(cudaMemsetAsync(sws.dgate, 0, sizeof(float) * (size_t)cfg->T * cfg->top_k, st));
   }
-  // B6, B7 depend only on dgate (B1): on the tensor-core path they run on the side stream, beside B2-B4
-  const bool tc_router = use_umma(*cfg) && cfg->T > 0;
+  // B6, B7 depend only on dgate: on the tensor-core path they run on the side stream, beside B2-B4 (forked after B1, or after
+  // the DH launch when that is where dgate comes from)
   SideStream* side = tc_router ? side_stream() : nullptr;
-  cudaStream_t rst = st;
-  if (side) {
-    FOMOE_CUDA_OK(cudaEventRecord(side->fork, st));
-    FOMOE_CUDA_OK(cudaStreamWaitEvent(side->s, side->fork, 0));
-    rst = side->s;
-  }
+  cudaStream_t rst = side ? side->s : st;
   auto router_bwd = [&]() -> int {
-    int r = launch_gate_bwd(*cfg, *route, rws, sws.dgate, sws.dz, tc_router ? sws.dz_bf : nullptr, sws.Ez, rst);
+    int r = launch_gate_bwd(*cfg, *route, rws, sws.dgate, dgate_in_dh ? sws.dgate_part : nullptr, sws.n_dgate_parts, sws.dz,
+                            tc_router ? sws.dz_bf : nullptr, sws.Ez, rst);
     if (r != FOMOE_OK) return r;
     // (the tensor-core router of fomoe_route left W_r in bf16 in the route workspace)
     return tc_router ? umma_router_bwd(*cfg, x, w_router, route_umma_supported(*cfg) ? rws.wr_bf : nullptr, sws, dw_router, rst)
                      : simt_router_bwd(*cfg, x, w_router, sws, dw_router, rst);
   };
+  bool forked = false;
+  auto fork_router = [&]() -> int {   // side stream: waits for everything queued on `st` so far, then runs the router's backward
+    FOMOE_CUDA_OK(cudaEventRecord(side->fork, st));
+    FOMOE_CUDA_OK(cudaStreamWaitEvent(side->s, side->fork, 0));
+    forked = true;
+    return router_bwd();
+  };
+  const std::function<int()> after_dh = [&]() -> int { return side ? fork_router() : FOMOE_OK; };
   // everything between the fork and the join: whatever it returns, the side stream is joined back into `st` afterwards (an
   // error return must not leave a forked stream dangling, least of all inside a stream capture)
   auto forked_region = [&]() -> int {
     int r = FOMOE_OK;
-    if (side) {
-      r = router_bwd();
+    if (side && !dgate_in_dh) {
+      r = fork_router();
       if (r != FOMOE_OK) return r;
     }
     // B2-B4 (+ shared experts)
-    r = use_umma(*cfg) ? umma_ffn_bwd(*cfg, n_res, x, dy, rws, aws, sws, w, dw_gate, dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, st)
+    r = use_umma(*cfg) ? umma_ffn_bwd(*cfg, n_res, x, dy, rws, aws, sws, w, dw_gate, dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, st,
+                                      dgate_in_dh, dgate_in_dh ? &after_dh : nullptr)
                        : simt_ffn_bwd(*cfg, n_res, x, dy, rws, aws, sws, w, dw_gate, dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, st);
     if (r != FOMOE_OK) return r;
-    return side ? FOMOE_OK : router_bwd();
+    return forked ? FOMOE_OK : router_bwd();
   };
   rc = forked_region();
-  if (side) {
+  if (side && forked) {
     cudaError_t e1 = cudaEventRecord(side->join, side->s);
     cudaError_t e2 = cudaStreamWaitEvent(st, side->join, 0);
     if (rc == FOMOE_OK && e1 != cudaSuccess) return set_cuda_error(e1, "cudaEventRecord(join)");

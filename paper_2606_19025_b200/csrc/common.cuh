@@ -4,6 +4,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <functional>
+
 #include "../../include/fomoe.h"
 
 namespace fomoe {
@@ -177,6 +179,9 @@ struct ScratchWs {
   void* du;        // [R_cap, F]
   void* dxp;       // [R_cap, d]
   float* dgate;    // [T*k] fp32
+  float* dgate_part; // [R_cap, n_dgate_parts] fp32: per padded row, partial <dh, h> sums written by the DH epilogue (two-matrix
+                   // expert on the tensor-core path: dgate = sum(parts) / gate, without reading o or dy again)
+  int n_dgate_parts; // 2 * ceil(F / 256): two epilogue warps share the 32-column chunks of every 256-column tile
   float* dz;       // [T, E] fp32
   float* dx_r;     // [T, d] fp32  router term dz W_r^T
   void* dsa;       // [T, n_sh*F_sh]
@@ -204,6 +209,8 @@ inline ScratchWs carve_scratch_ws(const fomoe_config& c, int R_cap, void* base) 
   w.du = take(es * (size_t)R_cap * c.d_ff);
   w.dxp = take(es * (size_t)R_cap * c.d_model);
   w.dgate = (float*)take(sizeof(float) * (size_t)c.T * c.top_k);
+  w.n_dgate_parts = 2 * ((c.d_ff + 255) / 256);
+  w.dgate_part = (float*)take(sizeof(float) * (size_t)R_cap * (size_t)w.n_dgate_parts);
   w.dz = (float*)take(sizeof(float) * (size_t)c.T * c.E);
   w.dx_r = (float*)take(sizeof(float) * (size_t)c.T * c.d_model);
   w.dsa = take(es * (size_t)c.T * fs);
@@ -233,8 +240,10 @@ int launch_combine(const fomoe_config& c, const fomoe_route_state& r, const Rout
                    void* y, cudaStream_t st);
 int launch_combine_bwd(const fomoe_config& c, const void* dy, const void* o, const RouteWs& ws, void* dop, float* dgate,
                        cudaStream_t st);
-int launch_gate_bwd(const fomoe_config& c, const fomoe_route_state& r, const RouteWs& ws, const float* dgate, float* dz,
-                    void* dz_bf, int ldz_bf, cudaStream_t st);
+int launch_scale_rows(const fomoe_config& c, const void* dy, const RouteWs& ws, void* dop, cudaStream_t st);
+// dgate_part != nullptr: dgate of a kept pair = sum of its row's n_parts partials / its gate (see ScratchWs::dgate_part)
+int launch_gate_bwd(const fomoe_config& c, const fomoe_route_state& r, const RouteWs& ws, const float* dgate, const float* dgate_part,
+                    int n_parts, float* dz, void* dz_bf, int ldz_bf, cudaStream_t st);
 int launch_dx_sum(const fomoe_config& c, const RouteWs& ws, const void* dxp, const void* dx_sh, const float* dx_r, const void* dx_r_t,
                   void* dx, cudaStream_t st);
 
@@ -254,9 +263,12 @@ int simt_router_bwd(const fomoe_config& c, const void* x, const float* w_router,
 bool umma_supported(const fomoe_config& c);
 int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs& rws, const ActWs& aws, const ScratchWs& sws,
                  const FfnPtrs& w, cudaStream_t st);
+// dgate_in_dh: the DH epilogue also writes sws.dgate_part (two-matrix expert only); after_dh, if set, is called right after
+// the routed DH launch (the router's backward chain can start there)
 int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy, const RouteWs& rws, const ActWs& aws,
                  const ScratchWs& sws, const FfnPtrs& w, void* dw_gate, void* dw_up, void* dw_down, void* d_sh_gate,
-                 void* d_sh_up, void* d_sh_down, cudaStream_t st);
+                 void* d_sh_up, void* d_sh_down, cudaStream_t st, bool dgate_in_dh = false,
+                 const std::function<int()>* after_dh = nullptr);
 
 // F1-F4 on tensor cores (ROUTE mode of the grouped kernel); called by launch_route_umma after the preparation kernel
 int umma_route(const fomoe_config& c, const void* x, const void* wr_split, int NP, int Epad, int pieces, const float* bias, int n_res,

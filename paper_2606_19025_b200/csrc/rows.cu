@@ -133,13 +133,39 @@ combine_bwd_kernel(const T* __restrict__ dy, const T* __restrict__ o, const int3
   }
 }
 
+// do[r] = g_r * dy[token(r)] only (0 for padding rows): B1 without the <dy, o> dot, for the path whose dgate comes out of the
+// DH epilogue (umma_gemm.cu)
+template <typename T, int V>
+__global__ void __launch_bounds__(kRowThreads)
+scale_rows_kernel(const T* __restrict__ dy, const int32_t* __restrict__ prow_token, const float* __restrict__ prow_gate,
+                  const int32_t* __restrict__ n_mtiles, int d, T* __restrict__ dop) {
+  pdl_launch_dependents();
+  pdl_wait();
+  const int rows = n_mtiles[1];
+  for (int r = blockIdx.x; r < rows; r += gridDim.x) {
+    const int t = prow_token[r];
+    const float g = t >= 0 ? prow_gate[r] : 0.f;
+    for (int c = threadIdx.x * V; c < d; c += kRowThreads * V) {
+      Vec<T, V> a;
+      if (t >= 0) {
+        a.load(dy + (size_t)t * d + c);
+#pragma unroll
+        for (int i = 0; i < V; ++i) a.v[i] *= g;
+      } else {
+        a.zero();
+      }
+      a.store(dop + (size_t)r * d + c);
+    }
+  }
+}
+
 // Gate rule + gate function backward (row B6): dz[t,:] from dgate[t,:].  One warp per token.
 // DZ = float (row stride E) or bf16 (row stride ldz >= E, padding columns zeroed: K-operand of the tensor-core router backward)
 template <typename DZ>
 __global__ void gate_bwd_kernel(const float* __restrict__ probs, const int32_t* __restrict__ topk_idx,
                                 const float* __restrict__ gate, const int32_t* __restrict__ pair_prow,
-                                const float* __restrict__ dgate, int T_, int E, int k, int gate_fn, int gate_rule,
-                                float inv_tau, DZ* __restrict__ dz, int ldz) {
+                                const float* __restrict__ dgate, const float* __restrict__ dgate_part, int n_parts, int T_, int E,
+                                int k, int gate_fn, int gate_rule, float inv_tau, DZ* __restrict__ dz, int ldz) {
   pdl_launch_dependents();
   pdl_wait();
   const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
@@ -151,10 +177,17 @@ __global__ void gate_bwd_kernel(const float* __restrict__ probs, const int32_t* 
   float dg = 0.f, g = 0.f, p = 0.f;
   if (lane < k) {
     e = topk_idx[(size_t)t * k + lane];
-    kept = pair_prow[(size_t)t * k + lane] >= 0;
+    const int pr = pair_prow[(size_t)t * k + lane];
+    kept = pr >= 0;
     g = gate[(size_t)t * k + lane];
     p = probs[(size_t)t * E + e];
-    dg = kept ? dgate[(size_t)t * k + lane] : 0.f;
+    if (kept && dgate_part) {   // <dy, o> = <dh, h> / g with dh = g dy W_down: partial sums from the DH epilogue, fixed order
+      float sacc = 0.f;
+      for (int i = 0; i < n_parts; ++i) sacc += dgate_part[(size_t)pr * n_parts + i];
+      dg = g != 0.f ? sacc / g : 0.f;
+    } else {
+      dg = kept ? dgate[(size_t)t * k + lane] : 0.f;
+    }
   }
   float dp = 0.f;  // dL/dp of the expert this lane owns
   if (gate_rule == FOMOE_DROP_ONLY) {
@@ -255,15 +288,23 @@ int launch_combine_bwd(const fomoe_config& c, const void* dy, const void* o, con
   return FOMOE_OK;
 }
 
-int launch_gate_bwd(const fomoe_config& c, const fomoe_route_state& r, const RouteWs& ws, const float* dgate, float* dz,
-                    void* dz_bf, int ldz_bf, cudaStream_t st) {
+int launch_scale_rows(const fomoe_config& c, const void* dy, const RouteWs& ws, void* dop, cudaStream_t st) {
+  ROWS_DISPATCH(c, FOMOE_CUDA_OK(launch_pdl(scale_rows_kernel<T, V>, row_grid(ws.R_cap, c.d_model), kRowThreads, 0, st, (const T*)dy, ws.prow_token,
+                                            ws.prow_gate, ws.n_mtiles, c.d_model, (T*)dop)));
+  FOMOE_LAUNCH_OK("scale_rows_kernel");
+  return FOMOE_OK;
+}
+
+int launch_gate_bwd(const fomoe_config& c, const fomoe_route_state& r, const RouteWs& ws, const float* dgate, const float* dgate_part,
+                    int n_parts, float* dz, void* dz_bf, int ldz_bf, cudaStream_t st) {
   if (c.T == 0) return FOMOE_OK;
   if (dz_bf)
     FOMOE_CUDA_OK(launch_pdl(gate_bwd_kernel<__nv_bfloat16>, ceil_div(c.T, 8), 256, 0, st, r.probs, r.topk_idx, r.gate, ws.pair_prow, dgate,
-                             c.T, c.E, c.top_k, c.gate_fn, c.gate_rule, 1.0f / c.temperature, (__nv_bfloat16*)dz_bf, ldz_bf));
+                             dgate_part, n_parts, c.T, c.E, c.top_k, c.gate_fn, c.gate_rule, 1.0f / c.temperature, (__nv_bfloat16*)dz_bf,
+                             ldz_bf));
   else
-    FOMOE_CUDA_OK(launch_pdl(gate_bwd_kernel<float>, ceil_div(c.T, 8), 256, 0, st, r.probs, r.topk_idx, r.gate, ws.pair_prow, dgate, c.T,
-                             c.E, c.top_k, c.gate_fn, c.gate_rule, 1.0f / c.temperature, dz, c.E));
+    FOMOE_CUDA_OK(launch_pdl(gate_bwd_kernel<float>, ceil_div(c.T, 8), 256, 0, st, r.probs, r.topk_idx, r.gate, ws.pair_prow, dgate,
+                             dgate_part, n_parts, c.T, c.E, c.top_k, c.gate_fn, c.gate_rule, 1.0f / c.temperature, dz, c.E));
   FOMOE_LAUNCH_OK("gate_bwd_kernel");
   return FOMOE_OK;
 }

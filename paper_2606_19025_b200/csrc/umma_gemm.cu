@@ -95,6 +95,9 @@ struct UmmaParams {
   float* tail_part;
   bf16 *out0, *out1, *out2;    // FWD1: a,u,h | FWD2/DX: out | DH: da,du | WGRAD: dW
   const bf16 *in0, *in1;       // DH: a,u
+  const bf16* in_h;            // DH, two-matrix expert (in1 == nullptr): the saved h, streamed in u's ring slot, for
+  float* dgate_part;           //   dgate_part[row, 2 n_tile + half] = sum over this warp's chunks of dh * h  (ScratchWs::dgate_part)
+  int n_dgate_parts;
   RouteEpi r;                  // ROUTE
   // WGRAD, several weight gradients of the same row groups in ONE launch (dW_down, dW_gate, dW_up): n_jobs > 0 overrides
   // M, N, out0; job j reads tensor maps m[2j] (A) and m[2j+1] (B).  One launch instead of three saves two kernel prologues
@@ -928,6 +931,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
       int pcc = half;
       bool pvalid = pid < sched.total;
       Tile pt = pvalid ? sched.decode(pid) : Tile{};
+      const bf16* in_second = p.in1 ? p.in1 : p.in_h;
       auto issue = [&](int slot) {
         while (pvalid && pt.n_tile * BN + pcc * 32 >= p.F) {  // this warp has no (more) chunk in the tile
           pcc = half;
@@ -947,7 +951,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
               const bool ok = r < prows;
               const size_t g = off + (size_t)(ok ? r : 0) * p.ld + c * 8;
               cp_async16(sa + stg_off(r, c), p.in0 + g, ok);
-              if (p.in1) cp_async16(su + stg_off(r, c), p.in1 + g, ok);   // in1 == nullptr: two-matrix expert, da only
+              if (in_second) cp_async16(su + stg_off(r, c), in_second + g, ok);   // SwiGLU: silu(a); two-matrix expert: h (or nothing)
             }
           }
           pcc += 2;
@@ -972,6 +976,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
         const size_t base = (size_t)row0 * p.ld + (size_t)t.part * p.F;
         mbar_wait(smem_u32(&tfull_bar[as]), aphase);
         tc_fence_after();
+        float dg_acc = 0.f;   // <dh, h> over this warp's chunks of the tile, for this lane's row
 #pragma unroll 1
         for (int cc = half; cc < BN / 32; cc += 2) {
           const int n = t.n_tile * BN + cc * 32;
@@ -986,7 +991,7 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
 #pragma unroll
             for (int g8 = 0; g8 < 4; ++g8) {
               const uint32_t o = stg_off(lane, g8);
-              uint4 wa = lds128(sa + o), wu = p.in1 ? lds128(su + o) : make_uint4(0u, 0u, 0u, 0u);
+              uint4 wa = lds128(sa + o), wu = in_second ? lds128(su + o) : make_uint4(0u, 0u, 0u, 0u);
               uint32_t* pa = reinterpret_cast<uint32_t*>(&wa);
               uint32_t* pu = reinterpret_cast<uint32_t*>(&wu);
 #pragma unroll
@@ -994,7 +999,8 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
                 const float2 a2 = unpack_bf16x2(pa[i]), u2 = unpack_bf16x2(pu[i]);
                 const float d0 = dh[g8 * 8 + 2 * i], d1 = dh[g8 * 8 + 2 * i + 1];
                 pa[i] = pack_bf16x2(d0 * a2.x, d1 * a2.y);
-                pu[i] = pack_bf16x2(d0 * u2.x, d1 * u2.y);
+                if (p.in1) pu[i] = pack_bf16x2(d0 * u2.x, d1 * u2.y);
+                else { dg_acc = fmaf(d0, u2.x, dg_acc); dg_acc = fmaf(d1, u2.y, dg_acc); }   // second stream = h: gate gradient
               }
               sts128(sa + o, wa);   // da over a, du over u: every lane rewrites exactly the bytes it read
               if (p.in1) sts128(su + o, wu);
@@ -1007,6 +1013,8 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
           issue(slot);                                        // refill the slot just stored from
           if (++slot == kDhDepth) slot = 0;
         }
+        if (p.dgate_part && rows_valid > 0 && lane < rows_valid)
+          p.dgate_part[(size_t)(row0 + lane) * p.n_dgate_parts + 2 * t.n_tile + half] = dg_acc;
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive_cluster(tempty_leader + 8 * as);
@@ -1374,7 +1382,7 @@ int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs&
 
 int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy, const RouteWs& rws, const ActWs& aws,
                  const ScratchWs& sws, const FfnPtrs& w, void* dw_gate, void* dw_up, void* dw_down, void* d_sh_gate,
-                 void* d_sh_up, void* d_sh_down, cudaStream_t st) {
+                 void* d_sh_up, void* d_sh_down, cudaStream_t st, bool dgate_in_dh, const std::function<int()>* after_dh) {
   const int d = c.d_model, F = c.d_ff;
   const bool silu = c.expert_fn == FOMOE_EXPERT_SILU;   // two-matrix expert: one saved factor, dxp = dA W_up, dW_up = dA^T x
   if (n_res > 0) {
@@ -1389,8 +1397,10 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
         m.m[2] = m.m[3] = m.m[0];
         UmmaParams q = p;
         q.in0 = (const bf16*)aws.a; q.in1 = silu ? nullptr : (const bf16*)aws.u; q.out0 = (bf16*)sws.da; q.out1 = (bf16*)sws.du;
+        if (dgate_in_dh && silu) { q.in_h = (const bf16*)aws.h; q.dgate_part = sws.dgate_part; q.n_dgate_parts = sws.n_dgate_parts; }
         int rc = launch<DH>(m, q, st, "umma_grouped_kernel<DH>");
         if (rc != FOMOE_OK) return rc;
+        if (after_dh) { rc = (*after_dh)(); if (rc != FOMOE_OK) return rc; }
       }
       {  // dxp = dA W_gate + dU W_up
         TmaMaps m{};
