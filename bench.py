@@ -233,6 +233,8 @@ def hbm_bytes(name: str, P: int, T: int, w: W.MoEWorkload):
         return (P + T * (2 if w.n_sh else 1)) * w.d * s, None
     if name.startswith("combine_bwd"):
         return 3 * P * w.d * s, None
+    if name.startswith("scale_rows"):   # do = g dy without the <dy, o> dot (two-matrix expert: dgate comes out of the DH epilogue)
+        return (P * w.d * s, "dy served from L2: only the write counted") if x_in_l2 else (2 * P * w.d * s, None)
     if name.startswith("dx_sum"):
         return (P + T * (2 + (1 if w.n_sh else 0))) * w.d * s, None
     return None
