@@ -546,10 +546,13 @@ def run_gpu(args, w, n_res):
             if mf / ms > ideal:   # a speed-up above the FLOP ratio means the all-resident arm ran less efficiently: say why
                 a, b = clocks.get("sm_mhz"), clocks_full.get("sm_mhz")
                 sk["above_ideal_because"] = (
-                    f"the longer all-resident step ran at a lower SM clock ({b} MHz against {a} MHz for the skip arm, power cap); "
-                    f"clock-normalised speed-up {mf / ms * (b / a):.2f}x" if a and b and b < 0.98 * a else
+                    f"the longer all-resident step settles under the power cap (NVML: {b} MHz, reasons {clocks_full.get('reasons')}) while "
+                    f"the short skip arm samples {a} MHz: the arms do not run at the same clock, so the ratio overstates the kernels' "
+                    f"share of the gain; per-arm TFLOP/s: {sk['tflops_all_resident']:.0f} (all resident) vs {out['tflops']:.0f} (skip)"
+                    if a and b and b < 0.98 * a else
                     f"not a clock effect ({b} vs {a} MHz): the all-resident arm reached {sk['tflops_all_resident']:.0f} TFLOP/s "
-                    f"against {out['tflops']:.0f} for the skip arm on the same kernels")
+                    f"against {out['tflops']:.0f} for the skip arm on the same kernels (its larger routed share runs the less "
+                    f"efficient routed GEMMs and row kernels)")
             out["skip_token"] = sk
             del full, full_step
 
