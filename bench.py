@@ -207,6 +207,8 @@ def gemm_flops(mode: str, P: int, T: int, w: W.MoEWorkload, launches_per_step: f
         return 2.0 * T * w.d * w.E
     if "router" in mode:   # dz W_r^T and x^T dz: 2*T*d*E each
         return 2.0 * T * w.d * w.E
+    if mode.startswith("fine_gather_kernel"):   # fine_gemm.cu: F1 and DH are one GEMM over the kept rows, WG is both weight gradients
+        return (4.0 if "<WG>" in mode else 2.0) * P * w.d * w.F
     shared = "shared" in mode
     rows, F = (T * w.n_sh, w.F_sh) if shared else (P, w.F)
     mult = 4 if (("FWD1" in mode and "FWD1S" not in mode) or ("DX" in mode and w.expert_fn == W.EXPERT_SWIGLU)) else 2
@@ -366,7 +368,7 @@ def run_gpu(args, w, n_res):
                     k["note"] = note
                 k["frac"] = k["achieved"] / peaks["hbm_gbs"]
                 k["frac_of_nominal_8000"] = k["achieved"] / 8000.0
-            elif name.startswith("umma_grouped_kernel"):
+            elif name.startswith("umma_grouped_kernel") or name.startswith("fine_gather_kernel"):
                 fl = gemm_flops(name, P, w.T, w, n / args.steps)
                 k.update(bound="tensor", achieved=fl / (tt / n / 1e3) / 1e12, unit="TFLOP/s")
                 k["frac"] = k["achieved"] / tc_peak

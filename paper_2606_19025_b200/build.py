@@ -8,7 +8,7 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 LIB = HERE / "libfomoe.so"
-SOURCES = ["api.cu", "route.cu", "route_umma.cu", "rows.cu", "simt_gemm.cu", "umma_gemm.cu", "pack.cu", "optim.cu", "periln.cu", "diag.cu"]
+SOURCES = ["api.cu", "route.cu", "route_umma.cu", "rows.cu", "simt_gemm.cu", "umma_gemm.cu", "fine_gemm.cu", "pack.cu", "optim.cu", "periln.cu", "diag.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--expt-relaxed-constexpr",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "-cudart", "static"]
 

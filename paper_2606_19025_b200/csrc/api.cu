@@ -201,7 +201,9 @@ static int moe_fwd_impl(const fomoe_config* cfg, const void* x, const fomoe_rout
   FfnPtrs w{w_gate, w_up, w_down, sh_gate, sh_up, sh_down};
   note_api_entry("@fomoe_moe_fwd", st);
   if (cfg->T == 0) return FOMOE_OK;
-  if (n_res > 0) {
+  // the permuted copy of x: not needed when both of its readers (forward GEMM 1, dW_up) gather their rows themselves
+  const int fine = use_umma(*cfg) ? fine_mask(*cfg) : 0;
+  if (n_res > 0 && (fine & 5) != 5) {
     rc = launch_gather_rows(*cfg, x, rws, aws.xp, st);
     if (rc != FOMOE_OK) return rc;
   }
@@ -254,7 +256,10 @@ static int moe_bwd_impl(const fomoe_config* cfg, const void* dy, const void* x, 
   // DH epilogue (dh = do W_down is there in fp32 and F is narrow), so B1 neither reads o nor reduces: one pass over [P, d] less
   const bool tc_router = use_umma(*cfg) && cfg->T > 0;
   const bool dgate_in_dh = tc_router && n_res > 0 && cfg->expert_fn == FOMOE_EXPERT_SILU;
-  if (n_res > 0 && cfg->T > 0) {
+  const int fine = tc_router ? fine_mask(*cfg) : 0;   // (fine_gemm.cu: bit 1 = DH gathers dy rows, bit 2 = so do the weight gradients)
+  if (n_res > 0 && cfg->T > 0 && (fine & 6) == 6) {
+    // no B1 kernel at all: the gate scales DH's accumulator, dgate is DH's <dh, h>
+  } else if (n_res > 0 && cfg->T > 0) {
     rc = dgate_in_dh ? launch_scale_rows(*cfg, dy, rws, sws.dop, st) : launch_combine_bwd(*cfg, dy, aws.o, rws, sws.dop, sws.dgate, st);
     if (rc != FOMOE_OK) return rc;
   } else {
@@ -265,7 +270,8 @@ static int moe_bwd_impl(const fomoe_config* cfg, const void* dy, const void* x, 
   SideStream* side = tc_router ? side_stream() : nullptr;
   cudaStream_t rst = side ? side->s : st;
   auto router_bwd = [&]() -> int {
-    int r = launch_gate_bwd(*cfg, *route, rws, sws.dgate, dgate_in_dh ? sws.dgate_part : nullptr, sws.n_dgate_parts, sws.dz,
+    int r = launch_gate_bwd(*cfg, *route, rws, sws.dgate, dgate_in_dh ? sws.dgate_part : nullptr,
+                            (fine & 2) ? -sws.n_dgate_parts : sws.n_dgate_parts, sws.dz,
                             tc_router ? sws.dz_bf : nullptr, sws.Ez, rst);
     if (r != FOMOE_OK) return r;
     // (the tensor-core router of fomoe_route left W_r in bf16 in the route workspace)

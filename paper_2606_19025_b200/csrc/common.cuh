@@ -241,7 +241,8 @@ int launch_combine(const fomoe_config& c, const fomoe_route_state& r, const Rout
 int launch_combine_bwd(const fomoe_config& c, const void* dy, const void* o, const RouteWs& ws, void* dop, float* dgate,
                        cudaStream_t st);
 int launch_scale_rows(const fomoe_config& c, const void* dy, const RouteWs& ws, void* dop, cudaStream_t st);
-// dgate_part != nullptr: dgate of a kept pair = sum of its row's n_parts partials / its gate (see ScratchWs::dgate_part)
+// dgate_part != nullptr: dgate of a kept pair = sum of its row's n_parts partials / its gate (see ScratchWs::dgate_part);
+// n_parts < 0: -n_parts partials that are NOT scaled by the gate (the gathered DH of fine_gemm.cu), no division
 int launch_gate_bwd(const fomoe_config& c, const fomoe_route_state& r, const RouteWs& ws, const float* dgate, const float* dgate_part,
                     int n_parts, float* dz, void* dz_bf, int ldz_bf, cudaStream_t st);
 int launch_dx_sum(const fomoe_config& c, const RouteWs& ws, const void* dxp, const void* dx_sh, const float* dx_r, const void* dx_r_t,
@@ -269,6 +270,16 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
                  const ScratchWs& sws, const FfnPtrs& w, void* dw_gate, void* dw_up, void* dw_down, void* d_sh_gate,
                  void* d_sh_up, void* d_sh_down, cudaStream_t st, bool dgate_in_dh = false,
                  const std::function<int()>* after_dh = nullptr);
+
+// Fine-grained two-matrix experts (d_expert = 128), fine_gemm.cu: the expert GEMMs gather their token-indexed
+// operand rows inside the kernel (no permuted copy of x or dy).  fine_mask: which of them apply to this configuration
+// (bit 0 = forward GEMM 1, bit 1 = DH, bit 2 = the weight gradients; 0 = none: the grouped kernels of umma_gemm.cu run).
+int fine_mask(const fomoe_config& c);
+int fine_fwd1(const fomoe_config& c, int n_res, const void* x, const RouteWs& rws, const ActWs& aws, const void* w_up, cudaStream_t st);
+int fine_dh(const fomoe_config& c, int n_res, const void* dy, const RouteWs& rws, const ActWs& aws, const ScratchWs& sws, void* hg,
+            const void* w_down, cudaStream_t st);
+int fine_wgrad(const fomoe_config& c, int n_res, const void* x, const void* dy, const RouteWs& rws, const ScratchWs& sws, const void* hg,
+               void* dw_up, void* dw_down, cudaStream_t st);
 
 // F1-F4 on tensor cores (ROUTE mode of the grouped kernel); called by launch_route_umma after the preparation kernel
 int umma_route(const fomoe_config& c, const void* x, const void* wr_split, int NP, int Epad, int pieces, const float* bias, int n_res,

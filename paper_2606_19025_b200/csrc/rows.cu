@@ -182,9 +182,10 @@ __global__ void gate_bwd_kernel(const float* __restrict__ probs, const int32_t* 
     g = gate[(size_t)t * k + lane];
     p = probs[(size_t)t * E + e];
     if (kept && dgate_part) {   // <dy, o> = <dh, h> / g with dh = g dy W_down: partial sums from the DH epilogue, fixed order
+      const int np = n_parts < 0 ? -n_parts : n_parts;   // n_parts < 0: the partials are <dy W_down, h> itself, not scaled by g
       float sacc = 0.f;
-      for (int i = 0; i < n_parts; ++i) sacc += dgate_part[(size_t)pr * n_parts + i];
-      dg = g != 0.f ? sacc / g : 0.f;
+      for (int i = 0; i < np; ++i) sacc += dgate_part[(size_t)pr * np + i];
+      dg = n_parts < 0 ? sacc : g != 0.f ? sacc / g : 0.f;
     } else {
       dg = kept ? dgate[(size_t)t * k + lane] : 0.f;
     }

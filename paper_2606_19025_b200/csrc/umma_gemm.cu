@@ -1305,7 +1305,10 @@ int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs&
     const uint64_t R = (uint64_t)rws.R_cap;
     UmmaParams p{};
     p.n_mtiles = rws.n_mtiles; p.tile_slot = rws.tile_slot; p.pair_info = rws.pair_info; p.parts = 1; p.d = d; p.F = F; p.ld = F;
-    if (silu) {   // two-matrix expert: a = X W_up^T, h = silu(a)
+    if (silu && (fine_mask(c) & 1)) {   // d_expert = 128: x rows gathered inside the kernel (fine_gemm.cu)
+      int rc = fine_fwd1(c, n_res, x, rws, aws, w.w_up, st);
+      if (rc != FOMOE_OK) return rc;
+    } else if (silu) {   // two-matrix expert: a = X W_up^T, h = silu(a)
       TmaMaps m{};
       MAP_OK(make_map(&m.m[0], aws.xp, d, R, d, 128));
       MAP_OK(make_map(&m.m[1], w.w_up, d, (uint64_t)n_res * F, d, 128));
@@ -1389,8 +1392,14 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
     const uint64_t R = (uint64_t)rws.R_cap;
     UmmaParams p{};
     p.n_mtiles = rws.n_mtiles; p.tile_slot = rws.tile_slot; p.pair_info = rws.pair_info; p.pad_offsets = rws.pad_offsets; p.pad_end64 = rws.pad_end64; p.parts = 1; p.d = d; p.F = F; p.ld = F;
+    const int fine = silu ? fine_mask(c) : 0;
+    void* hg = sws.du;    // fine path: g h [R, F] (the two-matrix expert has no du)
     if (c.T > 0) {
-      {  // dh = dO W_down, fused SwiGLU backward
+      if (fine & 2) {  // dh = dy[token] W_down gathered in the kernel; da, hg = g h and <dh, h> out of its epilogue
+        int rc = fine_dh(c, n_res, dy, rws, aws, sws, hg, w.w_down, st);
+        if (rc != FOMOE_OK) return rc;
+        if (after_dh) { rc = (*after_dh)(); if (rc != FOMOE_OK) return rc; }
+      } else {  // dh = dO W_down, fused SwiGLU backward
         TmaMaps m{};
         MAP_OK(make_map(&m.m[0], sws.dop, d, R, d, 128));
         MAP_OK(make_map(&m.m[1], w.w_down, F, (uint64_t)n_res * d, F, 64));
@@ -1420,7 +1429,10 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
     struct WG { const void* A; int lda; const void* B; int ldb; int M, N; void* out; };
     const WG jobs[3] = {{sws.dop, d, aws.h, F, d, F, dw_down}, {sws.da, F, aws.xp, d, F, d, silu ? dw_up : dw_gate},
                         {sws.du, F, aws.xp, d, F, d, dw_up}};
-    {   // one launch for all of them (same row groups, same K ranges)
+    if (fine & 4) {
+      int rc = fine_wgrad(c, n_res, x, dy, rws, sws, hg, dw_up, dw_down, st);
+      if (rc != FOMOE_OK) return rc;
+    } else {   // one launch for all of them (same row groups, same K ranges)
       TmaMaps m{};
       UmmaParams q = p;
       const int nj = silu ? 2 : 3;
