@@ -102,6 +102,11 @@ __device__ __forceinline__ void g_tmem_ld16(uint32_t taddr, float (&v)[16]) {
 __device__ __forceinline__ void g_sts128(uint32_t addr, const uint4& v) {
   asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
+__device__ __forceinline__ uint4 g_lds128(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+  return v;
+}
 __device__ __forceinline__ uint32_t g_pack(float lo, float hi) {
   __nv_bfloat162 h = __floats2bfloat162_rn(lo, hi);
   return *reinterpret_cast<uint32_t*>(&h);
@@ -410,55 +415,85 @@ fine_gather_kernel(const __grid_constant__ GMaps maps, const __grid_constant__ G
           }
         }
       } else if (MODE == G_DH) {
-        for (int half = 0; half < it.ntiles; ++half) {
-          const int rw = it.row0 + half * GT + q * 32, row = rw + lane;
-          const float g = p.prow_token[row] >= 0 ? p.prow_gate[row] : 0.f;
-          float dg = 0.f;   // <dy W_down, h> of this lane's row, fixed order
-#pragma unroll 1
-          for (int cc = 0; cc < 4; ++cc) {
-            const uint32_t s0 = stg_w + (nst & 1) * 2 * kGStgTile, s1 = s0 + kGStgTile;
-            if (lane == 0) bulk_wait_read<1>();
-            __syncwarp();
+        // The saved factors silu'(a) and h of a 32 x 32 chunk are copied (cp.async, each lane its own row's 64 bytes) into
+        // the two staging tiles one chunk ahead, overwritten in place with da and hg, and stored from there.
+        const int n8 = 4 * it.ntiles;                          // chunks of this item: (half, 32-column block)
+        const uint32_t loff = (uint32_t)(lane * 64), lsw = (uint32_t)((lane >> 1) & 3);
+        auto issue = [&](int c8) {
+          const uint32_t sa = stg_w + (c8 & 1) * 2 * kGStgTile + loff, sh = sa + kGStgTile;
+          const size_t off = (size_t)(it.row0 + (c8 >> 2) * GT + q * 32 + lane) * GT + (c8 & 3) * 32;
 #pragma unroll
-            for (int sub = 0; sub < 2; ++sub) {
-              const size_t off = (size_t)row * GT + cc * 32 + sub * 16;
-              const uint4* pa = reinterpret_cast<const uint4*>(p.in0 + off);
-              const uint4* ph = reinterpret_cast<const uint4*>(p.in_h + off);
-              uint4 wa[2] = {__ldg(pa), __ldg(pa + 1)}, wh[2] = {__ldg(ph), __ldg(ph + 1)};
-              float v[16], hg[16];
-              g_tmem_ld16(tacc + half * 128 + cc * 32 + sub * 16, v);
-              tmem_ld_wait();
-#pragma unroll
-              for (int j = 0; j < 2; ++j) {
-                const uint32_t* ua = reinterpret_cast<const uint32_t*>(&wa[j]);
-                const uint32_t* uh = reinterpret_cast<const uint32_t*>(&wh[j]);
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                  const float2 a2 = g_unpack(ua[i]), h2 = g_unpack(uh[i]);
-                  const float d0 = v[8 * j + 2 * i], d1 = v[8 * j + 2 * i + 1];
-                  dg = fmaf(d0, h2.x, dg);
-                  dg = fmaf(d1, h2.y, dg);
-                  v[8 * j + 2 * i] = (g * d0) * a2.x;        // da = dh silu'(a), dh = g (dy W_down)
-                  v[8 * j + 2 * i + 1] = (g * d1) * a2.y;
-                  hg[8 * j + 2 * i] = g * h2.x;              // the weight gradient's operand: dW_down = dy^T (g h)
-                  hg[8 * j + 2 * i + 1] = g * h2.y;
-                }
-              }
-              g_put16(s0, lane, 2 * sub, v);
-              g_put16(s1, lane, 2 * sub, hg);
-            }
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            __syncwarp();
-            if (lane == 0) {
-              tma_store_2d(&maps.m[1], s0, cc * 32, rw);
-              tma_store_2d(&maps.m[2], s1, cc * 32, rw);
-              bulk_commit();
-            }
-            ++nst;
+          for (int qq = 0; qq < 4; ++qq) {
+            g_cp_async16(sa + ((qq ^ lsw) << 4), p.in0 + off + qq * 8, true);
+            g_cp_async16(sh + ((qq ^ lsw) << 4), p.in_h + off + qq * 8, true);
           }
-          float* dp = p.dgate_part + (size_t)row * p.n_dgate_parts;
-          dp[0] = dg;
-          for (int i = 1; i < p.n_dgate_parts; ++i) dp[i] = 0.f;
+          asm volatile("cp.async.commit_group;" ::: "memory");
+        };
+        if (lane == 0) bulk_wait_read<0>();   // the previous item's last stores have read the tiles
+        __syncwarp();
+        issue(0);
+        float g = 0.f, dg = 0.f;
+        int row = 0;
+#pragma unroll 1
+        for (int c8 = 0; c8 < n8; ++c8) {
+          const int half = c8 >> 2, cc = c8 & 3;
+          if (cc == 0) {
+            row = it.row0 + half * GT + q * 32 + lane;
+            g = p.prow_token[row] >= 0 ? p.prow_gate[row] : 0.f;
+            dg = 0.f;                                          // <dy W_down, h> of this lane's row, fixed order
+          }
+          if (c8 + 1 < n8) {
+            if (c8 >= 1) {                                     // the other pair of tiles: chunk c8 - 1's stores must have read it
+              if (lane == 0) bulk_wait_read<0>();
+              __syncwarp();
+            }
+            issue(c8 + 1);
+            asm volatile("cp.async.wait_group 1;" ::: "memory");
+          } else {
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+          }
+          const uint32_t sa = stg_w + (c8 & 1) * 2 * kGStgTile + loff, sh = sa + kGStgTile;
+#pragma unroll
+          for (int sub = 0; sub < 2; ++sub) {
+            float v[16];
+            g_tmem_ld16(tacc + half * 128 + cc * 32 + sub * 16, v);
+            uint4 wa[2], wh[2];
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+              wa[j] = g_lds128(sa + (((2 * sub + j) ^ lsw) << 4));
+              wh[j] = g_lds128(sh + (((2 * sub + j) ^ lsw) << 4));
+            }
+            tmem_ld_wait();
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+              uint32_t* ua = reinterpret_cast<uint32_t*>(&wa[j]);
+              uint32_t* uh = reinterpret_cast<uint32_t*>(&wh[j]);
+#pragma unroll
+              for (int i = 0; i < 4; ++i) {
+                const float2 a2 = g_unpack(ua[i]), h2 = g_unpack(uh[i]);
+                const float d0 = v[8 * j + 2 * i], d1 = v[8 * j + 2 * i + 1];
+                dg = fmaf(d0, h2.x, dg);
+                dg = fmaf(d1, h2.y, dg);
+                ua[i] = g_pack((g * d0) * a2.x, (g * d1) * a2.y);   // da = dh silu'(a), dh = g (dy W_down)
+                uh[i] = g_pack(g * h2.x, g * h2.y);                 // the weight gradient's operand: dW_down = dy^T (g h)
+              }
+              g_sts128(sa + (((2 * sub + j) ^ lsw) << 4), wa[j]);
+              g_sts128(sh + (((2 * sub + j) ^ lsw) << 4), wh[j]);
+            }
+          }
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          __syncwarp();
+          if (lane == 0) {
+            const int rw = it.row0 + half * GT + q * 32;
+            tma_store_2d(&maps.m[1], sa - loff, cc * 32, rw);
+            tma_store_2d(&maps.m[2], sh - loff, cc * 32, rw);
+            bulk_commit();
+          }
+          if (cc == 3) {
+            float* dp = p.dgate_part + (size_t)row * p.n_dgate_parts;
+            dp[0] = dg;
+            for (int i = 1; i < p.n_dgate_parts; ++i) dp[i] = 0.f;
+          }
         }
       } else {
         // job 0: rows = f, 8 chunks of 32 d columns; job 1: two halves of 128 d rows, 4 chunks of 32 f columns each
