@@ -65,9 +65,10 @@ struct GParams {
   float* dgate_part;           // DH: [R, n_dgate_parts]: part 0 = <dh, h> (not scaled by the gate), the rest 0
   int n_dgate_parts;
   int d, n_res;
-  // WG with few tiles (n_res * 2 * d / 256 < SMs): every tile's K range is cut into `ks` parts, each part an item of its own
-  // writing an fp32 partial [128, 256] to `part`; fine_wg_reduce_kernel adds them in a fixed order
-  int ks;
+  // WG: the tiles of the last, partially filled round of the grid (tile ids >= wg_full; all of them when the tiles do not
+  // fill the SMs once) have their K range cut into `ks` parts, each part an item of its own writing an fp32 partial
+  // [128, 256] to `part`; fine_wg_reduce_kernel adds them in a fixed order
+  int ks, wg_full;
   float* part;
 };
 
@@ -140,7 +141,7 @@ struct GItem {
   int slot;
   int num_kb;
   int job, n0;   // WG: 0 = dW_up (gathered operand = B, N = 256), 1 = dW_down (gathered = A, two 128-row halves); first d column
-  long pidx;     // WG split-K: index of this item's partial tile in GParams::part
+  long pidx;     // WG split-K: index of this item's partial tile in GParams::part, -1 = a whole tile (stored as bf16)
 };
 
 template <int MODE>
@@ -149,8 +150,9 @@ struct GSched {
   long total, full;
   __device__ GSched(const GParams& p_, int grid) : p(p_) {
     if (MODE == G_WG) {
-      total = (long)p.n_res * 2 * (p.d / 256) * p.ks;
-      full = total;
+      const long tiles = (long)p.n_res * 2 * (p.d / 256);
+      full = p.wg_full;
+      total = full + (tiles - full) * p.ks;
     } else {
       const long n_pairs = p.n_mtiles[2];
       full = n_pairs / grid * grid;
@@ -162,16 +164,20 @@ struct GSched {
     it.job = 0; it.n0 = 0;
     if (MODE == G_WG) {
       const int ntn = p.d / 256;
-      it.pidx = id;
-      const int kpart = (int)(id % p.ks);
-      id /= p.ks;
+      it.pidx = -1;
+      int kpart = 0;
+      if (id >= full) {
+        it.pidx = id - full;
+        kpart = (int)(it.pidx % p.ks);
+        id = full + it.pidx / p.ks;
+      }
       it.slot = (int)(id / (2 * ntn));
       const int rem = (int)(id % (2 * ntn));
       it.job = rem / ntn;
       it.n0 = (rem % ntn) * 256;
       it.row0 = p.pad_offsets[it.slot];
       it.num_kb = (p.pad_end64[it.slot] - it.row0 + GK - 1) / GK;
-      if (p.ks > 1) {   // this part's K blocks
+      if (it.pidx >= 0 && p.ks > 1) {   // this part's K blocks
         const int per = (it.num_kb + p.ks - 1) / p.ks, kb0 = min(kpart * per, it.num_kb), kb1 = min(kb0 + per, it.num_kb);
         it.row0 += kb0 * GK;
         it.num_kb = kb1 - kb0;
@@ -498,7 +504,7 @@ fine_gather_kernel(const __grid_constant__ GMaps maps, const __grid_constant__ G
       } else {
         // job 0: rows = f, 8 chunks of 32 d columns; job 1: two halves of 128 d rows, 4 chunks of 32 f columns each
         const int n_chunks = 8;
-        if (p.ks > 1) {   // fp32 partial of this K part: row-per-lane 64-byte segments (small: only when the tiles do not fill the GPU)
+        if (it.pidx >= 0 && p.ks > 1) {   // fp32 partial of this K part: row-per-lane 64-byte segments (tail tiles only)
           float* dst = p.part + ((size_t)it.pidx * GT + q * 32 + lane) * 256;
 #pragma unroll 1
           for (int c16 = 0; c16 < 16; ++c16) {
@@ -556,18 +562,18 @@ fine_gather_kernel(const __grid_constant__ GMaps maps, const __grid_constant__ G
   if (warp == 2) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kGTmemCols) : "memory");
 }
 
-// adds the ks partials of every WG tile in a fixed order and writes dW_up / dW_down as bf16.  grid = (tiles, 8 row slabs)
+// adds the ks partials of every split WG tile in a fixed order and writes dW_up / dW_down as bf16.  grid = (split tiles, 8 row slabs)
 __global__ void __launch_bounds__(256)
-fine_wg_reduce_kernel(const float* __restrict__ part, int ks, int d, bf16* __restrict__ dw_up, bf16* __restrict__ dw_down) {
+fine_wg_reduce_kernel(const float* __restrict__ part, int ks, int first_tile, int d, bf16* __restrict__ dw_up, bf16* __restrict__ dw_down) {
   pdl_launch_dependents();
   pdl_wait();
-  const int tile = blockIdx.x, ntn = d / 256;
+  const int tile = first_tile + blockIdx.x, ntn = d / 256;
   const int slot = tile / (2 * ntn), rem = tile % (2 * ntn), job = rem / ntn, n0 = (rem % ntn) * 256;
   for (int e = blockIdx.y * 16 * 256 + threadIdx.x * 4; e < (blockIdx.y + 1) * 16 * 256; e += 256 * 4) {
     const int r = e >> 8, c = e & 255;
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
     for (int j = 0; j < ks; ++j) {
-      const float4 v = *reinterpret_cast<const float4*>(part + (((size_t)tile * ks + j) * GT + r) * 256 + c);
+      const float4 v = *reinterpret_cast<const float4*>(part + (((size_t)blockIdx.x * ks + j) * GT + r) * 256 + c);
       acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
     }
     uint2 o;
@@ -595,7 +601,7 @@ GParams base_params(const fomoe_config& c, int n_res, const RouteWs& rws) {
   GParams p{};
   p.n_mtiles = rws.n_mtiles; p.tile_slot = rws.tile_slot; p.pair_info = rws.pair_info; p.pad_offsets = rws.pad_offsets;
   p.pad_end64 = rws.pad_end64; p.prow_token = rws.prow_token; p.prow_gate = rws.prow_gate;
-  p.d = c.d_model; p.n_res = n_res; p.ks = 1;
+  p.d = c.d_model; p.n_res = n_res; p.ks = 1; p.wg_full = 0;
   return p;
 }
 
@@ -650,15 +656,20 @@ int fine_wgrad(const fomoe_config& c, int n_res, const void* x, const void* dy, 
   MAP_OK(make_map_box(&m.m[3], dw_down, GT, (uint64_t)n_res * c.d_model, GT, 32, 32, CU_TENSOR_MAP_SWIZZLE_64B));
   GParams p = base_params(c, n_res, rws);
   p.g0 = (const bf16*)x; p.g1 = (const bf16*)dy;
-  // few tiles (P1: 32): cut K so that the items fill the SMs; the partials live where the scaled copy of dy would (unused here)
-  const int tiles = n_res * 2 * (c.d_model / 256);
-  int ks = num_sms() / tiles;
+  // tiles that do not fill the SMs once (P1: 32): cut K so that the items do; the partials live where the scaled copy of dy
+  // would (unused on this path).  The kernel can split the last round of a longer schedule too (wg_full > 0; P3: 68 of 512
+  // tiles, kernel 176 -> 162 us) but the step does not get faster: the router's backward chain on the side stream runs on
+  // the SMs that round leaves idle, so only the single-round case is split.
+  const int tiles = n_res * 2 * (c.d_model / 256), grid = num_sms();
+  const int full = tiles / grid * grid, tail = tiles - full;
+  int ks = (tail > 0 && (full == 0 || getenv("FOMOE_FINE_TAILSPLIT"))) ? grid / tail : 1;
   if (ks > 8) ks = 8;
-  while (ks > 1 && (size_t)tiles * ks * GT * 256 * sizeof(float) > sizeof(bf16) * (size_t)R * c.d_model) --ks;
+  while (ks > 1 && (size_t)tail * ks * GT * 256 * sizeof(float) > sizeof(bf16) * (size_t)R * c.d_model) --ks;
+  p.wg_full = ks > 1 ? full : tiles;
   if (ks > 1) { p.ks = ks; p.part = (float*)sws.dop; }
   int rc = g_launch<G_WG>(m, p, st, "fine_gather_kernel<WG>");
   if (rc != FOMOE_OK || ks <= 1) return rc;
-  FOMOE_CUDA_OK(launch_pdl(fine_wg_reduce_kernel, dim3(tiles, 8), 256, 0, st, (const float*)p.part, ks, c.d_model, (bf16*)dw_up, (bf16*)dw_down));
+  FOMOE_CUDA_OK(launch_pdl(fine_wg_reduce_kernel, dim3(tail, 8), 256, 0, st, (const float*)p.part, ks, full, c.d_model, (bf16*)dw_up, (bf16*)dw_down));
   FOMOE_LAUNCH_OK("fine_wg_reduce_kernel");
   return FOMOE_OK;
 }

@@ -49,6 +49,7 @@ def test_fine_path_is_the_one_that_runs():
     dict(T=700, n_res=16),                             # every expert resident
     dict(T=1500, n_sh=1, F_sh=192, n_res=7),           # a shared expert beside the gathered routed path
     dict(T=640, d=1024, E=32, k=8, n_res=16, seed=12), # 16 x 2 x 4 = 128 weight-gradient tiles: one K part
+    dict(T=500, d=1024, E=32, k=8, n_res=20, seed=14), # 160 tiles on 148 SMs: one full round stored directly, 12 tail tiles in 8 K parts
     dict(T=600, d=512, gate_fn=W.GATE_SOFTMAX, gate_rule=W.RULE_RENORM_RESIDENT),
 ], ids=lambda kw: "-".join(f"{k}{v}" for k, v in kw.items()) or "base")
 def test_fine_full_parity(oracle64, kw):
