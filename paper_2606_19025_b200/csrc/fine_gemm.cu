@@ -144,6 +144,25 @@ struct GItem {
   long pidx;     // WG split-K: index of this item's partial tile in GParams::part, -1 = a whole tile (stored as bf16)
 };
 
+// WG tile numbering (shared with fine_wg_reduce_kernel).  d <= 1024: column block outermost -- neighbouring tiles gather the
+// same 256 columns of x / dy for different slots (P2: 62 -> 55 us, P1: 28 -> 27 us).  Wider rows: slot outermost, so that the
+// tiles in flight cover whole rows; with the column block outermost every CTA would read the same 512-byte stripe of 4 KB
+// rows at once and the kernel slows down although its DRAM traffic drops (P3: 169 -> 196 us, measured).
+__device__ __forceinline__ void wg_tile(long id, int n_res, int d, int& slot, int& job, int& n0) {
+  const int ntn = d / 256;
+  if (ntn <= 4) {
+    n0 = (int)(id / (2 * n_res)) * 256;
+    const int rem = (int)(id % (2 * n_res));
+    slot = rem >> 1;
+    job = rem & 1;
+  } else {
+    slot = (int)(id / (2 * ntn));
+    const int rem = (int)(id % (2 * ntn));
+    job = rem / ntn;
+    n0 = (rem % ntn) * 256;
+  }
+}
+
 template <int MODE>
 struct GSched {
   const GParams& p;
@@ -163,7 +182,6 @@ struct GSched {
     GItem it;
     it.job = 0; it.n0 = 0;
     if (MODE == G_WG) {
-      const int ntn = p.d / 256;
       it.pidx = -1;
       int kpart = 0;
       if (id >= full) {
@@ -171,10 +189,7 @@ struct GSched {
         kpart = (int)(it.pidx % p.ks);
         id = full + it.pidx / p.ks;
       }
-      it.slot = (int)(id / (2 * ntn));
-      const int rem = (int)(id % (2 * ntn));
-      it.job = rem / ntn;
-      it.n0 = (rem % ntn) * 256;
+      wg_tile(id, p.n_res, p.d, it.slot, it.job, it.n0);
       it.row0 = p.pad_offsets[it.slot];
       it.num_kb = (p.pad_end64[it.slot] - it.row0 + GK - 1) / GK;
       if (it.pidx >= 0 && p.ks > 1) {   // this part's K blocks
@@ -564,11 +579,11 @@ fine_gather_kernel(const __grid_constant__ GMaps maps, const __grid_constant__ G
 
 // adds the ks partials of every split WG tile in a fixed order and writes dW_up / dW_down as bf16.  grid = (split tiles, 8 row slabs)
 __global__ void __launch_bounds__(256)
-fine_wg_reduce_kernel(const float* __restrict__ part, int ks, int first_tile, int d, bf16* __restrict__ dw_up, bf16* __restrict__ dw_down) {
+fine_wg_reduce_kernel(const float* __restrict__ part, int ks, int first_tile, int n_res, int d, bf16* __restrict__ dw_up, bf16* __restrict__ dw_down) {
   pdl_launch_dependents();
   pdl_wait();
-  const int tile = first_tile + blockIdx.x, ntn = d / 256;
-  const int slot = tile / (2 * ntn), rem = tile % (2 * ntn), job = rem / ntn, n0 = (rem % ntn) * 256;
+  int slot, job, n0;
+  wg_tile(first_tile + blockIdx.x, n_res, d, slot, job, n0);
   for (int e = blockIdx.y * 16 * 256 + threadIdx.x * 4; e < (blockIdx.y + 1) * 16 * 256; e += 256 * 4) {
     const int r = e >> 8, c = e & 255;
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -669,7 +684,7 @@ int fine_wgrad(const fomoe_config& c, int n_res, const void* x, const void* dy, 
   if (ks > 1) { p.ks = ks; p.part = (float*)sws.dop; }
   int rc = g_launch<G_WG>(m, p, st, "fine_gather_kernel<WG>");
   if (rc != FOMOE_OK || ks <= 1) return rc;
-  FOMOE_CUDA_OK(launch_pdl(fine_wg_reduce_kernel, dim3(tail, 8), 256, 0, st, (const float*)p.part, ks, full, c.d_model, (bf16*)dw_up, (bf16*)dw_down));
+  FOMOE_CUDA_OK(launch_pdl(fine_wg_reduce_kernel, dim3(tail, 8), 256, 0, st, (const float*)p.part, ks, full, n_res, c.d_model, (bf16*)dw_up, (bf16*)dw_down));
   FOMOE_LAUNCH_OK("fine_wg_reduce_kernel");
   return FOMOE_OK;
 }
