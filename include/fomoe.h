@@ -212,6 +212,23 @@ FOMOE_API int fomoe_periln_bwd(int32_t T, int32_t d_model, int32_t dtype, const 
                      void* stream);
 
 /*
+ * fomoe_periln_bwd without a caller-owned workspace, for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid allocation): the per-CTA dgamma / dbeta partial sums live in a static device
+ * array of fomoe_periln_bwd_noalloc_max_floats() = 4 Mi floats (16 MiB), which every GPU that loads the library holds until
+ * the process exits.  Same arguments (all device pointers, caller-owned), same kernels and the same fixed-order reduction as
+ * fomoe_periln_bwd: bit-identical results.  The call allocates nothing (no cudaMalloc / cudaFree / allocating library
+ * routine); its only set-up is one cudaGetSymbolAddress per device.
+ *   Limit: 2 * min(T, 8 * SM count) * d_model <= 4 Mi (on a 148-SM B200: every T up to d_model = 1771, wider rows only for
+ *   fewer tokens).  Beyond it: FOMOE_ERR_UNSUPPORTED, text via fomoe_last_cuda_error(); use fomoe_periln_bwd then.
+ *   Sharing: every call on a device uses the same array.  Calls on ONE stream are ordered and safe; calls that overlap on the
+ *   GPU (several streams, concurrent graph launches) race on it.  Nothing in it needs clearing between calls (each call
+ *   overwrites what it later reads).
+ */
+FOMOE_API size_t fomoe_periln_bwd_noalloc_max_floats(void);
+FOMOE_API int fomoe_periln_bwd_noalloc(int32_t T, int32_t d_model, int32_t dtype, const void* dout, const void* x, const float* stats,
+                     const float* gamma, float alpha, const void* dresidual, void* dx, float* dgamma, float* dbeta, void* stream);
+
+/*
  * The same block with the LayerNorms FUSED into the layer's own row kernels ("post-LN + depth multiplier +
  * residual fused into combine"; Eq. 15, 601):
  *   fomoe_moe_fwd_periln = fomoe_moe_fwd, whose combine also writes  out = residual + alpha LN(y)  and stats (y is still written: the

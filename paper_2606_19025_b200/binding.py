@@ -28,7 +28,8 @@ EXPORTS = ("fomoe_workspace_bytes", "fomoe_route", "fomoe_moe_fwd", "fomoe_moe_b
            "fomoe_adamw_resident", "fomoe_outer_nesterov", "fomoe_periln_workspace_bytes", "fomoe_periln_fwd", "fomoe_periln_bwd",
            "fomoe_moe_step_host", "fomoe_moe_step_host_join", "fomoe_last_launch_count", "fomoe_last_cuda_error", "fomoe_abi_version",
            "fomoe_set_force_simt", "fomoe_profile_enable", "fomoe_profile_collect", "fomoe_debug_validate_resident",
-           "fomoe_routing_stats", "fomoe_moe_fwd_periln", "fomoe_moe_bwd_periln")
+           "fomoe_routing_stats", "fomoe_moe_fwd_periln", "fomoe_moe_bwd_periln", "fomoe_periln_bwd_noalloc",
+           "fomoe_periln_bwd_noalloc_max_floats")
 STAT_NAMES = ("kept_fraction", "ghost_fraction", "zero_kept_tokens", "load_cv", "routing_entropy", "max_load", "min_load")
 
 
@@ -70,6 +71,7 @@ def lib() -> C.CDLL:
         for name in EXPORTS:
             getattr(_lib, name).restype = C.c_int
         _lib.fomoe_last_cuda_error.restype = C.c_char_p
+        _lib.fomoe_periln_bwd_noalloc_max_floats.restype = C.c_size_t
         if _lib.fomoe_abi_version() != 5:
             raise FomoeError("libfomoe.so ABI version mismatch")
     return _lib
@@ -223,6 +225,18 @@ def fomoe_periln_bwd(dout, x, stats, gamma, dx, dgamma, dbeta, partials, dresidu
     T, d = x.shape
     _check(lib().fomoe_periln_bwd(C.c_int32(T), C.c_int32(d), C.c_int32(_dt(x)), _p(dout), _p(x), _p(stats), _p(gamma), C.c_float(alpha),
                                   _p(dresidual), _p(dx), _p(dgamma), _p(dbeta), _p(partials), _stream(stream)), "fomoe_periln_bwd")
+
+
+def fomoe_periln_bwd_noalloc(dout, x, stats, gamma, dx, dgamma, dbeta, dresidual=None, alpha=1.0, stream=None) -> None:
+    """fomoe_periln_bwd with its partial-sum workspace in the library's static device array (no allocation anywhere)."""
+    T, d = x.shape
+    _check(lib().fomoe_periln_bwd_noalloc(C.c_int32(T), C.c_int32(d), C.c_int32(_dt(x)), _p(dout), _p(x), _p(stats), _p(gamma),
+                                          C.c_float(alpha), _p(dresidual), _p(dx), _p(dgamma), _p(dbeta), _stream(stream)),
+           "fomoe_periln_bwd_noalloc")
+
+
+def fomoe_periln_bwd_noalloc_max_floats() -> int:
+    return int(lib().fomoe_periln_bwd_noalloc_max_floats())
 
 
 def _arr3(ts):

@@ -37,6 +37,12 @@ int set_cuda_error(cudaError_t e, const char* where) {
   snprintf(g_err, sizeof(g_err), "%s: %s (%s)", where, cudaGetErrorName(e), cudaGetErrorString(e));
   return FOMOE_ERR_CUDA;
 }
+// for entry points that live in another translation unit (fomoe_periln_bwd_noalloc, periln.cu)
+int set_error_text(int code, const char* text) {
+  snprintf(g_err, sizeof(g_err), "%s", text);
+  return code;
+}
+void reset_launch_count() { g_launches = 0; }
 
 // The one piece of state the library owns: a side stream and two events per host thread, used by fomoe_moe_bwd to run the
 // router's backward chain (gate_bwd, dz W_r^T, x^T dz) beside the expert GEMMs.  Fork / join through events, so the pattern

@@ -19,6 +19,8 @@ constexpr int kMaxK = 32;
 void note_launch(const char* name, cudaStream_t st);   // counts the launch; records a profiling event when enabled
 void note_api_entry(const char* name, cudaStream_t st);  // profiling marker at the start of an entry point
 int set_cuda_error(cudaError_t e, const char* where);
+int set_error_text(int code, const char* text);   // returns `code`; the text is what fomoe_last_cuda_error() then reports
+void reset_launch_count();
 #define FOMOE_CUDA_OK(expr)                                          \
   do {                                                               \
     cudaError_t e__ = (expr);                                        \

@@ -6,6 +6,7 @@
 // The row is staged once in shared memory (fp32), so mean and the centred variance are computed exactly as LayerNorm
 // defines them and global memory is read once.  Bound: HBM.
 #include "common.cuh"
+#include <stdio.h>
 #include <stdlib.h>
 
 namespace fomoe {
@@ -753,3 +754,60 @@ int launch_dx_sum_periln(const fomoe_config& c, const RouteWs& ws, const void* d
 }
 
 }  // namespace fomoe
+
+// ---------------------------------------------------------------------------------------------------------
+// Allocation-free Peri-LN backward: fomoe_periln_bwd with its `partials` workspace in a static device array.
+//
+// For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it) and
+// so cannot provide fomoe_periln_workspace_bytes() bytes of scratch: the per-CTA dgamma / dbeta partial sums live in the
+// array below, 16 MiB that every GPU which loads libfomoe.so holds until the process exits.  Same kernels, same grid and
+// same fixed-order reduction as fomoe_periln_bwd: the results are bit-identical to it.
+//   * limit: 2 * periln_blocks(T) * d_model <= kNoAllocFloats (periln_blocks = min(T, 8 * SMs): on a 148-SM B200 any T up
+//     to d_model = 1771; larger rows only for fewer tokens); beyond it FOMOE_ERR_UNSUPPORTED with a text in fomoe_last_cuda_error().
+//   * every call on a device shares the array: calls that overlap on the GPU (different streams, or concurrent graphs) RACE.
+//     Calls on one stream are ordered and safe.  Nothing in it has to start at zero -- every CTA of the backward kernel
+//     overwrites its own 2 * d_model partials before the reduce kernel reads them -- so the previous call's contents are
+//     simply overwritten and no clearing pass is needed.
+//   * no cudaMalloc / cudaFree / allocating library call: the only set-up is cudaGetSymbolAddress, once per device.
+// In HOST code the array's name is a host-side stand-in for the symbol, not a device address: the kernels get the pointer
+// cudaGetSymbolAddress returns for the CURRENT device.
+// ---------------------------------------------------------------------------------------------------------
+constexpr size_t kNoAllocFloats = (size_t)4 << 20;   // 4 Mi floats = 16 MiB
+static __device__ __align__(256) float g_periln_noalloc_scratch[kNoAllocFloats];
+
+static float* periln_noalloc_scratch_ptr(cudaError_t* err) {
+  static float* addr[fomoe::kMaxDev] = {};   // per device; racing host threads write the same value
+  const int dev = fomoe::current_device();
+  *err = cudaSuccess;
+  if (!addr[dev]) {
+    float* ptr = nullptr;
+    *err = cudaGetSymbolAddress((void**)&ptr, g_periln_noalloc_scratch);   // resolves the symbol on the current device
+    if (*err != cudaSuccess) return nullptr;
+    addr[dev] = ptr;
+  }
+  return addr[dev];
+}
+
+extern "C" FOMOE_API size_t fomoe_periln_bwd_noalloc_max_floats(void) { return kNoAllocFloats; }
+
+extern "C" FOMOE_API int fomoe_periln_bwd_noalloc(int32_t T, int32_t d_model, int32_t dtype, const void* dout, const void* x, const float* stats,
+                                                  const float* gamma, float alpha, const void* dresidual, void* dx, float* dgamma,
+                                                  float* dbeta, void* stream) {
+  using namespace fomoe;
+  reset_launch_count();
+  if (T < 0 || d_model <= 0 || (dtype != FOMOE_F32 && dtype != FOMOE_BF16) || !gamma || !dgamma || !dbeta) return FOMOE_ERR_BADARG;
+  if (T > 0 && (!dout || !x || !stats || !dx)) return FOMOE_ERR_BADARG;
+  if ((size_t)d_model * 16 > 200 * 1024) return FOMOE_ERR_UNSUPPORTED;
+  const size_t need = 2 * (size_t)periln_blocks(T) * (size_t)d_model;
+  if (need > kNoAllocFloats) {
+    char msg[256];
+    snprintf(msg, sizeof(msg), "fomoe_periln_bwd_noalloc: T = %d, d_model = %d needs %zu floats of scratch, the static array holds %zu "
+             "(use fomoe_periln_bwd with a caller-owned workspace)", (int)T, (int)d_model, need, kNoAllocFloats);
+    return set_error_text(FOMOE_ERR_UNSUPPORTED, msg);
+  }
+  cudaError_t e;
+  float* partials = periln_noalloc_scratch_ptr(&e);
+  if (!partials) return set_cuda_error(e, "cudaGetSymbolAddress(g_periln_noalloc_scratch)");
+  note_api_entry("@fomoe_periln_bwd_noalloc", (cudaStream_t)stream);
+  return launch_periln_bwd(T, d_model, dtype, dout, x, stats, gamma, alpha, dresidual, dx, dgamma, dbeta, partials, (cudaStream_t)stream);
+}
