@@ -12,6 +12,7 @@ N > 1: one process per GPU (torchrun), independent replicas, no collective on th
 from __future__ import annotations
 
 import argparse
+import dataclasses
 import json
 import os
 import statistics
@@ -380,8 +381,24 @@ def run_gpu(args, w, n_res):
                     k["l2_operand_bytes"] = ob
                     k["l2_gbs"] = ob / (tt / n / 1e3) / 1e9
                     k["l2_frac_of_6300B_per_clk"] = k["l2_gbs"] / (6300 * (clocks.get("sm_mhz") or 1965.0) * 1e6 / 1e9)
+                if name in ("umma_grouped_kernel<FWD2>", "umma_grouped_kernel<DX>"):
+                    # with narrow experts these two are write streams of their [P, d] output, not contractions: report that rate
+                    # too (compare with hbm_write_probe below: what a plain memset reaches on this GPU)
+                    k["out_write_gbs"] = P * w.d * 2 / (tt / n / 1e3) / 1e9
             kernels.append(k)
         out["kernels"] = kernels
+        # a pure-write stream for comparison: cudaMemset of the 512 MiB flush buffer, timed live
+        for _ in range(3):
+            flush.zero_()
+        torch.cuda.synchronize()
+        w0, w1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        w0.record()
+        for _ in range(5):
+            flush.zero_()
+        w1.record()
+        torch.cuda.synchronize()
+        out["hbm_write_probe"] = {"memset_gbs": 5 * flush.numel() / (w0.elapsed_time(w1) / 1e3) / 1e9, "bytes": flush.numel(),
+                                  "note": "pure-write rate of cudaMemset; the copy peak in MEASURED_PEAKS.json is read + write"}
         # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed `ncu --set full` capture of
         # THIS revision's kernels (profiles/r2_traffic.md names the command); keyed by workload and by the name the library emits
         traffic_rows = {}
@@ -612,6 +629,7 @@ def main():
     ap.add_argument("--workload", default="C5", choices=sorted(W.CONFIGS),
                     help="C5 (BASELINE.json configs[4]) is the largest single-GPU configuration: the headline")
     ap.add_argument("--n-res", type=int, default=None)
+    ap.add_argument("--tokens", type=int, default=None, help="override the workload's token count T (scaling experiments)")
     ap.add_argument("--ref-tokens", type=int, default=16384, help="upper bound on the tokens per step of the CPU oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-all-resident", action="store_true")
@@ -625,6 +643,8 @@ def main():
                "--master-port", str(29500 + os.getpid() % 2000), str(Path(__file__).resolve()), *sys.argv[1:]]
         raise SystemExit(subprocess.call(cmd))
     w = W.config(args.workload)
+    if args.tokens is not None:
+        w = dataclasses.replace(w, T=args.tokens, name=f"{w.name}@T={args.tokens}")
     n_res = w.n_res if args.n_res is None else args.n_res
     if args.impl == "reference":
         run_reference(args, w, n_res)
