@@ -45,13 +45,23 @@ constexpr int kEpiWarps = 8;    // two warps per TMEM lane quarter; they take al
 constexpr int kStgTile = 2048;
 constexpr int kDhDepth = 3;  // DH epilogue: chunks of (a, u) kept in flight per warp with cp.async
 enum Mode { FWD1 = 0, FWD2 = 1, DH = 2, DX = 3, WGRAD = 4, ROUTE = 5, FWD1S = 6 };
-constexpr int kRouteStg = 57344;  // ROUTE epilogue scratch: slot map, per-stage histograms, top-k candidate / merge lists (k <= 32)
+// ROUTE epilogue scratch (struct RouteSmem<KMAX> below): slot map, per-stage histograms, top-k candidate / merge lists.  Its size
+// follows the list capacity, so that the short lists (k <= 8: 30 KB) leave room for a sixth TMA stage.
+__host__ __device__ constexpr int route_stg_bytes(int kmax) {
+  const int kn = kmax > 16 ? 16 : (kmax < 2 ? 2 : kmax);
+  const int net = kn * 128 * 8 + (kn + 1) * 256 * 8, ins = kmax > 16 ? 2 * kmax * 128 * 4 : 0;
+  return (4096 + (net > ins ? net : ins) + 1023) / 1024 * 1024;
+}
 // DH and FWD1 trade TMA stages for epilogue staging: DH streams a and u back in through a cp.async ring
-__host__ __device__ constexpr int stages_of(int mode) { return mode == DH ? 4 : (mode == FWD1 || mode == FWD1S || mode == ROUTE) ? 5 : 6; }
+__host__ __device__ constexpr int stages_of(int mode, int kmax = 0) {
+  return mode == DH ? 4 : mode == ROUTE ? (route_stg_bytes(kmax) <= 32768 ? 6 : 5) : (mode == FWD1 || mode == FWD1S) ? 5 : 6;
+}
 __host__ __device__ constexpr int stg_tiles_per_warp(int mode) { return mode == DH ? 2 * kDhDepth : mode == FWD1 ? 3 : 2; }   // FWD2 / DX: two tiles, alternating under the bulk stores
-__host__ __device__ constexpr int stg_bytes_of(int mode) { return mode == ROUTE ? kRouteStg : kEpiWarps * stg_tiles_per_warp(mode) * kStgTile; }
-__host__ __device__ constexpr int smem_bytes_of(int mode) {
-  return stages_of(mode) * kStageBytes + stg_bytes_of(mode) + 1024 /*align*/ + 256 /*barriers*/;
+__host__ __device__ constexpr int stg_bytes_of(int mode, int kmax = 0) {
+  return mode == ROUTE ? route_stg_bytes(kmax) : kEpiWarps * stg_tiles_per_warp(mode) * kStgTile;
+}
+__host__ __device__ constexpr int smem_bytes_of(int mode, int kmax = 0) {
+  return stages_of(mode, kmax) * kStageBytes + stg_bytes_of(mode, kmax) + 1024 /*align*/ + 256 /*barriers*/;
 }
 constexpr int kTmemCols = 512;
 
@@ -307,7 +317,10 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16]) {
 __device__ __forceinline__ void bar_sync_named(int id, int threads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory"); }
 
 constexpr int kNetK = 16;     // largest top-k list the sorting-network epilogue handles (k <= 16); k = 17..32 takes the insertion epilogue
-struct RouteSmem {            // lives in the kernel's staging area (kRouteStg bytes)
+template <int KMAX>
+struct RouteSmem {            // lives in the kernel's staging area (route_stg_bytes(KMAX) bytes)
+  static constexpr int KN = KMAX > kNetK ? kNetK : (KMAX < 2 ? 2 : KMAX);   // capacity of the sorting-network lists
+  static constexpr int KI = KMAX > kNetK ? KMAX : 1;                          // capacity of the insertion lists
   int32_t slot[128];          // resident slot of expert e, -1 = ghost
   float zb[128];              // additive logit term of expert e: router bias (or 0); -inf = no such column (e >= E, or a ghost
                               // expert under forced-local routing)
@@ -316,16 +329,19 @@ struct RouteSmem {            // lives in the kernel's staging area (kRouteStg b
   float sum[2][128];          // partial softmax denominators
   union {
     struct {                  // insertion epilogue (k > kNetK)
-      float lv[kMaxK][128];   // half 1 -> half 0: top-k values / ids of row r
-      int32_t li[kMaxK][128];
+      float lv[KI][128];      // half 1 -> half 0: top-k values / ids of row r
+      int32_t li[KI][128];
     } ins;
     struct {                  // sorting-network epilogue
-      uint2 hand[kNetK][128];          // half 1 -> half 0: sorted (value, id) list of row r
-      uint2 cand[kNetK + 1][256];      // per-thread candidate lists (thread-private), written in id order
+      uint2 hand[KN][128];             // half 1 -> half 0: sorted (value, id) list of row r
+      uint2 cand[KN + 1][256];         // per-thread candidate lists (thread-private), written in id order
     } net;
   };
 };
-static_assert(sizeof(RouteSmem) <= kRouteStg, "route epilogue scratch");
+static_assert(sizeof(RouteSmem<2>) <= route_stg_bytes(2) && sizeof(RouteSmem<4>) <= route_stg_bytes(4) &&
+              sizeof(RouteSmem<8>) <= route_stg_bytes(8) && sizeof(RouteSmem<16>) <= route_stg_bytes(16) &&
+              sizeof(RouteSmem<32>) <= route_stg_bytes(32), "route epilogue scratch");
+static_assert(smem_bytes_of(ROUTE, 8) <= 227 * 1024 && smem_bytes_of(ROUTE, 16) <= 227 * 1024 && smem_bytes_of(ROUTE, 32) <= 227 * 1024, "shared memory");
 
 // ---- sorting networks on registers (all indices are compile-time: nothing spills) ----
 // Descending bitonic networks.  Values only: a compare-exchange is one FMNMX pair; a NaN operand is dropped by fmaxf / fminf
@@ -399,7 +415,7 @@ __device__ __forceinline__ void stg256(float* p, const float* v) {   // 32-byte 
 //      then the <= KMAX candidates are sorted with their ids and the two halves' lists merged by half 0;
 //   C. probabilities.
 template <int KMAX>
-__device__ __forceinline__ void route_tile_epilogue_net(const UmmaParams& p, RouteSmem* rs, uint32_t taddr, int q, int half, int lane, int as,
+__device__ __forceinline__ void route_tile_epilogue_net(const UmmaParams& p, RouteSmem<KMAX>* rs, uint32_t taddr, int q, int half, int lane, int as,
                                                         int row0, bool live) {
   const RouteEpi& r = p.r;
   const int E = r.E, Epad = r.Epad;
@@ -576,7 +592,7 @@ __device__ __forceinline__ void route_tile_epilogue_net(const UmmaParams& p, Rou
 }
 
 template <int KMAX>
-__device__ __forceinline__ void route_tile_epilogue(const UmmaParams& p, RouteSmem* rs, uint32_t taddr, int q, int half, int lane, int as,
+__device__ __forceinline__ void route_tile_epilogue(const UmmaParams& p, RouteSmem<KMAX>* rs, uint32_t taddr, int q, int half, int lane, int as,
                                                     int row0, bool live) {
   const RouteEpi& r = p.r;
   const int E = r.E, Epad = r.Epad;
@@ -751,10 +767,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant__ UmmaParams p) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-  constexpr int kStages = stages_of(MODE);
+  constexpr int kStages = stages_of(MODE, KMAX);
   constexpr int kStgTilesPerWarp = stg_tiles_per_warp(MODE);
   uint8_t* stg_base = smem + kStages * kStageBytes;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(stg_base + stg_bytes_of(MODE));
+  uint64_t* bars = reinterpret_cast<uint64_t*>(stg_base + stg_bytes_of(MODE, KMAX));
   uint64_t* full_bar = bars;                          // [kStages]   used in the leader CTA only
   uint64_t* empty_bar = bars + kStages;               // [kStages]   one per CTA, released by the leader's commits
   uint64_t* tfull_bar = bars + 2 * kStages;           // [kAccStages] one per CTA
@@ -896,7 +912,8 @@ umma_grouped_kernel(const __grid_constant__ TmaMaps maps, const __grid_constant_
     const uint32_t stg0 = smem_u32(stg_base) + (uint32_t)((warp - 4) * (kStgTilesPerWarp * kStgTile));
     const uint32_t tempty_leader = smem_u32(&tempty_bar[0]) & 0xFEFFFFFFu;  // the pair leader's barrier (peer bit cleared); + 8 * stage
     if (MODE == ROUTE) {
-      RouteSmem* rs = reinterpret_cast<RouteSmem*>(stg_base);
+      constexpr int KE = KMAX > 0 ? KMAX : 2;
+      RouteSmem<KE>* rs = reinterpret_cast<RouteSmem<KE>*>(stg_base);
       {  // slot map and cleared histograms, visible to all epilogue warps before the first tile
         const int tid = threadIdx.x - 128;
         for (int i = tid; i < 128; i += kEpiWarps * 32) {
@@ -1236,10 +1253,10 @@ template <int MODE, int KMAX = 0>
 int launch(const TmaMaps& maps, const UmmaParams& p, cudaStream_t st, const char* name) {
   static PerDeviceOnce attr;
   if (attr.need()) {
-    FOMOE_CUDA_OK(cudaFuncSetAttribute(umma_grouped_kernel<MODE, KMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes_of(MODE)));
+    FOMOE_CUDA_OK(cudaFuncSetAttribute(umma_grouped_kernel<MODE, KMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes_of(MODE, KMAX)));
     attr.set();
   }
-  FOMOE_CUDA_OK(launch_pdl(umma_grouped_kernel<MODE, KMAX>, num_sms() & ~1, kThreads, smem_bytes_of(MODE), st, maps, p));
+  FOMOE_CUDA_OK(launch_pdl(umma_grouped_kernel<MODE, KMAX>, num_sms() & ~1, kThreads, smem_bytes_of(MODE, KMAX), st, maps, p));
   FOMOE_LAUNCH_OK(name);
   return FOMOE_OK;
 }
