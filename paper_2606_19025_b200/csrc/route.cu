@@ -194,19 +194,33 @@ perm_scan_scatter_kernel(const int32_t* __restrict__ topk_idx, const float* __re
   int32_t* warp_cnt = sm + n_res;        // [8][n_res]
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   constexpr int n_warps = kPermThreads / 32;
-  // (a) this block's exclusive base and the total of every slot
-  for (int s = warp; s < n_res; s += n_warps) {
-    int base = 0, tot = 0;
-    for (int b = lane; b < n_blk; b += 32) {
-      const int c = blk_hist[(size_t)b * n_res + s];
-      tot += c;
-      if (b < (int)blockIdx.x) base += c;
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) { base += __shfl_xor_sync(0xffffffffu, base, o); tot += __shfl_xor_sync(0xffffffffu, tot, o); }
-    if (lane == 0) { running[s] = base; s_cnt[s] = tot; }
-  }
+  // (a) this block's exclusive base and the total of every slot.  The [n_blk, n_res] histogram is walked in memory order
+  // (consecutive threads read consecutive words: every block reads all of it, so at T = 131072 the slot-per-warp walk with
+  // its n_res-word stride took 198 us; this one 1/10 of that); integer adds, so the result does not depend on their order
+  for (int i = threadIdx.x; i < n_res; i += kPermThreads) { running[i] = 0; s_cnt[i] = 0; }
   for (int i = threadIdx.x; i < 8 * n_res; i += kPermThreads) warp_cnt[i] = 0;
+  __syncthreads();
+  {
+    const long n_hist = (long)n_blk * n_res, n_before = (long)blockIdx.x * n_res;
+    if (kPermThreads % n_res == 0) {      // a thread meets one slot only: sums in registers, one shared-memory add at the end
+      int base = 0, tot = 0;
+      for (long i = threadIdx.x; i < n_hist; i += kPermThreads) {
+        const int c = blk_hist[i];
+        tot += c;
+        if (i < n_before) base += c;
+      }
+      atomicAdd(&running[threadIdx.x % n_res], base);
+      atomicAdd(&s_cnt[threadIdx.x % n_res], tot);
+    } else {
+      for (long i = threadIdx.x; i < n_hist; i += kPermThreads) {
+        const int c = blk_hist[i];
+        if (c == 0) continue;
+        const int sidx = (int)(i % n_res);
+        atomicAdd(&s_cnt[sidx], c);
+        if (i < n_before) atomicAdd(&running[sidx], c);
+      }
+    }
+  }
   __syncthreads();
   // (b) exclusive scans over the slots (warp 0): row offsets, tile-padded offsets, tile pairs
   if (warp == 0) {
