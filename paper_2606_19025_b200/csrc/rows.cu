@@ -71,11 +71,13 @@ gather_rows_kernel(const T* __restrict__ x, const int32_t* __restrict__ prow_tok
 template <typename T, int V>
 __global__ void __launch_bounds__(kRowThreads)
 combine_kernel(const T* __restrict__ o, const T* __restrict__ y_sh, const float* __restrict__ gate,
-               const int32_t* __restrict__ pair_prow, int T_, int d, int k, T* __restrict__ y) {
+               const int32_t* __restrict__ pair_prow, int T_, int d, int k, int rpb, T* __restrict__ y) {
   pdl_launch_dependents();
   pdl_wait();
-  for (int t = blockIdx.x; t < T_; t += gridDim.x) {
-    for (int c = threadIdx.x * V; c < d; c += kRowThreads * V) {
+  // rpb token rows per CTA (narrow rows: d / V < kRowThreads would leave threads idle), kRowThreads / rpb threads each
+  const int tpr = kRowThreads / rpb, sub = threadIdx.x / tpr, c0 = (threadIdx.x % tpr) * V;
+  for (int t = blockIdx.x * rpb + sub; t < T_; t += gridDim.x * rpb) {
+    for (int c = c0; c < d; c += tpr * V) {
       Vec<T, V> acc;
       if (y_sh) acc.load(y_sh + (size_t)t * d + c); else acc.zero();
       for (int j = 0; j < k; ++j) {
@@ -222,11 +224,12 @@ __global__ void gate_bwd_kernel(const float* __restrict__ probs, const int32_t* 
 template <typename T, int V>
 __global__ void __launch_bounds__(kRowThreads)
 dx_sum_kernel(const T* __restrict__ dxp, const T* __restrict__ dx_sh, const float* __restrict__ dx_r, const T* __restrict__ dx_r_t,
-              const int32_t* __restrict__ pair_prow, int T_, int d, int k, T* __restrict__ dx) {
+              const int32_t* __restrict__ pair_prow, int T_, int d, int k, int rpb, T* __restrict__ dx) {
   pdl_launch_dependents();
   pdl_wait();
-  for (int t = blockIdx.x; t < T_; t += gridDim.x) {
-    for (int c = threadIdx.x * V; c < d; c += kRowThreads * V) {
+  const int tpr = kRowThreads / rpb, sub = threadIdx.x / tpr, c0 = (threadIdx.x % tpr) * V;   // (as in combine_kernel)
+  for (int t = blockIdx.x * rpb + sub; t < T_; t += gridDim.x * rpb) {
+    for (int c = c0; c < d; c += tpr * V) {
       Vec<T, V> acc;
       if (dx_sh) acc.load(dx_sh + (size_t)t * d + c); else acc.zero();
       for (int j = 0; j < k; ++j) {
@@ -252,6 +255,15 @@ dx_sum_kernel(const T* __restrict__ dxp, const T* __restrict__ dx_sh, const floa
   }
 }
 
+// token rows per CTA of combine / dx_sum: the largest power of two (<= 8) whose rows' vector chunks fit the CTA's threads
+// (d = 512 bf16: 64 chunks -> 2 rows; on P1 dx_sum 25 -> 20 us, combine 16 -> 14 us); 1 once d / V > kRowThreads / 2
+static int rows_per_block(int d, int V) {
+  const int n = (d + V - 1) / V;
+  int r = 1;
+  while (r < 8 && n * r * 2 <= kRowThreads) r *= 2;
+  return r;
+}
+
 // dispatch on dtype and on whether rows are 16-byte vectorisable
 #define ROWS_DISPATCH(c, CALL)                                              \
   do {                                                                      \
@@ -274,8 +286,9 @@ int launch_gather_rows(const fomoe_config& c, const void* x, const RouteWs& ws, 
 int launch_combine(const fomoe_config& c, const fomoe_route_state& r, const RouteWs& ws, const void* o, const void* y_sh,
                    void* y, cudaStream_t st) {
   if (c.T == 0) return FOMOE_OK;
-  ROWS_DISPATCH(c, FOMOE_CUDA_OK(launch_pdl(combine_kernel<T, V>, row_grid(c.T, c.d_model), kRowThreads, 0, st, (const T*)o, (const T*)y_sh, r.gate,
-                                            ws.pair_prow, c.T, c.d_model, c.top_k, (T*)y)));
+  ROWS_DISPATCH(c, const int rpb = rows_per_block(c.d_model, V);
+                FOMOE_CUDA_OK(launch_pdl(combine_kernel<T, V>, row_grid(ceil_div(c.T, rpb), c.d_model * rpb), kRowThreads, 0, st, (const T*)o,
+                                         (const T*)y_sh, r.gate, ws.pair_prow, c.T, c.d_model, c.top_k, rpb, (T*)y)));
   FOMOE_LAUNCH_OK("combine_kernel");
   return FOMOE_OK;
 }
@@ -313,8 +326,9 @@ int launch_gate_bwd(const fomoe_config& c, const fomoe_route_state& r, const Rou
 int launch_dx_sum(const fomoe_config& c, const RouteWs& ws, const void* dxp, const void* dx_sh, const float* dx_r, const void* dx_r_t,
                   void* dx, cudaStream_t st) {
   if (c.T == 0) return FOMOE_OK;
-  ROWS_DISPATCH(c, FOMOE_CUDA_OK(launch_pdl(dx_sum_kernel<T, V>, row_grid(c.T, c.d_model), kRowThreads, 0, st, (const T*)dxp, (const T*)dx_sh, dx_r,
-                                            (const T*)dx_r_t, ws.pair_prow, c.T, c.d_model, c.top_k, (T*)dx)));
+  ROWS_DISPATCH(c, const int rpb = rows_per_block(c.d_model, V);
+                FOMOE_CUDA_OK(launch_pdl(dx_sum_kernel<T, V>, row_grid(ceil_div(c.T, rpb), c.d_model * rpb), kRowThreads, 0, st, (const T*)dxp,
+                                         (const T*)dx_sh, dx_r, (const T*)dx_r_t, ws.pair_prow, c.T, c.d_model, c.top_k, rpb, (T*)dx)));
   FOMOE_LAUNCH_OK("dx_sum_kernel");
   return FOMOE_OK;
 }
