@@ -63,3 +63,14 @@ def test_fine_many_pairs_full_rounds(oracle64):
     w = _w("fine_rounds", T=12000, d=256, E=16, k=8, n_res=8, seed=13)
     errs, _ = run_and_compare(H.Problem(w), oracle64)
     print("fine_rounds", errs)
+
+
+@pytest.mark.parametrize("name", ["P1", "P2", "P3"])
+def test_paper_shapes_full_size_every_element(oracle64, name):
+    """The paper's Medium, Large and XL shapes at full size (P1: T = 16384, d_model = 512, 16 experts of width 128, 4 active, 8
+    resident; P2: d_model = 1024, 32 experts, 8 active, 16 resident; P3: d_model = 2048, 64 experts, 16 active, 32 resident;
+    PAPER.md:300-309), i.e. exactly what bench.py --workload P1|P2|P3 times: every element of every output of the
+    forward and the backward against the fp64 oracle — 256 / 512 / 1048 row tiles (full rounds of pairs + the tail of singles),
+    the split-K (P1), single-round (P2) and multi-round (P3) weight gradients, two token rows per CTA in combine / dx_sum (P1)."""
+    errs, _ = run_and_compare(H.Problem(W.config(name)), oracle64)
+    print(name, "full", errs)
