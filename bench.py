@@ -427,6 +427,36 @@ def run_gpu(args, w, n_res):
         hbms = [k for k in kernels if k.get("bound") == "hbm"]
         if hbms:
             out["hbm_kernels"] = {k["name"]: round(k["frac"], 3) for k in hbms}
+        # ---- the routing call timed ALONE (fomoe_route only, L2 flushed before every call, after a pause that lets the SM clock
+        # recover): inside a long power-capped step the router runs at the GEMMs' reduced SM clock, and it is bound on the SM side
+        # (L2 -> SM operand delivery), so kernels[] above understates what the kernel does at full clock; this is
+        # the "kernel timed alone against the burst peak" form of the same number ----
+        time.sleep(1.0)
+        B.fomoe_profile_enable(True)
+        sampler2 = ClockSampler(local)
+        sampler2.start()
+        w_t0 = time.perf_counter()
+        for _ in range(max(50, args.steps)):
+            flush.zero_()
+            layer.route(x)
+        torch.cuda.synchronize()
+        w_t1 = time.perf_counter()
+        rclk = sampler2.stop((w_t0, w_t1))
+        rrecs = B.fomoe_profile_collect(65536)
+        B.fomoe_profile_enable(False)
+        ralone = {}
+        for name, t in rrecs:
+            a = ralone.setdefault(name, [0.0, 0])
+            a[0] += t
+            a[1] += 1
+        out["route_alone"] = {"clocks": rclk, "kernels": []}
+        for name, (tt, n) in ralone.items():
+            kk = {"name": name, "ms_per_launch": tt / n}
+            hbn = hbm_bytes(name, P, w.T, w)
+            if hbn is not None:
+                kk.update(bound="hbm", achieved=hbn[0] / (tt / n / 1e3) / 1e9, unit="GB/s", peak=peaks["hbm_gbs"])
+                kk["frac"] = kk["achieved"] / peaks["hbm_gbs"]
+            out["route_alone"]["kernels"].append(kk)
 
         # ---- end to end through the C ABI with HOST buffers (uploads x, dy; downloads y, dx every step).  Two arms:
         # "serial": one self-contained call per step (results complete when the stream is);  headline e2e: the same call with
