@@ -218,7 +218,7 @@ FOMOE_API int fomoe_periln_bwd(int32_t T, int32_t d_model, int32_t dtype, const 
  * the process exits.  Same arguments (all device pointers, caller-owned), same kernels and the same fixed-order reduction as
  * fomoe_periln_bwd: bit-identical results.  The call allocates nothing (no cudaMalloc / cudaFree / allocating library
  * routine); its only set-up is one cudaGetSymbolAddress per device.
- *   Limit: 2 * min(T, 8 * SM count) * d_model <= 4 Mi (on a 148-SM B200: every T up to d_model = 1771, wider rows only for
+ *   Limit: 2 * min(T, 4 * SM count) * d_model <= 4 Mi (on a 148-SM B200: every T up to d_model = 3543, wider rows only for
  *   fewer tokens).  Beyond it: FOMOE_ERR_UNSUPPORTED, text via fomoe_last_cuda_error(); use fomoe_periln_bwd then.
  *   Sharing: every call on a device uses the same array.  Calls on ONE stream are ordered and safe; calls that overlap on the
  *   GPU (several streams, concurrent graph launches) race on it.  Nothing in it needs clearing between calls (each call

@@ -3,9 +3,12 @@
 //   periln_fwd : out = [residual +] alpha (gamma xhat + beta), saves (mean, rstd)       — pre-LN (no residual) and post-LN + residual
 //   periln_bwd : dx = [dresidual +] rstd (dxhat - mean(dxhat) - xhat mean(dxhat xhat)), dxhat = alpha dout gamma;
 //                per-CTA partial dgamma / dbeta, summed by a second kernel in a fixed order (run-to-run identical)
-// The row is staged once in shared memory (fp32), so mean and the centred variance are computed exactly as LayerNorm
-// defines them and global memory is read once.  Bound: HBM.
+// Three forms of each: *_ring_kernel (rows prefetched by cp.async.bulk into a shared-memory ring, gamma / beta and the
+// accumulators in registers: the default for rows of at most two 16-byte vectors per thread), *_reg_kernel (row held in
+// registers, more CTAs per SM) and the general kernel that stages the row in shared memory as fp32.  Mean and the centred
+// variance are computed exactly as LayerNorm defines them and global memory is read once.  Bound: HBM.
 #include "common.cuh"
+#include "umma_ptx.cuh"
 #include <stdio.h>
 #include <stdlib.h>
 
@@ -274,6 +277,117 @@ periln_fwd_reg_kernel(const T* __restrict__ x, const float* __restrict__ gamma, 
   }
 }
 
+// The same kernel with the row loads taken off the critical path: thread 0 keeps a ring of kRingStages rows per CTA filled with
+// bulk copies (cp.async.bulk, completion on an mbarrier), kRingStages rows ahead of the row being normalised, so the bytes an
+// SM has in flight no longer depend on how many CTAs' registers fit.  Every thread then reads exactly the vectors it would
+// have loaded from global memory, and the arithmetic below that point is periln_fwd_reg_kernel's, statement for statement
+// (same bits).  Rows of d * sizeof(T) bytes, 16-byte multiples.
+constexpr int kRingStages = 3;
+__device__ __forceinline__ void bulk_row_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+template <typename T, int NV, bool RES>
+__global__ void __launch_bounds__(kLnThreads, 3)
+periln_fwd_ring_kernel(const T* __restrict__ x, const float* __restrict__ gamma, const float* __restrict__ beta, const T* __restrict__ residual,
+                       float alpha, float eps, int T_, int d, T* __restrict__ out, float* __restrict__ stats) {
+  constexpr int VN = VecN<T>::n;
+  extern __shared__ __align__(128) uint8_t ring[];   // [kRingStages][x row | residual row]
+  __shared__ float red[kLnThreads / 32];
+  __shared__ __align__(8) uint64_t full[kRingStages];
+  const uint32_t row_bytes = (uint32_t)d * sizeof(T), stage_bytes = row_bytes * (RES ? 2 : 1);
+  const uint32_t ring0 = smem_u32(ring), full0 = smem_u32(full);
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < kRingStages; ++s) mbar_init(full0 + 8 * s, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  pdl_launch_dependents();
+  pdl_wait();
+  auto issue = [&](int t, int s) {   // thread 0: row t into stage s
+    mbar_expect_tx(full0 + 8 * s, stage_bytes);
+    bulk_row_load(ring0 + s * stage_bytes, x + (size_t)t * d, row_bytes, full0 + 8 * s);
+    if (RES) bulk_row_load(ring0 + s * stage_bytes + row_bytes, residual + (size_t)t * d, row_bytes, full0 + 8 * s);
+  };
+  if (threadIdx.x == 0)
+    for (int s = 0; s < kRingStages; ++s) {
+      const long t = (long)blockIdx.x + (long)s * gridDim.x;
+      if (t < T_) issue((int)t, s);
+    }
+  // with the loads prefetched, occupancy no longer decides the bytes in flight: gamma / beta live in registers for the whole
+  // kernel and the row is widened to fp32 once (the register-resident kernel re-reads 4 bytes of gamma / beta per byte of row
+  // from L1 and widens the row three times: ncu shows it bound by issue slots and the L1 pipe, not by DRAM)
+  float g[NV][VN], b[NV][VN];
+#pragma unroll
+  for (int j = 0; j < NV; ++j) {
+    const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
+#pragma unroll
+    for (int i = 0; i < VN; ++i) { g[j][i] = 0.f; b[j][i] = 0.f; }
+    if (c < d) { ld_param<T, VN>(gamma + c, g[j]); ld_param<T, VN>(beta + c, b[j]); }
+  }
+  int stage = 0;
+  uint32_t phase = 0;
+  for (int t = blockIdx.x; t < T_; t += gridDim.x) {
+    const size_t base = (size_t)t * d;
+    float v[NV][VN];
+    uint4 rr[NV];
+    mbar_wait(full0 + 8 * stage, phase);
+    const uint32_t srow = ring0 + stage * stage_bytes;
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
+      uint4 xr = make_uint4(0u, 0u, 0u, 0u);
+      rr[j] = make_uint4(0u, 0u, 0u, 0u);
+      if (c < d) {
+        asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(xr.x), "=r"(xr.y), "=r"(xr.z), "=r"(xr.w)
+                     : "r"(srow + c * (uint32_t)sizeof(T)) : "memory");
+        if (RES)
+          asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(rr[j].x), "=r"(rr[j].y), "=r"(rr[j].z), "=r"(rr[j].w)
+                       : "r"(srow + row_bytes + c * (uint32_t)sizeof(T)) : "memory");
+      }
+      unpack<T>(xr, v[j]);
+    }
+    __syncthreads();   // every thread has its vectors: the stage can be refilled
+    if (threadIdx.x == 0) {
+      const long tn = (long)t + (long)kRingStages * gridDim.x;
+      if (tn < T_) issue((int)tn, stage);
+    }
+    if (++stage == kRingStages) { stage = 0; phase ^= 1; }
+    float s = 0.f;
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
+      if (c < d) {
+#pragma unroll
+        for (int i = 0; i < VN; ++i) s += v[j][i];
+      }
+    }
+    const float mean = block_sum(s, red) / (float)d;
+    float q = 0.f;
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
+      if (c < d) {
+#pragma unroll
+        for (int i = 0; i < VN; ++i) { v[j][i] -= mean; q += v[j][i] * v[j][i]; }
+      }
+    }
+    const float rstd = rsqrtf(block_sum(q, red) / (float)d + eps);
+    if (threadIdx.x == 0) { stats[2 * (size_t)t] = mean; stats[2 * (size_t)t + 1] = rstd; }
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
+      if (c < d) {
+        float r[VN], o[VN];
+        unpack<T>(rr[j], r);
+#pragma unroll
+        for (int i = 0; i < VN; ++i) o[i] = ln_out(v[j][i], rstd, g[j][i], b[j][i], alpha, RES, r[i]);
+        stv<T>(out + base + c, o);
+      }
+    }
+  }
+}
+
 // Rows held as loaded (see periln_fwd_reg_kernel).  The dgamma / dbeta accumulators live in shared memory when the row is at
 // most two vectors per thread (each thread reads and writes only its own columns: no conflicts, no atomics, fixed token
 // order), which brings the kernel from 80-127 registers to <= 64 and from 2-3 resident CTAs per SM to 4.
@@ -366,6 +480,123 @@ periln_bwd_reg_kernel(const T* __restrict__ dout, const T* __restrict__ x, const
       for (int i = 0; i < VN; ++i) {
         partials[((size_t)blockIdx.x * 2) * d + c + i] = kSmemAcc ? acc_sm[c + i] : ag[j][i];
         partials[((size_t)blockIdx.x * 2 + 1) * d + c + i] = kSmemAcc ? acc_sm[d + c + i] : ab[j][i];
+      }
+    }
+  }
+}
+
+// The backward with its rows prefetched through the same kind of ring (dout row | x row | dresidual row per stage) and, since
+// occupancy no longer matters, gamma and the dgamma / dbeta accumulators in registers for the whole kernel (the register kernel
+// above reads and writes 16 bytes of shared-memory accumulators and re-reads 8 bytes of gamma per byte of row).  Same grid,
+// same token order per CTA and the same element formulas as periln_bwd_reg_kernel: same bits, partials included.
+template <typename T, int NV, bool RES>
+__global__ void __launch_bounds__(kLnThreads, 2)
+periln_bwd_ring_kernel(const T* __restrict__ dout, const T* __restrict__ x, const float* __restrict__ stats, const float* __restrict__ gamma,
+                       float alpha, const T* __restrict__ dresidual, int T_, int d, T* __restrict__ dx, float* __restrict__ partials) {
+  constexpr int VN = VecN<T>::n;
+  constexpr int kRows = RES ? 3 : 2;
+  extern __shared__ __align__(128) uint8_t ring[];
+  __shared__ float red[2 * (kLnThreads / 32)];
+  __shared__ __align__(8) uint64_t full[kRingStages];
+  const uint32_t row_bytes = (uint32_t)d * sizeof(T), stage_bytes = row_bytes * kRows;
+  const uint32_t ring0 = smem_u32(ring), full0 = smem_u32(full);
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < kRingStages; ++s) mbar_init(full0 + 8 * s, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  pdl_launch_dependents();
+  pdl_wait();
+  auto issue = [&](int t, int s) {
+    mbar_expect_tx(full0 + 8 * s, stage_bytes);
+    bulk_row_load(ring0 + s * stage_bytes, dout + (size_t)t * d, row_bytes, full0 + 8 * s);
+    bulk_row_load(ring0 + s * stage_bytes + row_bytes, x + (size_t)t * d, row_bytes, full0 + 8 * s);
+    if (RES) bulk_row_load(ring0 + s * stage_bytes + 2 * row_bytes, dresidual + (size_t)t * d, row_bytes, full0 + 8 * s);
+  };
+  if (threadIdx.x == 0)
+    for (int s = 0; s < kRingStages; ++s) {
+      const long t = (long)blockIdx.x + (long)s * gridDim.x;
+      if (t < T_) issue((int)t, s);
+    }
+  float g[NV][VN], ag[NV][VN], ab[NV][VN];
+#pragma unroll
+  for (int j = 0; j < NV; ++j) {
+    const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
+#pragma unroll
+    for (int i = 0; i < VN; ++i) { g[j][i] = 0.f; ag[j][i] = 0.f; ab[j][i] = 0.f; }
+    if (c < d) ld_param<T, VN>(gamma + c, g[j]);
+  }
+  int stage = 0;
+  uint32_t phase = 0;
+  float2 st_cur = blockIdx.x < T_ ? *reinterpret_cast<const float2*>(stats + 2 * (size_t)blockIdx.x) : make_float2(0.f, 0.f);
+  for (int t = blockIdx.x; t < T_; t += gridDim.x) {
+    const size_t base = (size_t)t * d;
+    const float mean = st_cur.x, rstd = st_cur.y;
+    if ((long)t + gridDim.x < T_) st_cur = *reinterpret_cast<const float2*>(stats + 2 * ((size_t)t + gridDim.x));   // next row's, early
+    float gi[NV][VN], hi[NV][VN];
+    uint4 rr[NV];
+    mbar_wait(full0 + 8 * stage, phase);
+    const uint32_t srow = ring0 + stage * stage_bytes;
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
+      uint4 gr = make_uint4(0u, 0u, 0u, 0u), xr = make_uint4(0u, 0u, 0u, 0u);
+      rr[j] = make_uint4(0u, 0u, 0u, 0u);
+      if (c < d) {
+        const uint32_t a = srow + c * (uint32_t)sizeof(T);
+        asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(gr.x), "=r"(gr.y), "=r"(gr.z), "=r"(gr.w) : "r"(a) : "memory");
+        asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(xr.x), "=r"(xr.y), "=r"(xr.z), "=r"(xr.w) : "r"(a + row_bytes) : "memory");
+        if (RES)
+          asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(rr[j].x), "=r"(rr[j].y), "=r"(rr[j].z), "=r"(rr[j].w)
+                       : "r"(a + 2 * row_bytes) : "memory");
+      }
+      unpack<T>(gr, gi[j]);
+      unpack<T>(xr, hi[j]);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      const long tn = (long)t + (long)kRingStages * gridDim.x;
+      if (tn < T_) issue((int)tn, stage);
+    }
+    if (++stage == kRingStages) { stage = 0; phase ^= 1; }
+    float s1 = 0.f, s2 = 0.f;
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
+      if (c < d) {
+#pragma unroll
+        for (int i = 0; i < VN; ++i) {
+          gi[j][i] = __fmul_rn(alpha, gi[j][i]);
+          hi[j][i] = __fmul_rn(hi[j][i] - mean, rstd);
+          ln_bwd_acc(gi[j][i], hi[j][i], g[j][i], ag[j][i], ab[j][i], s1, s2);   // fixed token order per CTA
+        }
+      }
+    }
+    block_sum2(s1, s2, red);
+    const float m1 = s1 / (float)d, m2 = s2 / (float)d;
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+      const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
+      if (c < d) {
+        float r[VN], o[VN];
+        unpack<T>(rr[j], r);
+#pragma unroll
+        for (int i = 0; i < VN; ++i) {
+          const float dxh = __fmul_rn(gi[j][i], g[j][i]);          // the same roundings as in ln_bwd_acc
+          o[i] = ln_dx(rstd, dxh, m1, hi[j][i], m2, RES, r[i]);
+        }
+        stv<T>(dx + base + c, o);
+      }
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < NV; ++j) {
+    const int c = (j * (int)blockDim.x + threadIdx.x) * VN;
+    if (c < d) {
+#pragma unroll
+      for (int i = 0; i < VN; ++i) {
+        partials[((size_t)blockIdx.x * 2) * d + c + i] = ag[j][i];
+        partials[((size_t)blockIdx.x * 2 + 1) * d + c + i] = ab[j][i];
       }
     }
   }
@@ -616,7 +847,9 @@ periln_reduce_kernel(const float* __restrict__ partials, int n_blk, int d, float
 
 }  // namespace
 
-int periln_blocks(int T) { int g = num_sms() * 8; if (g > T) g = T; return g < 1 ? 1 : g; }
+// CTAs of the backward kernels = partial dgamma / dbeta sums: 4 per SM is one wave of the register-resident and of the fused
+// kernels (4 CTAs resident) and two waves of the ring kernel (2 resident); every CTA costs 2 d floats of partial-sum traffic
+int periln_blocks(int T) { int g = num_sms() * 4; if (g > T) g = T; return g < 1 ? 1 : g; }
 
 // threads per CTA and vectors per thread needed to hold one row in registers; nv = 0: use the shared-memory kernels
 template <typename T> static void reg_shape(int d, int& threads, int& nv) {
@@ -638,6 +871,26 @@ static int periln_fwd_t(int Tn, int d, const void* x, const float* gamma, const 
   reg_shape<T>(d, threads, nv);
   const int grid_reg = Tn < num_sms() * 32 ? Tn : num_sms() * 32;
   const int grid = Tn < num_sms() * 16 ? Tn : num_sms() * 16;
+  static const int ring_mode = [] { const char* e = getenv("FOMOE_LN_RING"); return e ? atoi(e) : 1; }();   // FOMOE_LN_RING=0: the register-resident kernels
+  if (ring_mode && nv >= 1 && nv <= 2 && ((size_t)d * sizeof(T)) % 16 == 0) {
+    const size_t smem = (size_t)kRingStages * d * sizeof(T) * (residual ? 2 : 1);
+    const int ctas = threads == kLnThreads ? 3 : 6;
+    const int grid_ring = Tn < num_sms() * ctas ? Tn : num_sms() * ctas;
+#define LN_RING(NV, RES)                                                                                                            \
+    do {                                                                                                                          \
+      static PerDeviceOnce attr;                                                                                                  \
+      if (attr.need()) { FOMOE_CUDA_OK(cudaFuncSetAttribute(periln_fwd_ring_kernel<T, NV, RES>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024)); attr.set(); } \
+      FOMOE_CUDA_OK(launch_pdl(periln_fwd_ring_kernel<T, NV, RES>, grid_ring, threads, smem, st, (const T*)x, gamma, beta, (const T*)residual, \
+                               alpha, eps, Tn, d, (T*)out, stats));                                                               \
+    } while (0)
+    if (smem <= 96 * 1024) {
+      if (nv == 1) { if (residual) LN_RING(1, true); else LN_RING(1, false); }
+      else { if (residual) LN_RING(2, true); else LN_RING(2, false); }
+      FOMOE_LAUNCH_OK("periln_fwd_ring_kernel");
+      return FOMOE_OK;
+    }
+#undef LN_RING
+  }
 #define LN_FWD(NV)                                                                                                                  \
   do {                                                                                                                            \
     if (residual) FOMOE_CUDA_OK(launch_pdl(periln_fwd_reg_kernel<T, NV, true>, grid_reg, threads, 0, st, (const T*)x, gamma, beta,      \
@@ -670,6 +923,24 @@ static int periln_bwd_t(int Tn, int d, int nb, const void* dout, const void* x, 
                         const void* dresidual, void* dx, float* partials, cudaStream_t st) {
   int threads, nv;
   reg_shape<T>(d, threads, nv);
+  static const int ring_mode = [] { const char* e = getenv("FOMOE_LN_RING"); return e ? atoi(e) : 1; }();   // FOMOE_LN_RING=0: the register-resident kernels
+  if (ring_mode && nv >= 1 && nv <= 2 && ((size_t)d * sizeof(T)) % 16 == 0) {
+    const size_t smem = (size_t)kRingStages * d * sizeof(T) * (dresidual ? 3 : 2);
+#define LN_BRING(NV, RES)                                                                                                          \
+    do {                                                                                                                          \
+      static PerDeviceOnce attr;                                                                                                  \
+      if (attr.need()) { FOMOE_CUDA_OK(cudaFuncSetAttribute(periln_bwd_ring_kernel<T, NV, RES>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024)); attr.set(); } \
+      FOMOE_CUDA_OK(launch_pdl(periln_bwd_ring_kernel<T, NV, RES>, nb, threads, smem, st, (const T*)dout, (const T*)x, stats, gamma, alpha, \
+                               (const T*)dresidual, Tn, d, (T*)dx, partials));                                                    \
+    } while (0)
+    if (smem <= 100 * 1024) {
+      if (nv == 1) { if (dresidual) LN_BRING(1, true); else LN_BRING(1, false); }
+      else { if (dresidual) LN_BRING(2, true); else LN_BRING(2, false); }
+      FOMOE_LAUNCH_OK("periln_bwd_ring_kernel");
+      return FOMOE_OK;
+    }
+#undef LN_BRING
+  }
 #define LN_BWD(NV) FOMOE_CUDA_OK(launch_pdl(periln_bwd_reg_kernel<T, NV>, nb, threads, (NV <= 2 ? sizeof(float) * 2 * (size_t)d : 0), st, (const T*)dout, (const T*)x, stats, gamma, alpha, (const T*)dresidual, Tn, d, (T*)dx, partials))
   if (nv == 1) LN_BWD(1);
   else if (nv == 2) LN_BWD(2);
@@ -762,8 +1033,8 @@ int launch_dx_sum_periln(const fomoe_config& c, const RouteWs& ws, const void* d
 // so cannot provide fomoe_periln_workspace_bytes() bytes of scratch: the per-CTA dgamma / dbeta partial sums live in the
 // array below, 16 MiB that every GPU which loads libfomoe.so holds until the process exits.  Same kernels, same grid and
 // same fixed-order reduction as fomoe_periln_bwd: the results are bit-identical to it.
-//   * limit: 2 * periln_blocks(T) * d_model <= kNoAllocFloats (periln_blocks = min(T, 8 * SMs): on a 148-SM B200 any T up
-//     to d_model = 1771; larger rows only for fewer tokens); beyond it FOMOE_ERR_UNSUPPORTED with a text in fomoe_last_cuda_error().
+//   * limit: 2 * periln_blocks(T) * d_model <= kNoAllocFloats (periln_blocks = min(T, 4 * SMs): on a 148-SM B200 any T up
+//     to d_model = 3543; larger rows only for fewer tokens); beyond it FOMOE_ERR_UNSUPPORTED with a text in fomoe_last_cuda_error().
 //   * every call on a device shares the array: calls that overlap on the GPU (different streams, or concurrent graphs) RACE.
 //     Calls on one stream are ordered and safe.  Nothing in it has to start at zero -- every CTA of the backward kernel
 //     overwrites its own 2 * d_model partials before the reduce kernel reads them -- so the previous call's contents are
