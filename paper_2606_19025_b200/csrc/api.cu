@@ -386,6 +386,7 @@ int fomoe_periln_fwd(int32_t T, int32_t d_model, int32_t dtype, const void* x, c
   g_launches = 0;
   if (T < 0 || d_model <= 0 || (dtype != FOMOE_F32 && dtype != FOMOE_BF16) || !gamma || !beta || !(eps >= 0.f)) return FOMOE_ERR_BADARG;
   if (T > 0 && (!x || !out || !stats)) return FOMOE_ERR_BADARG;
+  if (!aligned16(x) || !aligned16(out) || !aligned16(residual) || !aligned16(gamma) || !aligned16(beta)) return FOMOE_ERR_BADARG;
   if ((size_t)d_model * 16 > 200 * 1024) return FOMOE_ERR_UNSUPPORTED;   // the backward stages 4 fp32 rows in shared memory
   note_api_entry("@fomoe_periln_fwd", (cudaStream_t)stream);
   return launch_periln_fwd(T, d_model, dtype, x, gamma, beta, eps, residual, alpha, out, stats, (cudaStream_t)stream);
@@ -396,6 +397,7 @@ int fomoe_periln_bwd(int32_t T, int32_t d_model, int32_t dtype, const void* dout
   g_launches = 0;
   if (T < 0 || d_model <= 0 || (dtype != FOMOE_F32 && dtype != FOMOE_BF16) || !gamma || !dgamma || !dbeta || !partials) return FOMOE_ERR_BADARG;
   if (T > 0 && (!dout || !x || !stats || !dx)) return FOMOE_ERR_BADARG;
+  if (!aligned16(dout) || !aligned16(x) || !aligned16(dresidual) || !aligned16(dx) || !aligned16(gamma) || !aligned16(partials)) return FOMOE_ERR_BADARG;
   if ((size_t)d_model * 16 > 200 * 1024) return FOMOE_ERR_UNSUPPORTED;
   note_api_entry("@fomoe_periln_bwd", (cudaStream_t)stream);
   return launch_periln_bwd(T, d_model, dtype, dout, x, stats, gamma, alpha, dresidual, dx, dgamma, dbeta, partials, (cudaStream_t)stream);

@@ -1068,6 +1068,7 @@ extern "C" FOMOE_API int fomoe_periln_bwd_noalloc(int32_t T, int32_t d_model, in
   reset_launch_count();
   if (T < 0 || d_model <= 0 || (dtype != FOMOE_F32 && dtype != FOMOE_BF16) || !gamma || !dgamma || !dbeta) return FOMOE_ERR_BADARG;
   if (T > 0 && (!dout || !x || !stats || !dx)) return FOMOE_ERR_BADARG;
+  if (((uintptr_t)dout | (uintptr_t)x | (uintptr_t)dresidual | (uintptr_t)dx | (uintptr_t)gamma) & 15) return FOMOE_ERR_BADARG;
   if ((size_t)d_model * 16 > 200 * 1024) return FOMOE_ERR_UNSUPPORTED;
   const size_t need = 2 * (size_t)periln_blocks(T) * (size_t)d_model;
   if (need > kNoAllocFloats) {
