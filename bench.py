@@ -124,6 +124,15 @@ class ClockSampler:
             self.stop_flag = True
             self.thread.join()
             src = "nvml, 2 ms poll"
+            if not self.rows:   # a region of a few ms can end before the first poll returns: one sample right after it
+                try:
+                    n = self.nvml
+                    sm = float(n.nvmlDeviceGetClockInfo(self.handle, n.NVML_CLOCK_SM))
+                    mx = float(n.nvmlDeviceGetMaxClockInfo(self.handle, n.NVML_CLOCK_SM))
+                    self.rows.append((sm, mx, [], time.perf_counter()))
+                    src = "nvml, one sample right after the timed region (no poll landed inside it)"
+                except Exception:
+                    pass
         elif self.proc is not None:
             time.sleep(0.15)
             self.proc.terminate()
