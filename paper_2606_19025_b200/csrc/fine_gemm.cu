@@ -677,7 +677,8 @@ int fine_wgrad(const fomoe_config& c, int n_res, const void* x, const void* dy, 
   // the SMs that round leaves idle, so only the single-round case is split.
   const int tiles = n_res * 2 * (c.d_model / 256), grid = num_sms();
   const int full = tiles / grid * grid, tail = tiles - full;
-  int ks = (tail > 0 && (full == 0 || getenv("FOMOE_FINE_TAILSPLIT"))) ? grid / tail : 1;
+  static const bool split_tail_round = getenv("FOMOE_FINE_TAILSPLIT") != nullptr;   // (A/B measurements of the multi-round case)
+  int ks = (tail > 0 && (full == 0 || split_tail_round)) ? grid / tail : 1;
   if (ks > 8) ks = 8;
   while (ks > 1 && (size_t)tail * ks * GT * 256 * sizeof(float) > sizeof(bf16) * (size_t)R * c.d_model) --ks;
   p.wg_full = ks > 1 ? full : tiles;
