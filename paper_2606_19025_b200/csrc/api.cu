@@ -50,10 +50,18 @@ void reset_launch_count() { g_launches = 0; }
 struct SideStream {
   cudaStream_t s = nullptr;
   cudaEvent_t fork = nullptr, join = nullptr;
+  // a second one for the weight-gradient GEMMs of the tensor-core path: they depend on DH only, so they run beside the
+  // bandwidth-bound dx scatter-sum (which co-resides with their one-CTA-per-SM kernels) instead of ahead of it
+  cudaStream_t s2 = nullptr;
+  cudaEvent_t fork2 = nullptr, join2 = nullptr;
   bool ok = false;
 };
 constexpr int kMaxDevices = 64;
 static thread_local SideStream g_side[kMaxDevices];   // one per (host thread, device): a device switch creates, never leaks
+static bool wg_stream_enabled() {   // FOMOE_WG_STREAM=0: weight gradients on the caller's stream, no stream priorities
+  static const bool on = [] { const char* e = getenv("FOMOE_WG_STREAM"); return !(e && e[0] == '0'); }();
+  return on;
+}
 static bool side_enabled() {
   static const bool on = [] { const char* e = getenv("FOMOE_SIDE_STREAM"); return !(e && e[0] == '0'); }();
   return on;
@@ -64,9 +72,16 @@ static SideStream* side_stream() {
   if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return nullptr;
   SideStream& sd = g_side[dev];
   if (!sd.ok) {
-    if (!sd.s && cudaStreamCreateWithFlags(&sd.s, cudaStreamNonBlocking) != cudaSuccess) return nullptr;
+    // priorities: the router's backward chain first (the dx scatter-sum waits for it, and its GEMMs need whole SMs), the
+    // weight gradients last (nothing in the step waits for them), so that when the DX kernel drains the chain gets the SMs
+    int prio_lo = 0, prio_hi = 0;
+    if (wg_stream_enabled()) cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);   // (numerically: lowest priority = largest value)
+    if (!sd.s && cudaStreamCreateWithPriority(&sd.s, cudaStreamNonBlocking, prio_hi) != cudaSuccess) return nullptr;
     if (!sd.fork && cudaEventCreateWithFlags(&sd.fork, cudaEventDisableTiming) != cudaSuccess) return nullptr;
     if (!sd.join && cudaEventCreateWithFlags(&sd.join, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+    if (!sd.s2 && cudaStreamCreateWithPriority(&sd.s2, cudaStreamNonBlocking, prio_lo) != cudaSuccess) return nullptr;
+    if (!sd.fork2 && cudaEventCreateWithFlags(&sd.fork2, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+    if (!sd.join2 && cudaEventCreateWithFlags(&sd.join2, cudaEventDisableTiming) != cudaSuccess) return nullptr;
     sd.ok = true;
   }
   return &sd;
@@ -284,7 +299,8 @@ static int moe_bwd_impl(const fomoe_config* cfg, const void* dy, const void* x, 
     return tc_router ? umma_router_bwd(*cfg, x, w_router, route_umma_supported(*cfg) ? rws.wr_bf : nullptr, sws, dw_router, rst)
                      : simt_router_bwd(*cfg, x, w_router, sws, dw_router, rst);
   };
-  bool forked = false;
+  bool forked = false, wg_forked = false;
+  const bool wg_overlap = wg_stream_enabled();
   auto fork_router = [&]() -> int {   // side stream: waits for everything queued on `st` so far, then runs the router's backward
     FOMOE_CUDA_OK(cudaEventRecord(side->fork, st));
     FOMOE_CUDA_OK(cudaStreamWaitEvent(side->s, side->fork, 0));
@@ -302,7 +318,8 @@ static int moe_bwd_impl(const fomoe_config* cfg, const void* dy, const void* x, 
     }
     // B2-B4 (+ shared experts)
     r = use_umma(*cfg) ? umma_ffn_bwd(*cfg, n_res, x, dy, rws, aws, sws, w, dw_gate, dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, st,
-                                      dgate_in_dh, dgate_in_dh ? &after_dh : nullptr)
+                                      dgate_in_dh, dgate_in_dh ? &after_dh : nullptr, (side && wg_overlap && cfg->T > 0) ? side->s2 : nullptr,
+                                      side ? side->fork2 : nullptr, &wg_forked)
                        : simt_ffn_bwd(*cfg, n_res, x, dy, rws, aws, sws, w, dw_gate, dw_up, dw_down, d_sh_gate, d_sh_up, d_sh_down, st);
     if (r != FOMOE_OK) return r;
     return forked ? FOMOE_OK : router_bwd();
@@ -314,12 +331,19 @@ static int moe_bwd_impl(const fomoe_config* cfg, const void* dy, const void* x, 
     if (rc == FOMOE_OK && e1 != cudaSuccess) return set_cuda_error(e1, "cudaEventRecord(join)");
     if (rc == FOMOE_OK && e2 != cudaSuccess) return set_cuda_error(e2, "cudaStreamWaitEvent(join)");
   }
-  if (rc != FOMOE_OK) return rc;
-  // B5 (with the pre-LN backward folded in when asked for)
-  if (ln) return launch_dx_sum_periln(*cfg, rws, sws.dxp, cfg->n_shared > 0 ? sws.dx_sh : nullptr, tc_router ? nullptr : sws.dx_r,
-                                      tc_router ? (const void*)sws.dx_r : nullptr, *ln, dx, st);
-  return launch_dx_sum(*cfg, rws, sws.dxp, cfg->n_shared > 0 ? sws.dx_sh : nullptr, tc_router ? nullptr : sws.dx_r,
-                       tc_router ? (const void*)sws.dx_r : nullptr, dx, st);
+  // B5 (with the pre-LN backward folded in when asked for); whatever happened, the weight-gradient stream is joined back
+  if (rc == FOMOE_OK)
+    rc = ln ? launch_dx_sum_periln(*cfg, rws, sws.dxp, cfg->n_shared > 0 ? sws.dx_sh : nullptr, tc_router ? nullptr : sws.dx_r,
+                                   tc_router ? (const void*)sws.dx_r : nullptr, *ln, dx, st)
+            : launch_dx_sum(*cfg, rws, sws.dxp, cfg->n_shared > 0 ? sws.dx_sh : nullptr, tc_router ? nullptr : sws.dx_r,
+                            tc_router ? (const void*)sws.dx_r : nullptr, dx, st);
+  if (side && wg_forked) {
+    cudaError_t e1 = cudaEventRecord(side->join2, side->s2);
+    cudaError_t e2 = cudaStreamWaitEvent(st, side->join2, 0);
+    if (rc == FOMOE_OK && e1 != cudaSuccess) return set_cuda_error(e1, "cudaEventRecord(join2)");
+    if (rc == FOMOE_OK && e2 != cudaSuccess) return set_cuda_error(e2, "cudaStreamWaitEvent(join2)");
+  }
+  return rc;
 }
 
 int fomoe_moe_bwd(const fomoe_config* cfg, const void* dy, const void* x, const fomoe_route_state* route, int32_t n_res,

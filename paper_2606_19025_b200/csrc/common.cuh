@@ -271,7 +271,8 @@ int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs&
 int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy, const RouteWs& rws, const ActWs& aws,
                  const ScratchWs& sws, const FfnPtrs& w, void* dw_gate, void* dw_up, void* dw_down, void* d_sh_gate,
                  void* d_sh_up, void* d_sh_down, cudaStream_t st, bool dgate_in_dh = false,
-                 const std::function<int()>* after_dh = nullptr);
+                 const std::function<int()>* after_dh = nullptr, cudaStream_t wg_stream = nullptr, cudaEvent_t wg_fork = nullptr,
+                 bool* wg_forked = nullptr);   // wg_stream: the weight gradients go there, forked (wg_fork) after the last DX launch
 
 // Fine-grained two-matrix experts (d_expert = 128), fine_gemm.cu: the expert GEMMs gather their token-indexed
 // operand rows inside the kernel (no permuted copy of x or dy).  fine_mask: which of them apply to this configuration

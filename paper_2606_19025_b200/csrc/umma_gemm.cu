@@ -1402,16 +1402,21 @@ int umma_ffn_fwd(const fomoe_config& c, int n_res, const void* x, const RouteWs&
 
 int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy, const RouteWs& rws, const ActWs& aws,
                  const ScratchWs& sws, const FfnPtrs& w, void* dw_gate, void* dw_up, void* dw_down, void* d_sh_gate,
-                 void* d_sh_up, void* d_sh_down, cudaStream_t st, bool dgate_in_dh, const std::function<int()>* after_dh) {
+                 void* d_sh_up, void* d_sh_down, cudaStream_t st_main, bool dgate_in_dh, const std::function<int()>* after_dh,
+                 cudaStream_t wg_stream, cudaEvent_t wg_fork, bool* wg_forked) {
   const int d = c.d_model, F = c.d_ff;
   const bool silu = c.expert_fn == FOMOE_EXPERT_SILU;   // two-matrix expert: one saved factor, dxp = dA W_up, dW_up = dA^T x
+  // Two phases over the same code: 0 = every data gradient (DH, DX; routed, then shared), 1 = every weight gradient.  The
+  // weight gradients depend on the DH outputs only, the dx scatter-sum (the caller's next launch) on the DX outputs only: with
+  // a second stream the bandwidth-bound scatter-sum runs beside the weight-gradient GEMMs instead of after them.
+  auto phase_fn = [&](const int phase, cudaStream_t st) -> int {
   if (n_res > 0) {
     const uint64_t R = (uint64_t)rws.R_cap;
     UmmaParams p{};
     p.n_mtiles = rws.n_mtiles; p.tile_slot = rws.tile_slot; p.pair_info = rws.pair_info; p.pad_offsets = rws.pad_offsets; p.pad_end64 = rws.pad_end64; p.parts = 1; p.d = d; p.F = F; p.ld = F;
     const int fine = silu ? fine_mask(c) : 0;
     void* hg = sws.du;    // fine path: g h [R, F] (the two-matrix expert has no du)
-    if (c.T > 0) {
+    if (c.T > 0 && phase == 0) {
       if (fine & 2) {  // dh = dy[token] W_down gathered in the kernel; da, hg = g h and <dh, h> out of its epilogue
         int rc = fine_dh(c, n_res, dy, rws, aws, sws, hg, w.w_down, st);
         if (rc != FOMOE_OK) return rc;
@@ -1446,7 +1451,8 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
     struct WG { const void* A; int lda; const void* B; int ldb; int M, N; void* out; };
     const WG jobs[3] = {{sws.dop, d, aws.h, F, d, F, dw_down}, {sws.da, F, aws.xp, d, F, d, silu ? dw_up : dw_gate},
                         {sws.du, F, aws.xp, d, F, d, dw_up}};
-    if (fine & 4) {
+    if (phase == 0) {
+    } else if (fine & 4) {
       int rc = fine_wgrad(c, n_res, x, dy, rws, sws, hg, dw_up, dw_down, st);
       if (rc != FOMOE_OK) return rc;
     } else {   // one launch for all of them (same row groups, same K ranges)
@@ -1466,6 +1472,7 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
     }
   }
   if (c.n_shared > 0 && c.T == 0) {  // empty batch: exact zeros
+    if (phase == 0) return FOMOE_OK;
     const size_t n = sizeof(bf16) * (size_t)c.n_shared * c.d_ff_shared * d;
     if (!silu) FOMOE_CUDA_OK(cudaMemsetAsync(d_sh_gate, 0, n, st));
     FOMOE_CUDA_OK(cudaMemsetAsync(d_sh_up, 0, n, st));
@@ -1474,7 +1481,7 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
     const int Fs = c.d_ff_shared, ns = c.n_shared, ld = ns * Fs;
     UmmaParams p{};
     p.dense_rows = c.T; p.parts = ns; p.d = d; p.F = Fs; p.ld = ld;
-    if (c.T > 0) {
+    if (c.T > 0 && phase == 0) {
       {
         TmaMaps m{};
         MAP_OK(make_map(&m.m[0], dy, d, c.T, d, 128));
@@ -1499,6 +1506,7 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
         if (rc != FOMOE_OK) return rc;
       }
     }
+    if (phase == 0) return FOMOE_OK;
     struct WG { const void* A; int lda; int a_gcol; const void* B; int ldb; int b_gcol; int M, N; void* out; };
     const WG jobs[3] = {{dy, d, 0, aws.sh, ld, Fs, d, Fs, d_sh_down},
                         {sws.dsa, ld, Fs, x, d, 0, Fs, d, silu ? d_sh_up : d_sh_gate},
@@ -1552,6 +1560,17 @@ int umma_ffn_bwd(const fomoe_config& c, int n_res, const void* x, const void* dy
     }
   }
   return FOMOE_OK;
+  };   // phase_fn
+  int rc = phase_fn(0, st_main);
+  if (rc != FOMOE_OK) return rc;
+  cudaStream_t wst = st_main;
+  if (wg_stream && wg_fork) {   // the weight gradients wait for everything queued on the main stream so far (DH and DX)
+    FOMOE_CUDA_OK(cudaEventRecord(wg_fork, st_main));
+    FOMOE_CUDA_OK(cudaStreamWaitEvent(wg_stream, wg_fork, 0));
+    if (wg_forked) *wg_forked = true;
+    wst = wg_stream;
+  }
+  return phase_fn(1, wst);
 }
 
 
